@@ -1,0 +1,233 @@
+/*
+ * evis_oracle.c -- ORACLE.  TEST INFRASTRUCTURE ONLY.
+ *
+ * A plain, slow, single-threaded CPU statement of what the EVIS per-pixel event-synthesis hot
+ * path computes, written from the paper (/root/reference/PAPER.md, arxiv 2607.08098), Sec. 3.2
+ * (HDR event formation, Eq. 3-4, lines 92-104) and Sec. 3.3 (bidirectional motion-vector
+ * warping, Eq. 5-7).  It follows the algorithm step by step in the paper's order
+ * and notation: no tiling, no fusion, no reordering.  It shares NO code with the CUDA path under
+ * paper_2607_08098_b200/csrc and neither includes the other.  Only tests/, the smoke check of
+ * __graft_entry__.py and the cpu_baseline / --impl reference legs of bench.py may call it.
+ *
+ * Precision.  The paper fixes none.  Floating point that DECIDES AN INTEGER (which pixel a
+ * source lands on, which source wins the z-test, how many events fire, the carried reference
+ * level that feeds the next count) is taken in the kernel's precision, IEEE binary32 with the
+ * operation order written below (compile with -ffp-contract=off so that only the fmaf() calls
+ * written here are fused).  The log-luminance is evaluated in binary64 and rounded once to
+ * binary32.  Timestamps decide nothing and are computed in binary64.
+ *
+ * Readings of the paper where it is silent or ambiguous are listed in DESIGN.md ("Readings");
+ * the tag [Rn] below names the reading a line depends on.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 zero motion identity, P2 substep S reproduces
+ * keyframe B, P3 integer translation, P4 8x8 gather-form brute force, P5 analytic two-rectangle
+ * occlusion, P6-P10 event-count / residual / timestamp closed forms.  UNPINNED by paper or
+ * mathematics (fixed by DESIGN.md readings only): log base R1, epsilon R2, initial reference
+ * level R6, nearest-pixel depth lookup R16, hole handling R20, the composite choice R19.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+#define EVO_EMPTY 0xFFFFFFFFFFFFFFFFull
+#define EVO_NONE  0xFFFFFFFFu
+
+typedef struct {
+    int32_t env, x, y;      /* pixel */
+    int32_t p;              /* polarity +1 / -1 */
+    int32_t substep;        /* i in 1..S */
+    int32_t k;              /* 1..n: which crossing inside this substep */
+    int32_t kf;             /* index of the keyframe interval */
+    int32_t pad;
+    double  t_off;          /* seconds from the start of the interval */
+} evo_event;
+
+static uint32_t f32_bits(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
+
+/* ---- Eq. 3 + log -----------------------------------------------------------
+ * I = 0.2126 R + 0.7152 G + 0.0722 B ;  L = log(I + eps), natural log [R1], I clamped at 0 [R3].
+ * binary64, products and sums each rounded (no fma), summed left to right, one rounding to f32. */
+void evo_log_luminance(const float *rad /* [n][3] */, int64_t n, float eps, float *L /* [n] */)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        double r = (double)rad[3 * i + 0], g = (double)rad[3 * i + 1], b = (double)rad[3 * i + 2];
+        double I = (0.2126 * r + 0.7152 * g) + 0.0722 * b;
+        if (!(I > 0.0)) I = 0.0;
+        L[i] = (float)log(I + (double)eps);
+    }
+}
+
+/* ---- Eq. 5-7: splat one keyframe in one direction for one substep ---------
+ * Source pixel p=(x,y) of keyframe X with displacement field `disp` and time weight w moves to
+ *     q = p + w * disp(p)                                                     (Eq. 5)
+ * direction B (src_is_B=1): disp = m_B (backward MV of B), w = 1-f   ->  q_B = p + (1-f) m_B
+ * direction A (src_is_B=0): disp = -m_A (or the explicit forward field), w = f -> q_A = p - f m_A
+ * The other endpoint of the correspondence is p + disp(p); its depth is looked up at the nearest
+ * pixel of the other keyframe [R16], falling back to the source's own depth outside the image.
+ *     Zt = (1-f) Z_A(p_A) + f Z_B(p_B)                                         (Eq. 7)
+ * Every integer pixel with positive bilinear weight is covered [R14]; per target the smallest
+ * (Zt bits, source index) is kept [R15] (Eq. 6: nearest surface only).
+ * zbuf[H*W] must be EVO_EMPTY-initialised by the caller.                                        */
+void evo_splat(int H, int W, int i, int S, int src_is_B,
+               const float *disp /* [H][W][2] */, const float *Zsrc, const float *Zoth,
+               uint64_t *zbuf)
+{
+    const float f = (float)i / (float)S;
+    const float g = 1.0f - f;
+    const float w = src_is_B ? g : f;
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            const int p = y * W + x;
+            const float dx = disp[2 * p + 0], dy = disp[2 * p + 1];
+            const float qx = fmaf(w, dx, (float)x);
+            const float qy = fmaf(w, dy, (float)y);
+            /* depth at the two endpoints of the correspondence */
+            const float ex = (float)x + dx, ey = (float)y + dy;
+            const float jx = floorf(ex + 0.5f), jy = floorf(ey + 0.5f);
+            const float zs = Zsrc[p];
+            float zo = zs;
+            if (jx >= 0.0f && jx <= (float)(W - 1) && jy >= 0.0f && jy <= (float)(H - 1))
+                zo = Zoth[(int)jy * W + (int)jx];
+            const float za = src_is_B ? zo : zs;
+            const float zb = src_is_B ? zs : zo;
+            const float zt = fmaf(f, zb, g * za);
+            if (!(zt > 0.0f) || isinf(zt)) continue;                    /* [R17] */
+            const float x0f = floorf(qx), y0f = floorf(qy);
+            if (!(x0f >= -1.0f && x0f <= (float)(W - 1))) continue;     /* also drops NaN/inf */
+            if (!(y0f >= -1.0f && y0f <= (float)(H - 1))) continue;
+            const int x0 = (int)x0f, y0 = (int)y0f;
+            const int hx = qx > x0f, hy = qy > y0f;     /* positive weight on the +1 neighbour */
+            const uint64_t key = ((uint64_t)f32_bits(zt) << 32) | (uint32_t)p;
+            for (int oy = 0; oy <= hy; ++oy)
+                for (int ox = 0; ox <= hx; ++ox) {
+                    const int tx = x0 + ox, ty = y0 + oy;
+                    if (tx < 0 || tx >= W || ty < 0 || ty >= H) continue;   /* [R18] */
+                    if (key < zbuf[ty * W + tx]) zbuf[ty * W + tx] = key;
+                }
+        }
+}
+
+/* ---- composite -----------------------------------------------------------------
+ * mode 0 [R19]: backward-warped B is primary; forward-warped A fills only B's holes; a pixel
+ * reached by neither keeps its previous value [R20].
+ * mode 1 [R19]: nearest of the two; where both hit the same surface (depths within 1 %) the two
+ * log values are blended with the time weights of Eq. 7: (1-f) L_A* + f L_B*.
+ * Out: Lhat[H*W]; win_dir[H*W] (0 = B, 1 = A, 2 = blend, 3 = hole); win_idx[H*W] source index of
+ * the chosen (mode 1 blend: the B) winner, EVO_NONE for a hole.                                   */
+void evo_composite(int H, int W, int i, int S, int mode,
+                   const uint64_t *zA, const uint64_t *zB, const float *LA, const float *LB,
+                   const float *Lprev, float *Lhat, uint8_t *win_dir, uint32_t *win_idx)
+{
+    const float f = (float)i / (float)S;
+    const float g = 1.0f - f;
+    for (int q = 0; q < H * W; ++q) {
+        const int hasA = zA[q] != EVO_EMPTY, hasB = zB[q] != EVO_EMPTY;
+        const uint32_t ia = (uint32_t)(zA[q] & 0xFFFFFFFFu), ib = (uint32_t)(zB[q] & 0xFFFFFFFFu);
+        float v; uint8_t d; uint32_t idx;
+        if (mode == 0) {
+            if (hasB)      { v = LB[ib]; d = 0; idx = ib; }
+            else if (hasA) { v = LA[ia]; d = 1; idx = ia; }
+            else           { v = Lprev[q]; d = 3; idx = EVO_NONE; }
+        } else {
+            if (hasA && hasB) {
+                float da, db;
+                uint32_t ua = (uint32_t)(zA[q] >> 32), ub = (uint32_t)(zB[q] >> 32);
+                memcpy(&da, &ua, 4); memcpy(&db, &ub, 4);
+                const float lo = da < db ? da : db;
+                if (fabsf(da - db) <= 0.01f * lo) { v = fmaf(f, LB[ib], g * LA[ia]); d = 2; idx = ib; }
+                else if (db < da)                 { v = LB[ib]; d = 0; idx = ib; }
+                else                              { v = LA[ia]; d = 1; idx = ia; }
+            }
+            else if (hasB) { v = LB[ib]; d = 0; idx = ib; }
+            else if (hasA) { v = LA[ia]; d = 1; idx = ia; }
+            else           { v = Lprev[q]; d = 3; idx = EVO_NONE; }
+        }
+        Lhat[q] = v;
+        if (win_dir) win_dir[q] = d;
+        if (win_idx) win_idx[q] = idx;
+    }
+}
+
+/* ---- Eq. 4 + reference update for one frame of one env ------------------------
+ * dL = L - Lref ; n = floor(|dL| / C) ; p = sgn(dL) ; Lref <- Lref + p n C.
+ * C = C+ for dL > 0, C- for dL < 0 [R4]; n capped at 255 [R7]; the k-th crossing of the frame is
+ * stamped by linear interpolation in log intensity between the previous and the current frame
+ * value [R8]: level_k = Lref + p k C, fr = (level_k - Lprev) / (L - Lprev) clamped to [0,1].
+ * Frame i covers ((i-1) T/S, i T/S].  Events are appended in (y, x, k) order.
+ * Returns the number of events this frame produced (all are counted; only those that fit are
+ * stored).                                                                                        */
+int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
+                        float c_pos, float c_neg, const float *Lhat,
+                        float *Lref, float *Lprev,
+                        evo_event *ev, int64_t cap, int64_t n_have)
+{
+    int64_t made = 0;
+    const double dt = (double)T / (double)S;
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            const int q = y * W + x;
+            const float L = Lhat[q];
+            const float d = L - Lref[q];
+            float C; int p;
+            if (d > 0.0f)      { C = c_pos; p = +1; }
+            else if (d < 0.0f) { C = c_neg; p = -1; }
+            else               { C = 1.0f;  p = 0; }
+            int n = 0;
+            if (p != 0) {
+                float r = floorf(fabsf(d) / C);
+                n = r >= 255.0f ? 255 : (int)r;
+            }
+            for (int k = 1; k <= n; ++k) {
+                const float lev = fmaf((float)(p * k), C, Lref[q]);
+                const double den = (double)L - (double)Lprev[q];
+                double fr = 1.0;
+                if (den != 0.0) fr = ((double)lev - (double)Lprev[q]) / den;
+                if (!(fr >= 0.0)) fr = 0.0;
+                if (fr > 1.0) fr = 1.0;
+                if (n_have + made < cap) {
+                    evo_event *o = &ev[n_have + made];
+                    o->env = env; o->x = x; o->y = y; o->p = p; o->substep = i; o->k = k;
+                    o->kf = kf; o->pad = 0;
+                    o->t_off = ((double)(i - 1) + fr) * dt;
+                }
+                ++made;
+            }
+            if (n > 0) Lref[q] = fmaf((float)(p * n), C, Lref[q]);
+            Lprev[q] = L;
+        }
+    return made;
+}
+
+/* ---- one keyframe interval of one env: A -> B, substeps i = 1..S ------------------------------
+ * i < S are the paper's K-1 intermediates (f = i/K); i = S is keyframe B itself [R10].
+ * fwdA: displacement of A's pixels towards B: -m_A or the explicit forward field.
+ * Optional debug outputs, each [S][H*W] or NULL: winners of each direction, composite, Lhat.     */
+int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, float c_pos, float c_neg,
+                     const float *LA, const float *fwdA, const float *ZA,
+                     const float *LB, const float *mB, const float *ZB,
+                     float *Lref, float *Lprev,
+                     uint64_t *zA, uint64_t *zB, float *Lhat,              /* scratch [H*W] each */
+                     evo_event *ev, int64_t cap, int64_t n_have,
+                     uint32_t *dbg_winA, uint32_t *dbg_winB, uint8_t *dbg_dir, uint32_t *dbg_idx,
+                     float *dbg_Lhat, int64_t *holes)
+{
+    const int64_t P = (int64_t)H * W;
+    int64_t made = 0;
+    for (int i = 1; i <= S; ++i) {
+        for (int64_t q = 0; q < P; ++q) { zA[q] = EVO_EMPTY; zB[q] = EVO_EMPTY; }
+        evo_splat(H, W, i, S, 0, fwdA, ZA, ZB, zA);
+        evo_splat(H, W, i, S, 1, mB, ZB, ZA, zB);
+        uint8_t *dd = dbg_dir ? dbg_dir + (int64_t)(i - 1) * P : 0;
+        uint32_t *di = dbg_idx ? dbg_idx + (int64_t)(i - 1) * P : 0;
+        evo_composite(H, W, i, S, mode, zA, zB, LA, LB, Lprev, Lhat, dd, di);
+        for (int64_t q = 0; q < P; ++q) {
+            if (dbg_winA) dbg_winA[(int64_t)(i - 1) * P + q] = zA[q] == EVO_EMPTY ? EVO_NONE : (uint32_t)zA[q];
+            if (dbg_winB) dbg_winB[(int64_t)(i - 1) * P + q] = zB[q] == EVO_EMPTY ? EVO_NONE : (uint32_t)zB[q];
+            if (dbg_Lhat) dbg_Lhat[(int64_t)(i - 1) * P + q] = Lhat[q];
+            if (holes && zA[q] == EVO_EMPTY && zB[q] == EVO_EMPTY) ++*holes;
+        }
+        made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, Lhat, Lref, Lprev,
+                                ev, cap, n_have + made);
+    }
+    return made;
+}

@@ -1,0 +1,166 @@
+"""ctypes front end of the C oracle (oracle/evis_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It shares nothing with the CUDA path; it mirrors the library's call shape
+(first keyframe initialises, every later keyframe closes one interval A -> B) so
+that the parity tests can feed both sides the same keyframes.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Dict, Optional
+
+import numpy as np
+
+from . import build as _build
+
+EVENT_DTYPE = np.dtype([("env", "<i4"), ("x", "<i4"), ("y", "<i4"), ("p", "<i4"), ("substep", "<i4"),
+                        ("k", "<i4"), ("kf", "<i4"), ("pad", "<i4"), ("t_off", "<f8")])
+NONE = 0xFFFFFFFF
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        fp, u64p, u32p, u8p = (C.POINTER(C.c_float), C.POINTER(C.c_uint64), C.POINTER(C.c_uint32),
+                               C.POINTER(C.c_uint8))
+        L.evo_log_luminance.argtypes = [fp, C.c_int64, C.c_float, fp]
+        L.evo_log_luminance.restype = None
+        L.evo_splat.argtypes = [C.c_int] * 5 + [fp, fp, fp, u64p]
+        L.evo_splat.restype = None
+        L.evo_composite.argtypes = [C.c_int] * 5 + [u64p, u64p, fp, fp, fp, fp, u8p, u32p]
+        L.evo_composite.restype = None
+        L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp, fp, C.c_void_p,
+                                                                        C.c_int64, C.c_int64]
+        L.evo_event_frame.restype = C.c_int64
+        L.evo_interval.argtypes = ([C.c_int] * 6 + [C.c_float] * 3 + [fp] * 8 + [u64p, u64p, fp]
+                                   + [C.c_void_p, C.c_int64, C.c_int64]
+                                   + [u32p, u32p, u8p, u32p, fp, C.POINTER(C.c_int64)])
+        L.evo_interval.restype = C.c_int64
+        _lib = L
+    return _lib
+
+
+def _f(a):
+    assert a.dtype == np.float32 and a.flags.c_contiguous
+    return a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
+
+
+def log_luminance(rad: np.ndarray, eps: float) -> np.ndarray:
+    """Eq. 3 + log.  rad [...,3] float32 -> L [...] float32."""
+    rad = np.ascontiguousarray(rad, dtype=np.float32)
+    out = np.empty(rad.shape[:-1], dtype=np.float32)
+    lib().evo_log_luminance(_f(rad), out.size, float(eps), _f(out))
+    return out
+
+
+def splat(i: int, S: int, src_is_B: bool, disp: np.ndarray, Zsrc: np.ndarray, Zoth: np.ndarray
+          ) -> np.ndarray:
+    """Eq. 5-7 for one env, one direction, one substep.  Returns the z-buffer [H,W] uint64."""
+    H, W = Zsrc.shape
+    z = np.full((H, W), 0xFFFFFFFFFFFFFFFF, dtype=np.uint64)
+    lib().evo_splat(H, W, i, S, int(src_is_B), _f(np.ascontiguousarray(disp, np.float32)),
+                    _f(np.ascontiguousarray(Zsrc, np.float32)), _f(np.ascontiguousarray(Zoth, np.float32)),
+                    _p(z, C.c_uint64))
+    return z
+
+
+def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float, T: float,
+                 Lref0: Optional[np.ndarray] = None):
+    """Event stage alone (Eq. 4): feed a sequence of S log frames [S,H,W] to one env.
+
+    Returns (events, Lref_final).  Lref and Lprev start at L0 (or Lref0 for the reference)."""
+    frames = np.ascontiguousarray(frames, np.float32)
+    S, H, W = frames.shape
+    Lprev = np.ascontiguousarray(L0, np.float32).copy()
+    Lref = Lprev.copy() if Lref0 is None else np.ascontiguousarray(Lref0, np.float32).copy()
+    cap = 1 << 16
+    while True:
+        ev = np.zeros(cap, dtype=EVENT_DTYPE)
+        lr, lp = Lref.copy(), Lprev.copy()
+        n = 0
+        for i in range(1, S + 1):
+            n += lib().evo_event_frame(H, W, 0, 0, i, S, float(T), float(c_pos), float(c_neg),
+                                       _f(frames[i - 1]), _f(lr), _f(lp), ev.ctypes.data, cap, n)
+        if n <= cap:
+            return ev[:n], lr
+        cap = int(n)
+
+
+class Oracle:
+    """Stateful oracle over E envs: ``step(keyframe)`` mirrors evis_step."""
+
+    def __init__(self, num_envs: int, height: int, width: int, substeps: int, c_pos: float, c_neg: float,
+                 log_eps: float, keyframe_dt: float, composite_mode: int = 0, debug: bool = False):
+        self.E, self.H, self.W, self.S = num_envs, height, width, substeps
+        self.c_pos, self.c_neg, self.eps, self.T = c_pos, c_neg, log_eps, keyframe_dt
+        self.mode = composite_mode
+        self.debug = debug
+        self.calls = 0
+        self.prev = None
+        self.Lref = None
+        self.Lprev = None
+        self.holes = 0
+        self.dbg: Dict[str, np.ndarray] = {}
+
+    def step(self, rad, mv_bwd, depth, mv_fwd=None) -> np.ndarray:
+        """Consume one keyframe.  The first call initialises (Lref = L, no events) [R6]; every later
+        call returns the events of interval kf = call_index - 1 in (env, substep, y, x, k) order.
+        ``mv_fwd`` is the forward field OF THIS keyframe, used when it plays the role of A in the
+        NEXT call; None = reuse -mv_bwd."""
+        E, H, W, S = self.E, self.H, self.W, self.S
+        rad = np.ascontiguousarray(rad, np.float32).reshape(E, H, W, 3)
+        mB = np.ascontiguousarray(mv_bwd, np.float32).reshape(E, H, W, 2)
+        ZB = np.ascontiguousarray(depth, np.float32).reshape(E, H, W)
+        LB = log_luminance(rad, self.eps)
+        fwd = -mB if mv_fwd is None else np.ascontiguousarray(mv_fwd, np.float32).reshape(E, H, W, 2)
+        fwd = np.ascontiguousarray(fwd)
+        cur = dict(L=LB, m=mB, Z=ZB, fwd=fwd)
+        if self.calls == 0:
+            self.Lref = LB.copy()
+            self.Lprev = LB.copy()
+            self.prev = cur
+            self.calls = 1
+            return np.zeros(0, dtype=EVENT_DTYPE)
+        A = self.prev
+        kf = self.calls - 1
+        P = H * W
+        zA = np.empty(P, np.uint64)
+        zB = np.empty(P, np.uint64)
+        Lhat = np.empty(P, np.float32)
+        if self.debug:
+            self.dbg = dict(winA=np.empty((E, S, H, W), np.uint32), winB=np.empty((E, S, H, W), np.uint32),
+                            dir=np.empty((E, S, H, W), np.uint8), idx=np.empty((E, S, H, W), np.uint32),
+                            Lhat=np.empty((E, S, H, W), np.float32))
+        holes = C.c_int64(0)
+        cap = max(1 << 16, 4 * E * P)
+        while True:
+            ev = np.zeros(cap, dtype=EVENT_DTYPE)
+            Lref, Lprev = self.Lref.copy(), self.Lprev.copy()
+            holes.value = 0
+            n = 0
+            for e in range(E):
+                d = self.dbg
+                n += lib().evo_interval(
+                    H, W, S, self.mode, e, kf, float(self.T), float(self.c_pos), float(self.c_neg),
+                    _f(A["L"][e]), _f(A["fwd"][e]), _f(A["Z"][e]), _f(LB[e]), _f(mB[e]), _f(ZB[e]),
+                    _f(Lref[e]), _f(Lprev[e]), _p(zA, C.c_uint64), _p(zB, C.c_uint64), _f(Lhat),
+                    ev.ctypes.data, cap, n,
+                    _p(d["winA"][e], C.c_uint32) if d else None, _p(d["winB"][e], C.c_uint32) if d else None,
+                    _p(d["dir"][e], C.c_uint8) if d else None, _p(d["idx"][e], C.c_uint32) if d else None,
+                    _f(d["Lhat"][e]) if d else None, C.byref(holes))
+            if n <= cap:
+                break
+            cap = int(n)
+        self.Lref, self.Lprev = Lref, Lprev
+        self.holes = holes.value
+        self.prev = cur
+        self.calls += 1
+        return ev[:n]

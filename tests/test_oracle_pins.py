@@ -1,0 +1,411 @@
+"""Pins for the CPU oracle (oracle/evis_oracle.c): it is checked against what the paper and the
+mathematics fix -- printed constants, closed forms, invariants, special cases and brute force --
+never against itself.  CPU only.  Pin numbers follow SURVEY.md Sec. 8(c) / DESIGN.md.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import evis_oracle as orc
+from paper_2607_08098_b200 import scenes
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+EMPTY = np.uint64(0xFFFFFFFFFFFFFFFF)
+
+
+def _rng(seed):
+    return np.random.default_rng(seed)
+
+
+# ------------------------------------------------------------------------------------------------
+# Eq. 3 + log
+# ------------------------------------------------------------------------------------------------
+def test_rec709_weights_and_log_closed_forms():
+    """PAPER.md:96 prints the weights; L = log(I + eps).  Single-channel inputs
+    isolate each weight (a permuted weight fails), math.log is the independent library routine."""
+    w = {}
+    for line in open(os.path.join(GOLD, "rec709_weights.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()
+        w[k] = float(v)
+    assert abs(w["R"] + w["G"] + w["B"] - 1.0) < 1e-12
+    eps = 1e-3
+    rad = np.array([[1, 0, 0], [0, 1, 0], [0, 0, 1], [1, 1, 1], [0, 0, 0], [2.5, 0.5, 4.0],
+                    [-1.0, 0.0, 0.0]], dtype=np.float32)
+    L = orc.log_luminance(rad, eps)
+    e32 = float(np.float32(eps))
+    exp = [math.log(w["R"] + e32), math.log(w["G"] + e32), math.log(w["B"] + e32),
+           math.log(w["R"] + w["G"] + w["B"] + e32), math.log(e32),
+           math.log(2.5 * w["R"] + 0.5 * w["G"] + 4.0 * w["B"] + e32),
+           math.log(e32)]                      # negative luminance clamps to 0 (reading R3)
+    for got, want in zip(L, exp):
+        assert got == np.float32(want) or abs(float(got) - want) <= 2.0 ** -23 * abs(want)
+
+
+def test_log_is_natural_log_of_linear_radiance():
+    """exp(L) - eps recovers I: pins log base e (R1) against a wrong base and a missing eps."""
+    r = _rng(1)
+    rad = (10.0 ** r.uniform(-3, 3, size=(1000, 3))).astype(np.float32)
+    L = orc.log_luminance(rad, 1e-3).astype(np.float64)
+    I = 0.2126 * rad[:, 0].astype(np.float64) + 0.7152 * rad[:, 1] + 0.0722 * rad[:, 2]
+    assert np.allclose(np.exp(L) - np.float32(1e-3), I, rtol=2e-6, atol=1e-8)  # L is rounded to binary32
+
+
+# ------------------------------------------------------------------------------------------------
+# helpers to drive the warp on hand-made keyframes
+# ------------------------------------------------------------------------------------------------
+def _oracle(E, H, W, S, c=0.2, mode=0, T=1.0 / 60, eps=1e-3, cn=None):
+    return orc.Oracle(E, H, W, S, c, c if cn is None else cn, eps, T, composite_mode=mode, debug=True)
+
+
+def _rad_from_L(L, eps=1e-3):
+    """Grey radiance whose log-luminance is (close to) L: only used to feed Oracle.step."""
+    I = np.exp(L.astype(np.float64)) - eps
+    return np.repeat(I[..., None], 3, axis=-1).astype(np.float32)
+
+
+# ------------------------------------------------------------------------------------------------
+# P1: zero motion, A = B
+# ------------------------------------------------------------------------------------------------
+def test_p1_zero_motion_is_identity_and_static_scene_is_silent():
+    r = _rng(2)
+    H, W, S = 13, 17, 5
+    rad = (10.0 ** r.uniform(-2, 2, size=(1, H, W, 3))).astype(np.float32)
+    depth = r.uniform(1, 9, size=(1, H, W)).astype(np.float32)
+    mv = np.zeros((1, H, W, 2), np.float32)
+    o = _oracle(1, H, W, S)
+    assert len(o.step(rad, mv, depth)) == 0
+    ev = o.step(rad, mv, depth)
+    own = np.arange(H * W, dtype=np.uint32).reshape(H, W)
+    L = orc.log_luminance(rad, 1e-3)[0]
+    for i in range(S):
+        assert np.array_equal(o.dbg["winA"][0, i], own)
+        assert np.array_equal(o.dbg["winB"][0, i], own)
+        assert np.array_equal(o.dbg["dir"][0, i], np.zeros((H, W), np.uint8))   # B is primary
+        assert np.array_equal(o.dbg["Lhat"][0, i], L)
+    assert len(ev) == 0 and o.holes == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# P2: f = 1 reproduces keyframe B for ANY motion field (Eq. 5: q_B = p at f = 1)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [0])
+def test_p2_last_substep_reproduces_keyframe_b(mode):
+    r = _rng(3)
+    H, W, S = 16, 21, 7
+    o = _oracle(1, H, W, S, mode=mode)
+    for _ in range(3):
+        rad = (10.0 ** r.uniform(-2, 2, size=(1, H, W, 3))).astype(np.float32)
+        depth = r.uniform(0.5, 9, size=(1, H, W)).astype(np.float32)
+        mv = r.uniform(-6, 6, size=(1, H, W, 2)).astype(np.float32)
+        o.step(rad, mv, depth)
+    own = np.arange(H * W, dtype=np.uint32).reshape(H, W)
+    assert np.array_equal(o.dbg["winB"][0, S - 1], own)
+    assert np.array_equal(o.dbg["Lhat"][0, S - 1], orc.log_luminance(rad, 1e-3)[0])
+    assert np.array_equal(o.Lprev[0], orc.log_luminance(rad, 1e-3)[0])
+
+
+# ------------------------------------------------------------------------------------------------
+# P3: integer-pixel translation warps exactly (signs of Eq. 5 in both directions, A-fill)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("d", [(1, 0), (-2, 1), (0, -1), (3, 2)])
+def test_p3_integer_translation_warps_exactly(d):
+    H, W, S = 20, 24, 4                      # S a power of two: i/S exact in binary32
+    dx, dy = d
+    r = _rng(4)
+    big = r.uniform(-3, 3, size=(H + 64, W + 64)).astype(np.float32)   # texture on an infinite plane
+
+    def tex(px, py):                          # log value of the surface point under pixel (x,y)
+        ys, xs = np.mgrid[0:H, 0:W]
+        return big[ys - py + 32, xs - px + 32]
+
+    LA, LB = tex(0, 0), tex(S * dx, S * dy)   # surface moved by D = S d between the keyframes
+    mv = np.empty((1, H, W, 2), np.float32)
+    mv[..., 0], mv[..., 1] = -S * dx, -S * dy            # backward MV: where it was in A
+    depth = np.full((1, H, W), 3.0, np.float32)
+    z64 = {}
+    for i in range(1, S + 1):
+        zA = orc.splat(i, S, False, -mv[0], depth[0], depth[0])
+        zB = orc.splat(i, S, True, mv[0], depth[0], depth[0])
+        z64[i] = (zA, zB)
+        want = tex(i * dx, i * dy)
+        ys, xs = np.mgrid[0:H, 0:W]
+        # B covers q iff its source q + (S-i) d lies inside; A iff q - i d lies inside
+        sbx, sby = xs + (S - i) * dx, ys + (S - i) * dy
+        sax, say = xs - i * dx, ys - i * dy
+        inB = (sbx >= 0) & (sbx < W) & (sby >= 0) & (sby < H)
+        inA = (sax >= 0) & (sax < W) & (say >= 0) & (say < H)
+        assert np.array_equal(zB != EMPTY, inB)
+        assert np.array_equal(zA != EMPTY, inA)
+        assert np.array_equal((zB & np.uint64(0xFFFFFFFF))[inB], (sby * W + sbx)[inB].astype(np.uint64))
+        assert np.array_equal((zA & np.uint64(0xFFFFFFFF))[inA], (say * W + sax)[inA].astype(np.uint64))
+        got = np.where(inB, LB.ravel()[np.clip(sby * W + sbx, 0, H * W - 1)],
+                       LA.ravel()[np.clip(say * W + sax, 0, H * W - 1)])
+        assert np.array_equal(got[inA | inB], want[inA | inB])
+
+
+def test_p3b_composite_through_the_full_interval():
+    """Same translation, driven through Oracle.step: Lhat equals the analytic frame wherever either
+    keyframe sees the surface; the rest are holes that hold the previous value."""
+    H, W, S, dx, dy = 18, 22, 4, 2, -1
+    r = _rng(5)
+    big = r.uniform(-3, 3, size=(H + 64, W + 64)).astype(np.float32)
+    ys, xs = np.mgrid[0:H, 0:W]
+    tex = lambda px, py: big[ys - py + 32, xs - px + 32]
+    o = _oracle(1, H, W, S)
+    mv = np.empty((1, H, W, 2), np.float32)
+    mv[..., 0], mv[..., 1] = -S * dx, -S * dy
+    depth = np.full((1, H, W), 3.0, np.float32)
+    radA, radB = _rad_from_L(tex(0, 0))[None], _rad_from_L(tex(S * dx, S * dy))[None]
+    LA, LB = orc.log_luminance(radA, 1e-3)[0], orc.log_luminance(radB, 1e-3)[0]
+    o.step(radA, mv, depth)
+    o.step(radB, mv, depth)
+    prev = LA
+    for i in range(1, S + 1):
+        sbx, sby = xs + (S - i) * dx, ys + (S - i) * dy
+        sax, say = xs - i * dx, ys - i * dy
+        inB = (sbx >= 0) & (sbx < W) & (sby >= 0) & (sby < H)
+        inA = (sax >= 0) & (sax < W) & (say >= 0) & (say < H)
+        want = np.where(inB, LB.ravel()[np.clip(sby * W + sbx, 0, H * W - 1)],
+                        np.where(inA, LA.ravel()[np.clip(say * W + sax, 0, H * W - 1)], prev))
+        assert np.array_equal(o.dbg["Lhat"][0, i - 1], want)
+        assert np.array_equal(o.dbg["dir"][0, i - 1], np.where(inB, 0, np.where(inA, 1, 3)))
+        prev = want
+
+
+# ------------------------------------------------------------------------------------------------
+# P4: 8x8 brute force, gather form, straight from the definition of S(q) (Eq. 6)
+# ------------------------------------------------------------------------------------------------
+def _brute_winner(H, W, i, S, src_is_B, disp, Zsrc, Zoth):
+    """For every target enumerate all sources; a source covers the target iff its landing point is
+    strictly within 1 px of it in x and in y (positive bilinear weight); lexicographic min of
+    (Zt, source index).  Inputs are dyadic so every product / sum below is exact in float64."""
+    f = i / S
+    w = (1 - f) if src_is_B else f
+    out = np.full((H, W), -1, dtype=np.int64)
+    for ty in range(H):
+        for tx in range(W):
+            best = None
+            for sy in range(H):
+                for sx in range(W):
+                    dx, dy = float(disp[sy, sx, 0]), float(disp[sy, sx, 1])
+                    qx, qy = sx + w * dx, sy + w * dy
+                    if not (abs(qx - tx) < 1 and abs(qy - ty) < 1):
+                        continue
+                    jx, jy = math.floor(sx + dx + 0.5), math.floor(sy + dy + 0.5)
+                    zs = float(Zsrc[sy, sx])
+                    zo = float(Zoth[jy, jx]) if (0 <= jx < W and 0 <= jy < H) else zs
+                    za, zb = (zo, zs) if src_is_B else (zs, zo)
+                    zt = (1 - f) * za + f * zb
+                    cand = (zt, sy * W + sx)
+                    if best is None or cand < best:
+                        best = cand
+            if best is not None:
+                out[ty, tx] = best[1]
+    return out
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_p4_bruteforce_splat_winners_8x8(seed):
+    H = W = 8
+    S = 4
+    r = _rng(100 + seed)
+    levels = np.array([1.0, 1.5, 2.0, 3.0, 6.0], np.float32)       # many depth ties
+    for src_is_B in (True, False):
+        disp = (r.integers(-12, 13, size=(H, W, 2)) / 4.0).astype(np.float32)   # multiples of 1/4 px
+        Zsrc = levels[r.integers(0, len(levels), size=(H, W))]
+        Zoth = levels[r.integers(0, len(levels), size=(H, W))]
+        for i in range(1, S + 1):
+            z = orc.splat(i, S, src_is_B, disp, Zsrc, Zoth)
+            got = np.where(z == EMPTY, -1, (z & np.uint64(0xFFFFFFFF)).astype(np.int64))
+            want = _brute_winner(H, W, i, S, src_is_B, disp, Zsrc, Zoth)
+            assert np.array_equal(got, want), (seed, src_is_B, i)
+
+
+def test_p4b_interpolated_depth_is_eq7():
+    """One source, different depth in A and B: the stored key carries (1-f) Z_A + f Z_B."""
+    H = W = 4
+    S = 4
+    Zb = np.full((H, W), 2.0, np.float32)
+    Za = np.full((H, W), 6.0, np.float32)
+    disp = np.zeros((H, W, 2), np.float32)
+    for i in range(1, S + 1):
+        z = orc.splat(i, S, True, disp, Zb, Za)
+        zt = (z >> np.uint64(32)).astype(np.uint32).view(np.float32)
+        assert np.all(zt == np.float32((1 - i / S) * 6.0 + (i / S) * 2.0))
+        z = orc.splat(i, S, False, disp, Za, Zb)     # direction A: source depth is Z_A
+        zt = (z >> np.uint64(32)).astype(np.uint32).view(np.float32)
+        assert np.all(zt == np.float32((1 - i / S) * 6.0 + (i / S) * 2.0))
+
+
+def test_tie_break_gives_ceil_shift():
+    """tests/golden/tie_break_ceil.txt (derivation there): constant-depth row shifted by delta."""
+    H, W = 1, 32
+    Z = np.full((H, W), 2.0, np.float32)
+    for line in open(os.path.join(GOLD, "tie_break_ceil.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        delta, shift = float(line.split()[0]), int(line.split()[1])
+        disp = np.zeros((H, W, 2), np.float32)
+        disp[..., 0] = delta
+        z = orc.splat(4, 4, False, disp, Z, Z)           # direction A at f = 1: q = p + delta
+        idx = (z & np.uint64(0xFFFFFFFF)).astype(np.int64)[0]
+        for t in range(W):
+            src = t - shift
+            if 0 <= src < W:
+                assert z[0, t] != EMPTY and idx[t] == src, (delta, t)
+
+
+# ------------------------------------------------------------------------------------------------
+# P5: two overlapping rectangles at different depths: nearest wins, compare with the analytic render
+# ------------------------------------------------------------------------------------------------
+def test_p5_occlusion_matches_analytic_render():
+    spec = scenes.SceneSpec("p5", 1, 64, 80, 2, 1.0 / 60.0, 8, 0.2, 0.2)
+    lo = hi = 1.0
+    mk = lambda depth, x0, y0, w, h, vx, vy, base, tid: scenes.Obj(
+        0, depth, x0, y0, w, h, vx, vy, scenes.TEX_FLAT, 8, base, [1.0, 1.0, 1.0], lo, hi, tex_id=tid)
+    objs = [mk(10.0, -1e6, -1e6, 4e6, 4e6, 0.0, 0.0, 0.05, 0),
+            mk(6.0, 10.0, 12.0, 40.0, 30.0, 200.0, -90.0, 1.0, 1),      # far rectangle
+            mk(2.0, 40.0, 20.0, 25.0, 28.0, -260.0, 120.0, 20.0, 2)]    # near rectangle crosses it
+    sc = scenes.Scene(spec, [objs], [0.0])
+    k0 = scenes.render_keyframe(sc, 0)
+    k1 = scenes.render_keyframe(sc, 1)
+    o = _oracle(1, spec.height, spec.width, spec.substeps)
+    o.step(k0["rad"].numpy(), k0["mv_bwd"].numpy(), k0["depth"].numpy(), k0["mv_fwd"].numpy())
+    o.step(k1["rad"].numpy(), k1["mv_bwd"].numpy(), k1["depth"].numpy(), k1["mv_fwd"].numpy())
+    S, T = spec.substeps, spec.keyframe_dt
+    worst = 1.0
+    for i in range(1, S + 1):
+        gt = scenes.render_at(sc, (i / S) * T)
+        Lgt = orc.log_luminance(gt["rad"].numpy(), 1e-3)[0]
+        got = o.dbg["Lhat"][0, i - 1]
+        bad = got != Lgt
+        # every disagreement must sit within 2 px of a depth silhouette of the true frame
+        d = gt["depth"].numpy()[0]
+        edge = np.zeros_like(bad)
+        for sy in range(-2, 3):
+            for sx in range(-2, 3):
+                sh = np.roll(np.roll(d, sy, 0), sx, 1)
+                edge |= sh != d
+        assert not np.any(bad & ~edge), f"substep {i}: mismatch away from silhouettes"
+        worst = min(worst, 1.0 - bad.mean())
+    assert worst > 0.97
+    # where both rectangles overlap in the true frame the near one (base 20) is what is seen
+    gt = scenes.render_at(sc, 0.5 * T)
+    assert o.holes < 0.02 * S * spec.height * spec.width
+
+
+# ------------------------------------------------------------------------------------------------
+# event stage alone: P6-P10 + hand-worked fixture
+# ------------------------------------------------------------------------------------------------
+def test_event_model_hand_worked_fixture():
+    frames, evs, lref = [], [], None
+    for line in open(os.path.join(GOLD, "event_model_by_hand.txt")):
+        if line.startswith("frames"):
+            frames = [float(v) for v in line.split()[1:]]
+        elif line.startswith("events"):
+            _, i, p, t = line.split()
+            evs.append((int(i), int(p), float(t)))
+        elif line.startswith("lref_final"):
+            lref = float(line.split()[1])
+    fr = np.array(frames, np.float32).reshape(len(frames), 1, 1)
+    ev, lr = orc.event_frames(fr, np.array([[1.0]], np.float32), 0.25, 0.5, 1.0)
+    assert [(int(e["substep"]), int(e["p"])) for e in ev] == [(i, p) for i, p, _ in evs]
+    assert np.allclose([e["t_off"] for e in ev], [t for _, _, t in evs], atol=1e-12)
+    assert float(lr[0, 0]) == lref
+
+
+@pytest.mark.parametrize("splits", [1, 2, 5, 16, 33])
+def test_p6_monotone_total_is_independent_of_substep_split(splits):
+    """Monotone L: total count = floor(|L_end - L_0| / C) however the path is cut (Eq. 4 + update).
+    Dyadic C and endpoints keep binary32 exact so the closed form is exact."""
+    C = 0.125
+    L0 = np.float32(-1.0)
+    for total in (0.0625, 0.125, 0.9375, 3.0, 5.4375):
+        for sign in (+1, -1):
+            Lend = L0 + np.float32(sign * total)
+            frames = (L0 + (Lend - L0) * (np.arange(1, splits + 1, dtype=np.float64) / splits))
+            frames = frames.astype(np.float32).reshape(splits, 1, 1)
+            frames[-1] = Lend
+            ev, lr = orc.event_frames(frames, np.array([[L0]], np.float32), C, C, 1.0)
+            assert len(ev) == math.floor(total / C)
+            assert all(int(e["p"]) == sign for e in ev)
+
+
+def test_p6b_ramp_of_k_plus_half_thresholds_gives_k_events():
+    C = 0.2
+    for k in range(0, 12):
+        for sign in (+1, -1):
+            frames = np.array([sign * (k + 0.5) * C], np.float32).reshape(1, 1, 1)
+            ev, lr = orc.event_frames(frames, np.zeros((1, 1), np.float32), C, C, 1.0)
+            assert len(ev) == k and all(int(e["p"]) == sign for e in ev)
+
+
+def test_p7_residual_bounds_and_reconstruction():
+    r = _rng(7)
+    S, H, W = 40, 6, 7
+    cp, cn = 0.2, 0.3
+    frames = np.cumsum(r.normal(0, 0.4, size=(S, H, W)), axis=0).astype(np.float32)
+    L0 = np.zeros((H, W), np.float32)
+    lref, lprev = L0.copy(), L0.copy()
+    npos = np.zeros((H, W), int)
+    nneg = np.zeros((H, W), int)
+    for i in range(S):
+        ev, lref = orc.event_frames(frames[i:i + 1], lprev, cp, cn, 1.0, Lref0=lref)
+        lprev = frames[i]
+        d = frames[i] - lref
+        assert np.all(d < cp + 1e-5) and np.all(d > -cn - 1e-5)       # sub-threshold residual kept
+        for e in ev:
+            (npos if e["p"] > 0 else nneg)[e["y"], e["x"]] += 1
+    recon = L0 + cp * npos - cn * nneg
+    assert np.all(np.abs(frames[-1] - recon) < max(cp, cn) + 1e-4)
+    assert np.allclose(lref, recon, atol=1e-4)
+
+
+def test_p8_linear_ramp_timestamps():
+    """L(t) = r t sampled at S frames: k-th event at t = k C / r (timestamps linear in L, R8)."""
+    C, r, S, T = 0.2, 37.0, 16, 1.0 / 60.0
+    frames = np.array([r * (i / S) * T for i in range(1, S + 1)], np.float32).reshape(S, 1, 1)
+    ev, _ = orc.event_frames(frames, np.zeros((1, 1), np.float32), C, C, T)
+    n = math.floor(r * T / C)
+    assert len(ev) == n
+    for k, e in enumerate(ev, start=1):
+        assert abs(e["t_off"] - k * np.float32(C) / r) < 2e-8
+
+
+def test_p9_timestamps_ordered_and_inside_their_substep():
+    r = _rng(9)
+    S, H, W, T = 12, 5, 5, 1.0 / 30.0
+    frames = np.cumsum(r.normal(0, 0.5, size=(S, H, W)), axis=0).astype(np.float32)
+    ev, _ = orc.event_frames(frames, np.zeros((H, W), np.float32), 0.2, 0.3, T)
+    assert len(ev) > 100
+    dt = T / S
+    last = {}
+    for e in ev:
+        i = int(e["substep"])
+        assert (i - 1) * dt - 1e-12 <= e["t_off"] <= i * dt + 1e-12
+        key = (int(e["x"]), int(e["y"]))
+        assert e["t_off"] >= last.get(key, -1.0)
+        last[key] = e["t_off"]
+
+
+def test_p10_up_then_down_with_asymmetric_thresholds():
+    cp, cn = 0.25, 0.5
+    D = np.float32(1.1875)                       # dyadic: 4 ON events, residual 0.1875
+    frames = np.array([D, 0.0], np.float32).reshape(2, 1, 1)
+    ev, lr = orc.event_frames(frames, np.zeros((1, 1), np.float32), cp, cn, 1.0)
+    on = [e for e in ev if e["p"] > 0]
+    off = [e for e in ev if e["p"] < 0]
+    assert len(on) == math.floor(D / cp) == 4
+    r_on = D - 4 * cp
+    assert len(off) == math.floor((D - r_on) / cn) == 2
+    assert float(lr[0, 0]) == 4 * cp - 2 * cn
+
+
+def test_event_count_cap_255():
+    frames = np.array([100.0], np.float32).reshape(1, 1, 1)
+    ev, lr = orc.event_frames(frames, np.zeros((1, 1), np.float32), 0.125, 0.125, 1.0)
+    assert len(ev) == 255 and float(lr[0, 0]) == 255 * 0.125
