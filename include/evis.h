@@ -1,0 +1,149 @@
+/*
+ * evis.h -- C ABI of the EVIS per-pixel event-synthesis hot path on B200 (sm_100a).
+ *
+ * What the library computes is defined by the paper (arxiv 2607.08098; /root/reference/PAPER.md):
+ *   Sec. 3.2, Eq. 3-4 (lines 92-104): Rec.709 luminance, L = log(I + eps), contrast-threshold
+ *            event count n = floor(|dL|/C), polarity, reference update L_ref += p n C;
+ *   Sec. 3.3, Eq. 5-7 (lines 106-131): bidirectional motion-vector warping of keyframes A and B
+ *            with z-buffered depth splatting, B primary / A fills holes (line 129).
+ * Readings of silent or ambiguous points: DESIGN.md Sec. 2 (R1-R24).
+ *
+ * Conventions.  E environments, H x W pixels, S substeps per keyframe interval (S = the paper's
+ * upsampling factor K).  Pixel (x, y) has its centre at integer coordinates, x right, y down.
+ * All image tensors are dense, row-major, env-major: index ((e*H + y)*W + x)*C + c.
+ * Motion vectors are in pixels: mv_bwd[p] is the displacement from pixel p of this keyframe to
+ * the same surface point in the PREVIOUS keyframe.
+ *
+ * Threading: a context may be used by one host thread at a time.  No function throws or aborts;
+ * every function returns an evis_status (0 = OK, negative = error).
+ */
+#ifndef EVIS_H_
+#define EVIS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct evis_ctx evis_ctx;       /* opaque; owned by the library */
+
+typedef enum {
+    EVIS_OK               =  0,
+    EVIS_ERR_INVALID_ARG  = -1,   /* NULL pointer, non-positive size, threshold <= 0, ... */
+    EVIS_ERR_CUDA         = -2,   /* a CUDA call failed; evis_last_cuda_error() has the code */
+    EVIS_ERR_OOM          = -3,   /* device allocation failed */
+    EVIS_ERR_OVERFLOW     = -4,   /* more events than event_capacity: the count returned is the
+                                     true count, the stored stream is an incomplete prefix */
+    EVIS_ERR_MOTION_BOUND = -5,   /* a motion vector exceeded max_motion_px on the tile path */
+    EVIS_ERR_BAD_STATE    = -6    /* call order violated (e.g. read before any step) */
+} evis_status;
+
+enum { EVIS_PATH_AUTO = 0, EVIS_PATH_GLOBAL = 1, EVIS_PATH_TILE = 2 };
+enum { EVIS_COMPOSITE_B_PRIMARY = 0, EVIS_COMPOSITE_BLEND = 1 };
+
+typedef struct {
+    int32_t  num_envs, height, width;   /* E, H, W  (> 0; H, W <= 32767; E <= 65535)            */
+    int32_t  substeps;                  /* S in 1..255 (K)                         */
+    float    c_pos, c_neg;              /* contrast thresholds C+, C- (> 0)  (Eq. 4, R4)         */
+    float    log_eps;                   /* eps of L = log(I + eps) (> 0)     (R2)   */
+    float    keyframe_dt;               /* T = 1/f_k in seconds (> 0)                            */
+    float    max_motion_px;             /* bound on |mv| (infinity norm) the caller guarantees;
+                                           0 = unknown -> global z-buffer path                   */
+    int32_t  composite_mode;            /* EVIS_COMPOSITE_*  (R19)                 */
+    int32_t  path;                      /* EVIS_PATH_*                                           */
+    int32_t  device;                    /* CUDA device ordinal                                   */
+    uint64_t event_capacity;            /* events stored per step (16 B each), > 0               */
+    int32_t  debug_capture;             /* 1: keep, for every substep of the last step, the
+                                           composite winner and the warped log frame (test hook;
+                                           costs 9 B per pixel-substep of device memory)         */
+    int32_t  reserved;
+} evis_config;
+
+/* One event, 16 bytes.  Absolute time = kf * T + t_off (form it in double).            (a7, R8) */
+typedef struct {
+    uint16_t x, y;          /* pixel                                                             */
+    uint16_t env;           /* environment                                                       */
+    int8_t   p;             /* polarity +1 / -1            (Eq. 4)                               */
+    uint8_t  substep;       /* i in 1..S: the frame at which the crossing was detected           */
+    float    t_off;         /* seconds from the start of the interval, in ((i-1) T/S, i T/S]     */
+    uint32_t kf;            /* index of the keyframe interval (0 = between keyframes 0 and 1)    */
+} evis_event;
+
+typedef struct {
+    int32_t  path;              /* EVIS_PATH_GLOBAL or EVIS_PATH_TILE actually used              */
+    int32_t  tile_w, tile_h;    /* ordering tile of the event stream                             */
+    int32_t  halo;              /* tile path: halo in pixels                                     */
+    uint64_t steps;             /* evis_step calls so far                                        */
+    uint64_t last_events;       /* true event count of the last step                             */
+    uint64_t last_holes;        /* pixel-substeps of the last step reached by neither keyframe   */
+    uint64_t kernel_launches;   /* kernels + memsets this library launched since creation        */
+    int32_t  last_overflow;     /* 1 if the last step overflowed event_capacity                  */
+    int32_t  last_motion_violation; /* 1 if a motion vector exceeded the tile-path bound         */
+    uint64_t device_bytes;      /* device memory owned by the context                            */
+} evis_info;
+
+/* Create a context: validates the configuration, allocates all device state.  *out is set only
+ * on success.  Errors: INVALID_ARG, CUDA, OOM. */
+int evis_create(const evis_config *cfg, evis_ctx **out);
+
+/* Consume one keyframe (all DEVICE pointers, float32, read-only, caller-owned; they may be
+ * freed or overwritten as soon as the work enqueued by this call has run on `cuda_stream`):
+ *   rad    [E,H,W,3] scene-linear radiance R,G,B
+ *   mv_bwd [E,H,W,2] backward motion vectors of this keyframe, pixels
+ *   mv_fwd [E,H,W,2] or NULL: displacement of this keyframe's pixels towards the NEXT keyframe,
+ *          used when this keyframe plays the role of A in the next call; NULL = the paper's
+ *          default, -mv_bwd (R12)
+ *   depth  [E,H,W]   depth, finite and > 0                (R17)
+ * The first call only initialises (L_ref = L, R6) and emits no events.  Every later call closes
+ * the interval kf = (call index - 1): warps A (previous keyframe) and B (this one) to the S
+ * substeps (Eq. 5-7), runs the event model on every substep (Eq. 4), appends the events to the
+ * context's device stream in deterministic order, carries L_ref forward and makes B the new A.
+ * `cuda_stream` is a cudaStream_t (NULL = default stream).  The call is asynchronous unless
+ * `n_events` (HOST pointer, nullable) is given: then it synchronises the stream and stores the
+ * true number of events of this step.  Errors: INVALID_ARG, CUDA; with n_events also OVERFLOW
+ * and MOTION_BOUND (the state has advanced regardless). */
+int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd,
+              const float *depth, void *cuda_stream, uint64_t *n_events);
+
+/* Same step with HOST buffers (pageable or pinned): copies them to device staging owned by the
+ * context on the context's own stream, runs the step and synchronises.  n_events nullable. */
+int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd,
+                   const float *depth, uint64_t *n_events);
+
+/* Copy the events of the last step, in the deterministic order
+ * (env, substep, tile row, tile column, y, x, crossing k), to `dst` (room for `max` events;
+ * device pointer if dst_is_device != 0, else host).  Synchronises.  *n_out = events copied
+ * (= min(true count, capacity, max)).  Errors: INVALID_ARG, BAD_STATE, CUDA. */
+int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t max, uint64_t *n_out);
+
+/* Device pointer to the ordered stream of the last step and its stored length (no copy);
+ * valid until the next evis_step on the same context. */
+int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_stored);
+
+/* Counters and geometry (synchronises the last step's stream). */
+int evis_get_info(evis_ctx *ctx, evis_info *info);
+
+/* State access for tests and checkpointing: the carried reference level L_ref and the last
+ * warped log frame L_prev, each [E,H,W] float32, to/from HOST memory.  Either may be NULL. */
+int evis_get_state(evis_ctx *ctx, float *l_ref, float *l_prev);
+int evis_set_state(evis_ctx *ctx, const float *l_ref, const float *l_prev);
+
+/* Test hook (needs debug_capture = 1): for the last step, per substep i-1 in [0,S), per pixel:
+ *   win   [S,E,H,W] uint32: source linear index y*W+x of the composite winner, 0xFFFFFFFF = hole
+ *   dir   [S,E,H,W] uint8 : 0 = from B, 1 = from A, 2 = blend (mode 1), 3 = hole
+ *   l_hat [S,E,H,W] float32: the warped log frame
+ * HOST pointers, each nullable. */
+int evis_debug_read(evis_ctx *ctx, uint32_t *win, uint8_t *dir, float *l_hat);
+
+/* Release everything.  NULL is accepted. */
+int evis_destroy(evis_ctx *ctx);
+
+const char *evis_strerror(int status);
+int         evis_last_cuda_error(const evis_ctx *ctx);   /* cudaError_t of the last failure */
+const char *evis_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EVIS_H_ */

@@ -159,7 +159,8 @@ void evo_composite(int H, int W, int i, int S, int mode,
 int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
                         float c_pos, float c_neg, const float *Lhat,
                         float *Lref, float *Lprev,
-                        evo_event *ev, int64_t cap, int64_t n_have)
+                        evo_event *ev, int64_t cap, int64_t n_have,
+                        float *dbg_dL /* [H*W] or NULL: dL = L - Lref before the update */)
 {
     int64_t made = 0;
     const double dt = (double)T / (double)S;
@@ -168,6 +169,7 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
             const int q = y * W + x;
             const float L = Lhat[q];
             const float d = L - Lref[q];
+            if (dbg_dL) dbg_dL[q] = d;
             float C; int p;
             if (d > 0.0f)      { C = c_pos; p = +1; }
             else if (d < 0.0f) { C = c_neg; p = -1; }
@@ -209,7 +211,7 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, fl
                      uint64_t *zA, uint64_t *zB, float *Lhat,              /* scratch [H*W] each */
                      evo_event *ev, int64_t cap, int64_t n_have,
                      uint32_t *dbg_winA, uint32_t *dbg_winB, uint8_t *dbg_dir, uint32_t *dbg_idx,
-                     float *dbg_Lhat, int64_t *holes)
+                     float *dbg_Lhat, float *dbg_dL, int64_t *holes)
 {
     const int64_t P = (int64_t)H * W;
     int64_t made = 0;
@@ -227,7 +229,7 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, fl
             if (holes && zA[q] == EVO_EMPTY && zB[q] == EVO_EMPTY) ++*holes;
         }
         made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, Lhat, Lref, Lprev,
-                                ev, cap, n_have + made);
+                                ev, cap, n_have + made, dbg_dL ? dbg_dL + (int64_t)(i - 1) * P : 0);
     }
     return made;
 }

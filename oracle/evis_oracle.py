@@ -34,11 +34,11 @@ def lib():
         L.evo_composite.argtypes = [C.c_int] * 5 + [u64p, u64p, fp, fp, fp, fp, u8p, u32p]
         L.evo_composite.restype = None
         L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp, fp, C.c_void_p,
-                                                                        C.c_int64, C.c_int64]
+                                                                        C.c_int64, C.c_int64, fp]
         L.evo_event_frame.restype = C.c_int64
         L.evo_interval.argtypes = ([C.c_int] * 6 + [C.c_float] * 3 + [fp] * 8 + [u64p, u64p, fp]
                                    + [C.c_void_p, C.c_int64, C.c_int64]
-                                   + [u32p, u32p, u8p, u32p, fp, C.POINTER(C.c_int64)])
+                                   + [u32p, u32p, u8p, u32p, fp, fp, C.POINTER(C.c_int64)])
         L.evo_interval.restype = C.c_int64
         _lib = L
     return _lib
@@ -88,7 +88,7 @@ def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float,
         n = 0
         for i in range(1, S + 1):
             n += lib().evo_event_frame(H, W, 0, 0, i, S, float(T), float(c_pos), float(c_neg),
-                                       _f(frames[i - 1]), _f(lr), _f(lp), ev.ctypes.data, cap, n)
+                                       _f(frames[i - 1]), _f(lr), _f(lp), ev.ctypes.data, cap, n, None)
         if n <= cap:
             return ev[:n], lr
         cap = int(n)
@@ -138,7 +138,7 @@ class Oracle:
         if self.debug:
             self.dbg = dict(winA=np.empty((E, S, H, W), np.uint32), winB=np.empty((E, S, H, W), np.uint32),
                             dir=np.empty((E, S, H, W), np.uint8), idx=np.empty((E, S, H, W), np.uint32),
-                            Lhat=np.empty((E, S, H, W), np.float32))
+                            Lhat=np.empty((E, S, H, W), np.float32), dL=np.empty((E, S, H, W), np.float32))
         holes = C.c_int64(0)
         cap = max(1 << 16, 4 * E * P)
         while True:
@@ -155,7 +155,7 @@ class Oracle:
                     ev.ctypes.data, cap, n,
                     _p(d["winA"][e], C.c_uint32) if d else None, _p(d["winB"][e], C.c_uint32) if d else None,
                     _p(d["dir"][e], C.c_uint8) if d else None, _p(d["idx"][e], C.c_uint32) if d else None,
-                    _f(d["Lhat"][e]) if d else None, C.byref(holes))
+                    _f(d["Lhat"][e]) if d else None, _f(d["dL"][e]) if d else None, C.byref(holes))
             if n <= cap:
                 break
             cap = int(n)

@@ -1,0 +1,216 @@
+"""Thin ctypes binding of the C ABI in include/evis.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libevis.so.  There is NO CPU fallback: if the
+library is missing or does not load, importing a symbol from it raises.  PyTorch is used for device
+memory and streams (tensors in, tensors out).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libevis.so")
+
+EVIS_OK = 0
+EVIS_ERR_INVALID_ARG, EVIS_ERR_CUDA, EVIS_ERR_OOM = -1, -2, -3
+EVIS_ERR_OVERFLOW, EVIS_ERR_MOTION_BOUND, EVIS_ERR_BAD_STATE = -4, -5, -6
+PATH_AUTO, PATH_GLOBAL, PATH_TILE = 0, 1, 2
+COMPOSITE_B_PRIMARY, COMPOSITE_BLEND = 0, 1
+
+EVENT_DTYPE = np.dtype([("x", "<u2"), ("y", "<u2"), ("env", "<u2"), ("p", "i1"), ("substep", "u1"),
+                        ("t_off", "<f4"), ("kf", "<u4")])
+assert EVENT_DTYPE.itemsize == 16
+
+
+class evis_config(C.Structure):
+    _fields_ = [("num_envs", C.c_int32), ("height", C.c_int32), ("width", C.c_int32), ("substeps", C.c_int32),
+                ("c_pos", C.c_float), ("c_neg", C.c_float), ("log_eps", C.c_float), ("keyframe_dt", C.c_float),
+                ("max_motion_px", C.c_float), ("composite_mode", C.c_int32), ("path", C.c_int32),
+                ("device", C.c_int32), ("event_capacity", C.c_uint64), ("debug_capture", C.c_int32),
+                ("reserved", C.c_int32)]
+
+
+class evis_info(C.Structure):
+    _fields_ = [("path", C.c_int32), ("tile_w", C.c_int32), ("tile_h", C.c_int32), ("halo", C.c_int32),
+                ("steps", C.c_uint64), ("last_events", C.c_uint64), ("last_holes", C.c_uint64),
+                ("kernel_launches", C.c_uint64), ("last_overflow", C.c_int32),
+                ("last_motion_violation", C.c_int32), ("device_bytes", C.c_uint64)]
+
+
+# every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
+SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
+           "evis_get_info", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
+           "evis_strerror", "evis_last_cuda_error", "evis_version"]
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """Load libevis.so.  Raises if it has not been built (python -m paper_2607_08098_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_2607_08098_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, u64p = C.c_void_p, C.POINTER(C.c_uint64)
+    L.evis_create.argtypes = [C.POINTER(evis_config), C.POINTER(vp)]
+    L.evis_step.argtypes = [vp, vp, vp, vp, vp, vp, u64p]
+    L.evis_step_host.argtypes = [vp, vp, vp, vp, vp, u64p]
+    L.evis_read_events.argtypes = [vp, vp, C.c_int, C.c_uint64, u64p]
+    L.evis_events_device.argtypes = [vp, C.POINTER(vp), u64p]
+    L.evis_get_info.argtypes = [vp, C.POINTER(evis_info)]
+    L.evis_get_state.argtypes = [vp, vp, vp]
+    L.evis_set_state.argtypes = [vp, vp, vp]
+    L.evis_debug_read.argtypes = [vp, vp, vp, vp]
+    L.evis_destroy.argtypes = [vp]
+    L.evis_strerror.argtypes = [C.c_int]
+    L.evis_strerror.restype = C.c_char_p
+    L.evis_last_cuda_error.argtypes = [vp]
+    L.evis_version.restype = C.c_char_p
+    for name in SYMBOLS:
+        getattr(L, name)              # raises AttributeError if the library lacks a declared symbol
+    _lib = L
+    return L
+
+
+class EvisError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {load().evis_strerror(status).decode()} ({status})")
+
+
+def _check(status: int, where: str, allow=()):
+    if status != EVIS_OK and status not in allow:
+        raise EvisError(status, where)
+    return status
+
+
+def _dev_ptr(t: Optional[torch.Tensor], shape: Tuple[int, ...], name: str) -> Optional[int]:
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
+        raise ValueError(f"{name}: need a contiguous float32 CUDA tensor of shape {shape}")
+    return t.data_ptr()
+
+
+def _host_ptr(t, shape, name) -> Optional[int]:
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        if not (t.dtype == np.float32 and t.flags.c_contiguous and tuple(t.shape) == tuple(shape)):
+            raise ValueError(f"{name}: need a C-contiguous float32 array of shape {shape}")
+        return t.ctypes.data
+    if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: need a contiguous float32 CPU tensor of shape {shape}")
+    return t.data_ptr()
+
+
+class Evis:
+    """One context of the library (evis_create .. evis_destroy); method names follow the ABI."""
+
+    def __init__(self, num_envs: int, height: int, width: int, substeps: int, c_pos: float, c_neg: float,
+                 log_eps: float, keyframe_dt: float, max_motion_px: float = 0.0, composite_mode: int = 0,
+                 path: int = PATH_AUTO, device: int = 0, event_capacity: int = 1 << 22,
+                 debug_capture: bool = False):
+        self._lib = load()
+        self.cfg = evis_config(num_envs, height, width, substeps, c_pos, c_neg, log_eps, keyframe_dt,
+                               max_motion_px, composite_mode, path, device, event_capacity,
+                               int(debug_capture), 0)
+        self._ctx = C.c_void_p()
+        _check(self._lib.evis_create(C.byref(self.cfg), C.byref(self._ctx)), "evis_create")
+        self.E, self.H, self.W, self.S = num_envs, height, width, substeps
+        self.device = device
+
+    # -- evis_step ---------------------------------------------------------------------------------
+    def step(self, rad: torch.Tensor, mv_bwd: torch.Tensor, depth: torch.Tensor,
+             mv_fwd: Optional[torch.Tensor] = None, sync: bool = False, stream: Optional[torch.cuda.Stream] = None,
+             allow=()) -> Optional[int]:
+        """Enqueue one keyframe on ``stream`` (default: torch's current stream).  With ``sync`` the call
+        waits and returns the true event count of the step."""
+        E, H, W = self.E, self.H, self.W
+        st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+        n = C.c_uint64(0)
+        rc = self._lib.evis_step(self._ctx, _dev_ptr(rad, (E, H, W, 3), "rad"), _dev_ptr(mv_bwd, (E, H, W, 2), "mv_bwd"),
+                                 _dev_ptr(mv_fwd, (E, H, W, 2), "mv_fwd"), _dev_ptr(depth, (E, H, W), "depth"),
+                                 C.c_void_p(st), C.byref(n) if sync else None)
+        _check(rc, "evis_step", allow)
+        return int(n.value) if sync else None
+
+    def step_host(self, rad, mv_bwd, depth, mv_fwd=None, allow=()) -> int:
+        """evis_step_host: HOST buffers (numpy or CPU tensors); copies, runs and synchronises."""
+        E, H, W = self.E, self.H, self.W
+        n = C.c_uint64(0)
+        rc = self._lib.evis_step_host(self._ctx, _host_ptr(rad, (E, H, W, 3), "rad"),
+                                      _host_ptr(mv_bwd, (E, H, W, 2), "mv_bwd"),
+                                      _host_ptr(mv_fwd, (E, H, W, 2), "mv_fwd"),
+                                      _host_ptr(depth, (E, H, W), "depth"), C.byref(n))
+        _check(rc, "evis_step_host", allow)
+        return int(n.value)
+
+    # -- evis_read_events --------------------------------------------------------------------------
+    def read_events(self, max_events: Optional[int] = None) -> np.ndarray:
+        """Events of the last step in the library's deterministic order (host structured array)."""
+        info = self.info()
+        n = min(info.last_events, self.cfg.event_capacity)
+        if max_events is not None:
+            n = min(n, max_events)
+        out = np.empty(n, dtype=EVENT_DTYPE)
+        got = C.c_uint64(0)
+        _check(self._lib.evis_read_events(self._ctx, out.ctypes.data if n else None, 0, n, C.byref(got)),
+               "evis_read_events")
+        return out[:got.value]
+
+    def read_events_into(self, host_buf: np.ndarray) -> int:
+        """evis_read_events into a preallocated (e.g. pinned) host buffer of EVENT_DTYPE."""
+        got = C.c_uint64(0)
+        _check(self._lib.evis_read_events(self._ctx, host_buf.ctypes.data, 0, host_buf.shape[0], C.byref(got)),
+               "evis_read_events")
+        return int(got.value)
+
+    def events_device(self) -> Tuple[int, int]:
+        """(device pointer, stored count) of the ordered stream of the last step; no copy."""
+        p, n = C.c_void_p(), C.c_uint64(0)
+        _check(self._lib.evis_events_device(self._ctx, C.byref(p), C.byref(n)), "evis_events_device")
+        return int(p.value or 0), int(n.value)
+
+    # -- info / state / debug ----------------------------------------------------------------------
+    def info(self) -> evis_info:
+        i = evis_info()
+        _check(self._lib.evis_get_info(self._ctx, C.byref(i)), "evis_get_info")
+        return i
+
+    def get_state(self) -> Tuple[np.ndarray, np.ndarray]:
+        shp = (self.E, self.H, self.W)
+        lref, lprev = np.empty(shp, np.float32), np.empty(shp, np.float32)
+        _check(self._lib.evis_get_state(self._ctx, lref.ctypes.data, lprev.ctypes.data), "evis_get_state")
+        return lref, lprev
+
+    def set_state(self, l_ref: Optional[np.ndarray], l_prev: Optional[np.ndarray]) -> None:
+        shp = (self.E, self.H, self.W)
+        _check(self._lib.evis_set_state(self._ctx, _host_ptr(l_ref, shp, "l_ref"), _host_ptr(l_prev, shp, "l_prev")),
+               "evis_set_state")
+
+    def debug_read(self):
+        """(win [S,E,H,W] u32, dir [S,E,H,W] u8, l_hat [S,E,H,W] f32) of the last step."""
+        shp = (self.S, self.E, self.H, self.W)
+        win, d, lh = np.empty(shp, np.uint32), np.empty(shp, np.uint8), np.empty(shp, np.float32)
+        _check(self._lib.evis_debug_read(self._ctx, win.ctypes.data, d.ctypes.data, lh.ctypes.data), "evis_debug_read")
+        return win, d, lh
+
+    def destroy(self) -> None:
+        if self._ctx:
+            self._lib.evis_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

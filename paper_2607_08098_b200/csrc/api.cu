@@ -1,0 +1,444 @@
+// api.cu -- the C ABI of include/evis.h: context, argument checks, launch sequencing.
+// No step of the path runs on the host: this file only allocates, validates and enqueues kernels.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "kernels.h"
+
+using namespace evis;
+
+static_assert(sizeof(evis_event) == 16, "evis_event is a 16-byte record");
+static_assert(sizeof(evis_config) == 64 && sizeof(evis_info) == 64, "ABI struct layout (binding.py mirrors it)");
+
+struct evis_ctx {
+    evis_config cfg;
+    Geom g;
+    int path;                         // EVIS_PATH_GLOBAL / EVIS_PATH_TILE in use
+    TilePlan tile;
+    cudaStream_t own_stream;          // evis_step_host, state/debug copies
+    cudaStream_t last_stream;
+    int last_cuda;
+
+    Keyframe kf[2];
+    int cur;                          // kf[cur] receives the next keyframe; kf[cur^1] is A
+    float *l_ref, *l_prev;
+    SubstepTable *tab;                // device
+    EventParams ep;
+
+    // global path z-buffers
+    unsigned long long *zmem;
+    size_t zmem_bytes;
+    int chunk_ne, chunk_ni, nset;
+
+    // event stream
+    uint4 *arrival, *ordered;
+    uint2 *directory;
+    uint32_t dir_entries;
+    unsigned long long *bsum;
+    unsigned long long *counters;     // device: [0] events, [1] holes, [2] motion violations
+    unsigned long long *h_counters;   // pinned host mirror
+    DebugOut dbg;
+
+    // host-buffer entry point staging
+    float *st_rad, *st_mv, *st_fwd, *st_depth;
+
+    uint64_t steps, launches, device_bytes;
+    uint64_t last_events, last_holes;
+    int last_overflow, last_motion;
+    bool have_events;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev;
+    bool ok;
+    explicit DeviceGuard(int dev) : prev(-1), ok(true)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+#define CU(call)                                                        \
+    do {                                                                \
+        cudaError_t e_ = (call);                                        \
+        if (e_ != cudaSuccess) {                                        \
+            ctx->last_cuda = (int)e_;                                   \
+            cudaGetLastError();                                         \
+            return e_ == cudaErrorMemoryAllocation ? EVIS_ERR_OOM : EVIS_ERR_CUDA; \
+        }                                                               \
+    } while (0)
+
+template <typename T>
+cudaError_t dalloc(evis_ctx *ctx, T **p, size_t count)
+{
+    const size_t bytes = count * sizeof(T);
+    cudaError_t e = cudaMalloc((void **)p, bytes ? bytes : 1);
+    if (e == cudaSuccess) ctx->device_bytes += bytes;
+    return e;
+}
+
+size_t env_size_mb(const char *name, size_t dflt)
+{
+    const char *v = getenv(name);
+    if (!v || !*v) return dflt;
+    const long long x = atoll(v);
+    return x > 0 ? (size_t)x : dflt;
+}
+
+void free_all(evis_ctx *ctx)
+{
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(ctx->kf[k].L); cudaFree(ctx->kf[k].mv); cudaFree(ctx->kf[k].fwd); cudaFree(ctx->kf[k].Z);
+    }
+    cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->tab); cudaFree(ctx->zmem);
+    cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
+    cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
+    cudaFree(ctx->st_rad); cudaFree(ctx->st_mv); cudaFree(ctx->st_fwd); cudaFree(ctx->st_depth);
+    if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+}
+
+int create_impl(evis_ctx *ctx)
+{
+    const evis_config &c = ctx->cfg;
+    Geom &g = ctx->g;
+    g.E = c.num_envs; g.H = c.height; g.W = c.width; g.S = c.substeps;
+    g.HW = c.height * c.width; g.Wc = c.width + 1; g.HWc = (c.height + 1) * (c.width + 1);
+    g.mode = c.composite_mode;
+    const size_t P = (size_t)g.E * g.HW;
+
+    CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+    for (int k = 0; k < 2; ++k) {
+        CU(dalloc(ctx, &ctx->kf[k].L, P));
+        CU(dalloc(ctx, &ctx->kf[k].mv, P));
+        CU(dalloc(ctx, &ctx->kf[k].Z, P));
+    }
+    CU(dalloc(ctx, &ctx->l_ref, P));
+    CU(dalloc(ctx, &ctx->l_prev, P));
+
+    // substep weights f_i = i/S, g_i = 1 - f_i in IEEE binary32 (same expression as the paper's f = i/K)
+    SubstepTable h;
+    memset(&h, 0, sizeof h);
+    for (int i = 0; i <= g.S; ++i) {
+        volatile float f = (float)i / (float)g.S;
+        volatile float gg = 1.0f - f;
+        h.f[i] = f; h.g[i] = gg;
+    }
+    CU(dalloc(ctx, &ctx->tab, 1));
+    CU(cudaMemcpy(ctx->tab, &h, sizeof h, cudaMemcpyHostToDevice));
+    volatile float dt = c.keyframe_dt / (float)g.S;
+    ctx->ep.c_pos = c.c_pos; ctx->ep.c_neg = c.c_neg; ctx->ep.dt = dt; ctx->ep.kf = 0;
+
+    // path selection
+    ctx->nset = g.mode == 0 ? 1 : 2;
+    ctx->path = EVIS_PATH_GLOBAL;
+    memset(&ctx->tile, 0, sizeof ctx->tile);
+    if (c.path != EVIS_PATH_GLOBAL && c.max_motion_px > 0.0f && plan_tile(g, c.max_motion_px, &ctx->tile))
+        ctx->path = EVIS_PATH_TILE;
+    if (c.path == EVIS_PATH_TILE && ctx->path != EVIS_PATH_TILE) return EVIS_ERR_INVALID_ARG;
+
+    uint32_t tiles_x, tiles_y;
+    if (ctx->path == EVIS_PATH_GLOBAL) {
+        // chunk = envs x substeps whose z-buffers fit the budget (EVIS_ZBUF_MB, default 512 MiB)
+        const size_t unit = (size_t)ctx->nset * 8u * ((size_t)g.HW + g.HWc);
+        const size_t budget = env_size_mb("EVIS_ZBUF_MB", 512) << 20;
+        if (unit * g.S <= budget) {
+            ctx->chunk_ni = g.S;
+            size_t ne = budget / (unit * g.S);
+            ctx->chunk_ne = (int)(ne > (size_t)g.E ? g.E : ne);
+        } else {
+            ctx->chunk_ne = 1;
+            size_t ni = budget / unit;
+            ctx->chunk_ni = (int)(ni < 1 ? 1 : (ni > (size_t)g.S ? g.S : ni));
+        }
+        ctx->zmem_bytes = unit * ctx->chunk_ne * ctx->chunk_ni;
+        CU(cudaMalloc((void **)&ctx->zmem, ctx->zmem_bytes));
+        ctx->device_bytes += ctx->zmem_bytes;
+        tiles_x = (g.W + G_TILE_W - 1) / G_TILE_W;
+        tiles_y = (g.H + G_TILE_H - 1) / G_TILE_H;
+    } else {
+        tiles_x = ctx->tile.tiles_x;
+        tiles_y = ctx->tile.tiles_y;
+    }
+    const unsigned long long ent = (unsigned long long)g.E * g.S * tiles_x * tiles_y;
+    if (ent >= 0xFFFFFFFFull) return EVIS_ERR_INVALID_ARG;
+    ctx->dir_entries = (uint32_t)ent;
+    CU(dalloc(ctx, &ctx->directory, (size_t)ent));
+    CU(dalloc(ctx, &ctx->bsum, (size_t)(ent / 2048 + 2)));
+    CU(dalloc(ctx, &ctx->arrival, (size_t)c.event_capacity));
+    CU(dalloc(ctx, &ctx->ordered, (size_t)c.event_capacity));
+    CU(dalloc(ctx, &ctx->counters, 4));
+    CU(cudaMemset(ctx->counters, 0, 4 * sizeof(unsigned long long)));
+    CU(cudaHostAlloc((void **)&ctx->h_counters, 4 * sizeof(unsigned long long), cudaHostAllocDefault));
+    memset(ctx->h_counters, 0, 4 * sizeof(unsigned long long));
+    if (c.debug_capture) {
+        CU(dalloc(ctx, &ctx->dbg.win, P * g.S));
+        CU(dalloc(ctx, &ctx->dbg.dir, P * g.S));
+        CU(dalloc(ctx, &ctx->dbg.l_hat, P * g.S));
+    }
+    if (ctx->path == EVIS_PATH_TILE) CU(tile_setup(g, ctx->tile));
+    return EVIS_OK;
+}
+
+int fetch_counters(evis_ctx *ctx)
+{
+    if (ctx->last_stream || ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    ctx->last_events = ctx->h_counters[0];
+    ctx->last_holes = ctx->h_counters[1];
+    ctx->last_motion = ctx->h_counters[2] != 0;
+    ctx->last_overflow = ctx->last_events > ctx->cfg.event_capacity;
+    return EVIS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *evis_version(void) { return "evis-b200 0.1 (sm_100a)"; }
+
+const char *evis_strerror(int s)
+{
+    switch (s) {
+        case EVIS_OK: return "ok";
+        case EVIS_ERR_INVALID_ARG: return "invalid argument";
+        case EVIS_ERR_CUDA: return "CUDA error";
+        case EVIS_ERR_OOM: return "out of device memory";
+        case EVIS_ERR_OVERFLOW: return "event capacity exceeded";
+        case EVIS_ERR_MOTION_BOUND: return "motion vector exceeds max_motion_px";
+        case EVIS_ERR_BAD_STATE: return "call order violated";
+        default: return "unknown status";
+    }
+}
+
+int evis_last_cuda_error(const evis_ctx *ctx) { return ctx ? ctx->last_cuda : 0; }
+
+int evis_create(const evis_config *cfg, evis_ctx **out)
+{
+    if (!cfg || !out) return EVIS_ERR_INVALID_ARG;
+    if (cfg->num_envs <= 0 || cfg->num_envs > 65535 || cfg->height <= 0 || cfg->height > 32767 ||
+        cfg->width <= 0 || cfg->width > 32767 || cfg->substeps < 1 || cfg->substeps > 255)
+        return EVIS_ERR_INVALID_ARG;
+    if (!(cfg->c_pos > 0.0f) || !(cfg->c_neg > 0.0f) || !(cfg->log_eps > 0.0f) || !(cfg->keyframe_dt > 0.0f))
+        return EVIS_ERR_INVALID_ARG;
+    if (!(cfg->max_motion_px >= 0.0f)) return EVIS_ERR_INVALID_ARG;
+    if (cfg->composite_mode != EVIS_COMPOSITE_B_PRIMARY && cfg->composite_mode != EVIS_COMPOSITE_BLEND)
+        return EVIS_ERR_INVALID_ARG;
+    if (cfg->path < EVIS_PATH_AUTO || cfg->path > EVIS_PATH_TILE) return EVIS_ERR_INVALID_ARG;
+    if (cfg->event_capacity == 0 || cfg->event_capacity > 0x7FFFFFFFull) return EVIS_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return EVIS_ERR_CUDA; }
+    if (cfg->device < 0 || cfg->device >= ndev) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(cfg->device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    evis_ctx *ctx = new (std::nothrow) evis_ctx();
+    if (!ctx) return EVIS_ERR_OOM;
+    memset(ctx, 0, sizeof *ctx);
+    ctx->cfg = *cfg;
+    const int rc = create_impl(ctx);
+    if (rc != EVIS_OK) { free_all(ctx); delete ctx; return rc; }
+    *out = ctx;
+    return EVIS_OK;
+}
+
+int evis_destroy(evis_ctx *ctx)
+{
+    if (!ctx) return EVIS_OK;
+    DeviceGuard guard(ctx->cfg.device);
+    cudaDeviceSynchronize();
+    free_all(ctx);
+    delete ctx;
+    return EVIS_OK;
+}
+
+int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd, const float *depth,
+              void *cuda_stream, uint64_t *n_events)
+{
+    if (!ctx || !rad || !mv_bwd || !depth) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Geom &g = ctx->g;
+    const size_t P = (size_t)g.E * g.HW;
+    Keyframe &B = ctx->kf[ctx->cur];
+    const Keyframe &A = ctx->kf[ctx->cur ^ 1];
+
+    if (mv_fwd && !B.fwd) {               // forward fields are optional: allocate on first use
+        for (int k = 0; k < 2; ++k) CU(dalloc(ctx, &ctx->kf[k].fwd, P));
+    }
+    B.has_fwd = mv_fwd != nullptr;
+    const bool first = ctx->steps == 0;
+    CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, B.L, B.mv, B.fwd, B.Z,
+                   first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr, st));
+    ctx->launches += 1;
+    ctx->last_stream = st;
+    if (first) {
+        ctx->h_counters[0] = ctx->h_counters[1] = ctx->h_counters[2] = 0;
+        ctx->steps = 1;
+        ctx->cur ^= 1;
+        ctx->have_events = true;
+        if (n_events) { CU(cudaStreamSynchronize(st)); *n_events = 0; }
+        return EVIS_OK;
+    }
+
+    ctx->ep.kf = (uint32_t)(ctx->steps - 1);
+    EventSink sink{ctx->arrival, ctx->cfg.event_capacity, ctx->counters, ctx->directory};
+    CU(cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), st));
+    CU(cudaMemsetAsync(ctx->directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
+    ctx->launches += 2;
+
+    if (ctx->path == EVIS_PATH_GLOBAL) {
+        for (int e0 = 0; e0 < g.E; e0 += ctx->chunk_ne) {
+            const int ne = g.E - e0 < ctx->chunk_ne ? g.E - e0 : ctx->chunk_ne;
+            for (int i0 = 1; i0 <= g.S; i0 += ctx->chunk_ni) {
+                const int ni = g.S + 1 - i0 < ctx->chunk_ni ? g.S + 1 - i0 : ctx->chunk_ni;
+                ZChunk zc;
+                zc.e0 = e0; zc.ne = ne; zc.i0 = i0; zc.ni = ni;
+                const size_t nd = (size_t)ctx->nset * ni * ne * g.HW, nc = (size_t)ctx->nset * ni * ne * g.HWc;
+                zc.zd = ctx->zmem;
+                zc.zc = ctx->zmem + nd;
+                CU(cudaMemsetAsync(ctx->zmem, 0xFF, (nd + nc) * 8u, st));
+                CU(launch_global_splat(g, zc, A, B, ctx->tab, st));
+                CU(launch_global_resolve(g, zc, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink,
+                                         ctx->counters + 1, ctx->dbg, st));
+                ctx->launches += 3;
+            }
+        }
+    } else {
+        CU(launch_tile(g, ctx->tile, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink, ctx->counters + 1,
+                       ctx->counters + 2, ctx->dbg, st));
+        ctx->launches += 1;
+    }
+    int nl = 0;
+    CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, st, &nl));
+    ctx->launches += nl;
+    CU(cudaMemcpyAsync(ctx->h_counters, ctx->counters, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    ctx->steps += 1;
+    ctx->cur ^= 1;
+    ctx->have_events = true;
+    if (n_events) {
+        const int rc = fetch_counters(ctx);
+        if (rc != EVIS_OK) return rc;
+        *n_events = ctx->last_events;
+        if (ctx->last_overflow) return EVIS_ERR_OVERFLOW;
+        if (ctx->last_motion) return EVIS_ERR_MOTION_BOUND;
+    }
+    return EVIS_OK;
+}
+
+int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd,
+                   const float *depth, uint64_t *n_events)
+{
+    if (!ctx || !rad || !mv_bwd || !depth) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    const size_t P = (size_t)ctx->g.E * ctx->g.HW;
+    if (!ctx->st_rad) {
+        CU(dalloc(ctx, &ctx->st_rad, 3 * P));
+        CU(dalloc(ctx, &ctx->st_mv, 2 * P));
+        CU(dalloc(ctx, &ctx->st_depth, P));
+    }
+    if (mv_fwd && !ctx->st_fwd) CU(dalloc(ctx, &ctx->st_fwd, 2 * P));
+    cudaStream_t st = ctx->own_stream;
+    CU(cudaMemcpyAsync(ctx->st_rad, rad, 3 * P * sizeof(float), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(ctx->st_mv, mv_bwd, 2 * P * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (mv_fwd) CU(cudaMemcpyAsync(ctx->st_fwd, mv_fwd, 2 * P * sizeof(float), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(ctx->st_depth, depth, P * sizeof(float), cudaMemcpyHostToDevice, st));
+    uint64_t n = 0;
+    const int rc = evis_step(ctx, ctx->st_rad, ctx->st_mv, mv_fwd ? ctx->st_fwd : nullptr, ctx->st_depth,
+                             (void *)st, &n);
+    if (n_events) *n_events = n;
+    return rc;
+}
+
+int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t max, uint64_t *n_out)
+{
+    if (!ctx || (!dst && max > 0)) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->have_events) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    const int rc = fetch_counters(ctx);
+    if (rc != EVIS_OK) return rc;
+    uint64_t n = ctx->last_events;
+    if (n > ctx->cfg.event_capacity) n = ctx->cfg.event_capacity;
+    if (n > max) n = max;
+    if (n) CU(cudaMemcpy(dst, ctx->ordered, n * sizeof(evis_event),
+                         dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    if (n_out) *n_out = n;
+    return EVIS_OK;
+}
+
+int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_stored)
+{
+    if (!ctx || !dev_ptr || !n_stored) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->have_events) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    const int rc = fetch_counters(ctx);
+    if (rc != EVIS_OK) return rc;
+    *dev_ptr = reinterpret_cast<const evis_event *>(ctx->ordered);
+    *n_stored = ctx->last_events < ctx->cfg.event_capacity ? ctx->last_events : ctx->cfg.event_capacity;
+    return EVIS_OK;
+}
+
+int evis_get_info(evis_ctx *ctx, evis_info *info)
+{
+    if (!ctx || !info) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (ctx->steps) { const int rc = fetch_counters(ctx); if (rc != EVIS_OK) return rc; }
+    memset(info, 0, sizeof *info);
+    info->path = ctx->path;
+    info->tile_w = ctx->path == EVIS_PATH_TILE ? ctx->tile.tw : G_TILE_W;
+    info->tile_h = ctx->path == EVIS_PATH_TILE ? ctx->tile.th : G_TILE_H;
+    info->halo = ctx->path == EVIS_PATH_TILE ? ctx->tile.halo : 0;
+    info->steps = ctx->steps;
+    info->last_events = ctx->last_events;
+    info->last_holes = ctx->last_holes;
+    info->kernel_launches = ctx->launches;
+    info->last_overflow = ctx->last_overflow;
+    info->last_motion_violation = ctx->last_motion;
+    info->device_bytes = ctx->device_bytes;
+    return EVIS_OK;
+}
+
+int evis_get_state(evis_ctx *ctx, float *l_ref, float *l_prev)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->steps) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    CU(cudaStreamSynchronize(ctx->last_stream));
+    const size_t bytes = (size_t)ctx->g.E * ctx->g.HW * sizeof(float);
+    if (l_ref) CU(cudaMemcpy(l_ref, ctx->l_ref, bytes, cudaMemcpyDeviceToHost));
+    if (l_prev) CU(cudaMemcpy(l_prev, ctx->l_prev, bytes, cudaMemcpyDeviceToHost));
+    return EVIS_OK;
+}
+
+int evis_set_state(evis_ctx *ctx, const float *l_ref, const float *l_prev)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->steps) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    CU(cudaStreamSynchronize(ctx->last_stream));
+    const size_t bytes = (size_t)ctx->g.E * ctx->g.HW * sizeof(float);
+    if (l_ref) CU(cudaMemcpy(ctx->l_ref, l_ref, bytes, cudaMemcpyHostToDevice));
+    if (l_prev) CU(cudaMemcpy(ctx->l_prev, l_prev, bytes, cudaMemcpyHostToDevice));
+    return EVIS_OK;
+}
+
+int evis_debug_read(evis_ctx *ctx, uint32_t *win, uint8_t *dir, float *l_hat)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->cfg.debug_capture || ctx->steps < 2) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    CU(cudaStreamSynchronize(ctx->last_stream));
+    const size_t n = (size_t)ctx->g.E * ctx->g.HW * ctx->g.S;
+    if (win) CU(cudaMemcpy(win, ctx->dbg.win, n * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    if (dir) CU(cudaMemcpy(dir, ctx->dbg.dir, n, cudaMemcpyDeviceToHost));
+    if (l_hat) CU(cudaMemcpy(l_hat, ctx->dbg.l_hat, n * sizeof(float), cudaMemcpyDeviceToHost));
+    return EVIS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,74 @@
+// kernels.h -- internal launch interface between api.cu and the kernel files (not part of the ABI).
+#pragma once
+#include "common.cuh"
+
+namespace evis {
+
+// One stored keyframe (device, owned by the context): planar so that the z-test gathers
+// (far-endpoint depth, winner's L) touch 4-byte elements.
+struct Keyframe {
+    float  *L;     // [E*H*W] log-luminance                         (a1)
+    float2 *mv;    // [E*H*W] backward motion vector, pixels
+    float2 *fwd;   // [E*H*W] explicit forward field, or unused     (R12)
+    float  *Z;     // [E*H*W] depth
+    bool    has_fwd;
+};
+
+struct Geom {
+    int E, H, W, S;
+    int HW;        // H*W
+    int Wc, HWc;   // class-11 cell grid: (W+1) x (H+1) cells, cell (x0+1, y0+1)
+    int mode;      // EVIS_COMPOSITE_*
+};
+
+struct DebugOut {  // all nullable; [S,E,H,W]
+    uint32_t *win;
+    uint8_t  *dir;
+    float    *l_hat;
+};
+
+// a1 + a9 (prep.cu)
+cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, const float *depth, long long n,
+                        float eps, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
+                        float *l_prev, cudaStream_t st);
+
+// ---- global z-buffer path (global_path.cu): any motion -----------------------------------------
+// z-buffers of one chunk = envs [e0, e0+ne) x substeps [i0, i0+ni):
+//   zd [nset][ni][ne][HW]   direct targets (footprints that are a single pixel or a 2-pixel edge)
+//   zc [nset][ni][ne][HWc]  class-11 cells: the source covers the 2x2 block whose top-left is the cell
+// nset = 1 in composite mode 0 (direction folded into the key's top bit), 2 in mode 1.
+struct ZChunk {
+    unsigned long long *zd, *zc;
+    int e0, ne, i0, ni;
+};
+constexpr int G_TILE_W = 32, G_TILE_H = 8;     // ordering tile of the global path
+
+cudaError_t launch_global_splat(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B,
+                                const SubstepTable *tab_dev, cudaStream_t st);
+cudaError_t launch_global_resolve(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B,
+                                  const SubstepTable *tab_dev, float *l_ref, float *l_prev,
+                                  const EventParams &ep, const EventSink &sink, unsigned long long *holes,
+                                  const DebugOut &dbg, cudaStream_t st);
+
+// ---- tile path (tile_path.cu): bounded motion, z-buffers in shared memory --------------------------
+struct TilePlan {
+    int tw, th;            // target tile (also the ordering tile)
+    int halo;              // source halo in pixels, >= ceil(max_motion_px) + 1
+    int tiles_x, tiles_y;
+    int threads;           // CTA size
+    int cand_cap;          // candidate sources kept in shared memory per tile
+    int smem_bytes;
+};
+bool plan_tile(const Geom &g, float max_motion_px, TilePlan *plan);     // false: motion too large for a tile
+cudaError_t tile_setup(const Geom &g, const TilePlan &plan);            // one-time function attributes
+cudaError_t launch_tile(const Geom &g, const TilePlan &plan, const Keyframe &A, const Keyframe &B,
+                        const SubstepTable *tab_dev, float *l_ref, float *l_prev, const EventParams &ep,
+                        const EventSink &sink, unsigned long long *holes, unsigned long long *motion_viol,
+                        const DebugOut &dbg, cudaStream_t st);
+
+// ---- a8 ordering (order.cu) ----------------------------------------------------------------------
+// directory entry d = (arrival offset, count); ordered stream = chunks concatenated in d order.
+cudaError_t launch_order(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out /*[n]*/,
+                         uint4 *ordered, cudaStream_t st, int *launches);
+
+}  // namespace evis

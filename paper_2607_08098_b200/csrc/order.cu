@@ -1,0 +1,112 @@
+// order.cu -- row a8, second half: deterministic ordering of the compacted event stream.
+//
+// The compaction kernels reserve space with one global atomic per (tile, substep) chunk, so chunks
+// land in the arrival buffer in scheduling order.  Each chunk left (arrival offset, count) in
+// directory[d], d = ((env * S + substep-1) * tiles_y + tile_y) * tiles_x + tile_x.  Here the chunks
+// are laid out in directory order: exclusive scan of the counts (three small kernels) and a
+// chunk-by-chunk 128-bit copy.  Inside a chunk the order is the block scan order of the producer
+// (pixel rank in the tile, then crossing index k), which is deterministic as well.
+#include "kernels.h"
+
+namespace evis {
+
+constexpr int ORD_NT = 256, ORD_PER_THREAD = 8, ORD_PER_BLOCK = ORD_NT * ORD_PER_THREAD;
+
+__device__ __forceinline__ unsigned long long block_scan_excl(unsigned long long v, unsigned long long *s_w,
+                                                              unsigned long long &total)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned long long incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned long long u = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+        if (lane >= d) incl += u;
+    }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        const int nw = blockDim.x >> 5;
+        unsigned long long w = lane < nw ? s_w[lane] : 0ull, wi = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned long long u = __shfl_up_sync(0xFFFFFFFFu, wi, d);
+            if (lane >= d) wi += u;
+        }
+        if (lane < nw) s_w[lane] = wi - w;
+        if (lane == 31) s_w[32] = wi;
+    }
+    __syncthreads();
+    total = s_w[32];
+    const unsigned long long r = s_w[warp] + incl - v;
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(ORD_NT)
+k_dir_blocksum(const uint2 *__restrict__ dir, uint32_t n, unsigned long long *__restrict__ bsum)
+{
+    __shared__ unsigned long long s_w[33];
+    const uint32_t base = blockIdx.x * ORD_PER_BLOCK + threadIdx.x * ORD_PER_THREAD;
+    unsigned long long v = 0;
+#pragma unroll
+    for (int j = 0; j < ORD_PER_THREAD; ++j)
+        if (base + j < n) v += dir[base + j].y;
+    unsigned long long total;
+    block_scan_excl(v, s_w, total);
+    if (threadIdx.x == 0) bsum[blockIdx.x] = total;
+}
+
+// single block: exclusive scan of the per-block sums in place
+__global__ void __launch_bounds__(1024)
+k_dir_scan_bsum(unsigned long long *__restrict__ bsum, uint32_t nb)
+{
+    __shared__ unsigned long long s_w[33];
+    const uint32_t per = (nb + blockDim.x - 1) / blockDim.x;
+    const uint32_t lo = threadIdx.x * per, hi = min(lo + per, nb);
+    unsigned long long v = 0;
+    for (uint32_t j = lo; j < hi; ++j) v += bsum[j];
+    unsigned long long total;
+    unsigned long long run = block_scan_excl(v, s_w, total);
+    for (uint32_t j = lo; j < hi; ++j) { const unsigned long long c = bsum[j]; bsum[j] = run; run += c; }
+}
+
+__global__ void __launch_bounds__(ORD_NT)
+k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__restrict__ bsum,
+           const uint4 *__restrict__ arrival, uint4 *__restrict__ ordered, unsigned long long cap)
+{
+    __shared__ unsigned long long s_w[33];
+    __shared__ unsigned long long s_dst[ORD_PER_BLOCK];
+    const uint32_t blk = blockIdx.x * ORD_PER_BLOCK;
+    const uint32_t base = blk + threadIdx.x * ORD_PER_THREAD;
+    uint32_t cnt[ORD_PER_THREAD];
+    unsigned long long v = 0;
+#pragma unroll
+    for (int j = 0; j < ORD_PER_THREAD; ++j) { cnt[j] = base + j < n ? dir[base + j].y : 0u; v += cnt[j]; }
+    unsigned long long total;
+    unsigned long long run = block_scan_excl(v, s_w, total) + bsum[blockIdx.x];
+    if (total == 0) return;
+#pragma unroll
+    for (int j = 0; j < ORD_PER_THREAD; ++j) { s_dst[threadIdx.x * ORD_PER_THREAD + j] = run; run += cnt[j]; }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (uint32_t e = warp; e < (uint32_t)ORD_PER_BLOCK && blk + e < n; e += ORD_NT / 32) {
+        const uint2 d = dir[blk + e];
+        if (d.y == 0) continue;
+        const unsigned long long src = d.x, dst = s_dst[e];
+        for (uint32_t k = lane; k < d.y; k += 32)
+            if (src + k < cap && dst + k < cap) ordered[dst + k] = arrival[src + k];
+    }
+}
+
+cudaError_t launch_order(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
+                         cudaStream_t st, int *launches)
+{
+    const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
+    k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum);
+    k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb);
+    k_dir_copy<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, ordered, sink.capacity);
+    if (launches) *launches += 3;
+    return cudaGetLastError();
+}
+
+}  // namespace evis

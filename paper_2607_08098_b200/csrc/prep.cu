@@ -1,0 +1,90 @@
+// prep.cu -- row a1 of the hot path: radiance -> log-luminance, once per keyframe pixel, fused
+// with taking ownership of the keyframe's motion vectors and depth (a9: this keyframe is the next
+// step's A, and the caller may free its tensors as soon as this kernel has run).
+//
+//   I = 0.2126 R + 0.7152 G + 0.0722 B        (Eq. 3)
+//   L = log(I + eps), natural log, I clamped at 0   (R1, R3)
+//
+// Evaluated in binary64 with every product and sum rounded separately (no fma), summed left to
+// right, and rounded once to binary32 -- the arithmetic contract of DESIGN.md Sec. 2.
+//
+// HBM-bound streaming kernel: 24 B read (+8 with mv_fwd) and 16 B written (+8) per pixel, 128-bit
+// loads and stores, four pixels per thread.
+#include "kernels.h"
+
+namespace evis {
+
+__device__ __forceinline__ float log_lum(float r, float g, float b, double eps)
+{
+    double I = __dadd_rn(__dadd_rn(__dmul_rn(0.2126, (double)r), __dmul_rn(0.7152, (double)g)),
+                         __dmul_rn(0.0722, (double)b));
+    if (!(I > 0.0)) I = 0.0;
+    return __double2float_rn(log(__dadd_rn(I, eps)));
+}
+
+// VEC: all pointers 16-byte aligned and n % 4 == 0 -> thread handles 4 consecutive pixels.
+template <bool VEC>
+__global__ void __launch_bounds__(256)
+k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float *__restrict__ fwd_in,
+       const float *__restrict__ depth, long long n, float eps_f,
+       float *__restrict__ L, float2 *__restrict__ mv_out, float2 *__restrict__ fwd_out,
+       float *__restrict__ Z, float *__restrict__ l_ref, float *__restrict__ l_prev)
+{
+    const double eps = (double)eps_f;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (VEC) {
+        const long long p = t * 4;
+        if (p >= n) return;
+        const float4 *r4 = reinterpret_cast<const float4 *>(rad + 3 * p);
+        const float4 a = __ldcs(r4), b = __ldcs(r4 + 1), c = __ldcs(r4 + 2);
+        float4 l;
+        l.x = log_lum(a.x, a.y, a.z, eps);
+        l.y = log_lum(a.w, b.x, b.y, eps);
+        l.z = log_lum(b.z, b.w, c.x, eps);
+        l.w = log_lum(c.y, c.z, c.w, eps);
+        *reinterpret_cast<float4 *>(L + p) = l;
+        if (l_ref) {                                  // first keyframe: L_ref = L_prev = L   (R6)
+            *reinterpret_cast<float4 *>(l_ref + p) = l;
+            *reinterpret_cast<float4 *>(l_prev + p) = l;
+        }
+        const float4 *m4 = reinterpret_cast<const float4 *>(mv + 2 * p);
+        float4 *mo = reinterpret_cast<float4 *>(mv_out + p);
+        mo[0] = __ldcs(m4);
+        mo[1] = __ldcs(m4 + 1);
+        if (fwd_in) {
+            const float4 *f4 = reinterpret_cast<const float4 *>(fwd_in + 2 * p);
+            float4 *fo = reinterpret_cast<float4 *>(fwd_out + p);
+            fo[0] = __ldcs(f4);
+            fo[1] = __ldcs(f4 + 1);
+        }
+        *reinterpret_cast<float4 *>(Z + p) = __ldcs(reinterpret_cast<const float4 *>(depth + p));
+    } else {
+        if (t >= n) return;
+        const float l = log_lum(rad[3 * t], rad[3 * t + 1], rad[3 * t + 2], eps);
+        L[t] = l;
+        if (l_ref) { l_ref[t] = l; l_prev[t] = l; }
+        mv_out[t] = make_float2(mv[2 * t], mv[2 * t + 1]);
+        if (fwd_in) fwd_out[t] = make_float2(fwd_in[2 * t], fwd_in[2 * t + 1]);
+        Z[t] = depth[t];
+    }
+}
+
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, const float *depth, long long n,
+                        float eps, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
+                        float *l_prev, cudaStream_t st)
+{
+    const bool vec = (n % 4 == 0) && aligned16(rad) && aligned16(mv) && aligned16(depth) && (!fwd || aligned16(fwd));
+    if (vec) {
+        const long long threads = n / 4;
+        k_prep<true><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, L, mv_out,
+                                                                         fwd_out, Z, l_ref, l_prev);
+    } else {
+        k_prep<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, L, mv_out,
+                                                                    fwd_out, Z, l_ref, l_prev);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace evis

@@ -1,0 +1,201 @@
+"""GPU parity: the CUDA library, called through the C ABI, against the CPU oracle on the same seeded
+inputs (north_star criteria, see tests/parity.py).  Sizes: what the oracle finishes in seconds, several
+tiles plus ragged tails; full-size BASELINE configs compare sampled envs (envs are independent, so the
+oracle computes them one by one)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2607_08098_b200 import binding, scenes
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+PATHS = [binding.PATH_GLOBAL, binding.PATH_AUTO]
+
+
+def _assert_tolerances(rep):
+    assert rep.max_dL <= parity.TOL_L, rep
+    assert rep.max_dt <= parity.TOL_T, rep
+    # ties are legal but must be rare (R5): report them
+    print(f"[parity] steps={rep.steps} events gpu/oracle={rep.events_gpu}/{rep.events_oracle} "
+          f"ties={rep.ties} max|dL|={rep.max_dL:.3g} max|dt|={rep.max_dt:.3g} holes={rep.holes}")
+    assert rep.ties <= max(2, rep.events_oracle // 100000)
+    assert rep.events_oracle > 0
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config1_full(path):
+    """BASELINE config 1 in full: 1 env, 346x260, S=16, C=0.2."""
+    spec = scenes.config(1)
+    rep = parity.run_parity(spec, 3, path=path)
+    _assert_tolerances(rep)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("use_fwd", [True, False])
+def test_config2_reduced(path, use_fwd):
+    """Config 2 recipe (32 overlapping rectangles, occlusion every step) at 3 envs, 211x157 (ragged)."""
+    spec = scenes.small(scenes.config(2), num_envs=3, height=157, width=211, num_keyframes=4)
+    rep = parity.run_parity(spec, 4, path=path, use_fwd=use_fwd)
+    _assert_tolerances(rep)
+    assert rep.holes > 0          # disocclusion actually happens in this workload
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config3_reduced_disk(path):
+    """Config 3 recipe (rotating spoked disk, rotational MV, C+ != C-, S=33) at 2 envs, 320x200."""
+    spec = scenes.small(scenes.config(3), num_envs=2, height=200, width=320, num_keyframes=3)
+    rep = parity.run_parity(spec, 3, path=path)
+    _assert_tolerances(rep)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config4_reduced_rl(path):
+    """Config 4 recipe (ego-motion + brightness ramp) at 5 envs, full 346x260 resolution."""
+    spec = scenes.small(scenes.config(4), num_envs=5, num_keyframes=4)
+    rep = parity.run_parity(spec, 4, path=path)
+    _assert_tolerances(rep)
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 7, 5), (2, 33, 9), (3, 8, 65)])
+@pytest.mark.parametrize("S", [1, 3, 16])
+def test_tiny_and_ragged_shapes(shape, S):
+    E, H, W = shape
+    spec = scenes.SceneSpec("tiny", E, H, W, 3, 1.0 / 60.0, S, 0.1, 0.15, num_rects=3, v_max=200.0, seed=77)
+    rep = parity.run_parity(spec, 3, path=binding.PATH_GLOBAL)
+    assert rep.max_dL <= parity.TOL_L and rep.max_dt <= parity.TOL_T
+
+
+def test_blend_mode_global():
+    """Composite mode 1 (R19): nearest of both winners, time-weighted blend on the same surface."""
+    spec = scenes.small(scenes.config(2), num_envs=2, height=120, width=160, num_keyframes=3)
+    rep = parity.run_parity(spec, 3, mode=1, path=binding.PATH_GLOBAL)
+    _assert_tolerances(rep)
+
+
+def test_large_s_166():
+    spec = scenes.SceneSpec("s166", 2, 90, 120, 3, 1.0 / 60.0, 166, 0.2, 0.2, num_rects=6, v_max=300.0, seed=5)
+    rep = parity.run_parity(spec, 3, path=binding.PATH_GLOBAL)
+    _assert_tolerances(rep)
+
+
+def test_chunked_zbuffer_budget(monkeypatch):
+    """Force the global path to split envs and substeps into several z-buffer chunks."""
+    monkeypatch.setenv("EVIS_ZBUF_MB", "1")
+    spec = scenes.small(scenes.config(4), num_envs=4, height=130, width=173, num_keyframes=3)
+    rep = parity.run_parity(spec, 3, path=binding.PATH_GLOBAL)
+    _assert_tolerances(rep)
+
+
+def _run_stream(spec, n_kf, path, seed_offset=0):
+    sc = scenes.make_scene(spec)
+    ev = binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg,
+                      spec.log_eps, spec.keyframe_dt, max_motion_px=spec.max_motion_px(), path=path,
+                      event_capacity=1 << 24)
+    outs = []
+    for k in range(n_kf):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        if k:
+            outs.append(ev.read_events().copy())
+    info = ev.info()
+    ev.destroy()
+    return outs, info
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_output_order_is_deterministic_and_tiled(path):
+    """Two runs give byte-identical ordered streams; the order is (env, substep, tile row, tile col,
+    y, x, time) with the tile geometry evis_get_info reports."""
+    spec = scenes.small(scenes.config(2), num_envs=3, height=157, width=211, num_keyframes=3)
+    a, info = _run_stream(spec, 3, path)
+    b, _ = _run_stream(spec, 3, path)
+    assert sum(len(x) for x in a) > 1000
+    for x, y in zip(a, b):
+        assert x.tobytes() == y.tobytes()
+    tw, th = info.tile_w, info.tile_h
+    for ev in a:
+        key = np.stack([ev["env"].astype(np.int64), ev["substep"].astype(np.int64), ev["y"] // th, ev["x"] // tw,
+                        ev["y"].astype(np.int64), ev["x"].astype(np.int64)], axis=1)
+        # lexicographic non-decreasing
+        d = np.diff(key, axis=0)
+        first = np.argmax(d != 0, axis=1)
+        lead = d[np.arange(len(d)), first]
+        assert np.all(lead >= 0)
+        same = np.all(d == 0, axis=1)
+        assert np.all(np.diff(ev["t_off"])[same] >= 0)
+
+
+def test_invariants_p7_p9_on_gpu_output():
+    """P7 / P9 on the library's output alone: timestamps inside their substep and per-pixel
+    reconstruction L_0 + C+ N+ - C- N- within one threshold of the final frame."""
+    spec = scenes.small(scenes.config(4), num_envs=8, num_keyframes=5)
+    sc = scenes.make_scene(spec)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                      max_motion_px=spec.max_motion_px(), event_capacity=1 << 24)
+    net = np.zeros((E, H, W), np.float64)
+    L0 = None
+    dt = spec.keyframe_dt / S
+    for k in range(spec.num_keyframes):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        if k == 0:
+            L0 = ev.get_state()[0].astype(np.float64)
+            continue
+        e = ev.read_events()
+        i = e["substep"].astype(np.float64)
+        assert np.all(e["t_off"] >= (i - 1) * dt - 1e-9) and np.all(e["t_off"] <= i * dt + 1e-9)
+        w = np.where(e["p"] > 0, spec.c_pos, -spec.c_neg)
+        np.add.at(net, (e["env"].astype(np.int64), e["y"].astype(np.int64), e["x"].astype(np.int64)), w)
+    lref, lprev = ev.get_state()
+    assert np.allclose(L0 + net, lref, atol=1e-4)
+    assert np.all(np.abs(lprev - lref) < max(spec.c_pos, spec.c_neg) + 1e-5)
+    ev.destroy()
+
+
+def test_event_capacity_overflow_is_reported():
+    spec = scenes.small(scenes.config(2), num_envs=2, height=120, width=160, num_keyframes=2)
+    sc = scenes.make_scene(spec)
+    ev = binding.Evis(2, 120, 160, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                      event_capacity=100)
+    k0 = scenes.render_keyframe(sc, 0, device="cuda")
+    k1 = scenes.render_keyframe(sc, 1, device="cuda")
+    ev.step(k0["rad"], k0["mv_bwd"], k0["depth"], sync=True)
+    with pytest.raises(binding.EvisError) as ei:
+        ev.step(k1["rad"], k1["mv_bwd"], k1["depth"], sync=True)
+    assert ei.value.status == binding.EVIS_ERR_OVERFLOW
+    info = ev.info()
+    assert info.last_overflow == 1 and info.last_events > 100
+    assert len(ev.read_events()) == 100
+    ev.destroy()
+
+
+def test_host_entry_point_matches_device_entry_point():
+    spec = scenes.small(scenes.config(1), num_keyframes=3)
+    sc = scenes.make_scene(spec)
+    mk = lambda: binding.Evis(1, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps,
+                              spec.keyframe_dt, max_motion_px=spec.max_motion_px(), event_capacity=1 << 22)
+    a, b = mk(), mk()
+    for k in range(3):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        na = a.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        h = {key: v.cpu().numpy() for key, v in kf.items()}
+        nb = b.step_host(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"])
+        assert na == nb
+        if k:
+            assert a.read_events().tobytes() == b.read_events().tobytes()
+    a.destroy(); b.destroy()
+
+
+def test_generator_is_device_independent():
+    """The seeded generator paints byte-identical keyframes on the CPU and on the GPU."""
+    for i in (1, 3, 4):
+        spec = scenes.small(scenes.config(i), num_envs=2, height=96, width=128)
+        sc = scenes.make_scene(spec)
+        for k in (0, 2):
+            c = scenes.render_keyframe(sc, k, device="cpu")
+            g = scenes.render_keyframe(sc, k, device="cuda")
+            for key in c:
+                assert torch.equal(c[key], g[key].cpu()), (i, k, key)
