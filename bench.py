@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the EVIS event-synthesis hot path on B200 (contract: see DESIGN.md Sec. 8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..4] [--impl ours|reference]
+
+One "step" = one evis_step call = one keyframe interval of the whole batch: log-luminance of the new
+keyframe, bidirectional warp with z-buffered splat to S substeps, event model on every substep,
+compaction + deterministic ordering.  The keyframes are seeded
+synthetic scenes (paper_2607_08098_b200/scenes.py) and are resident in HBM before the timed region
+(`value`); `e2e` repeats the measurement through evis_step_host / evis_read_events with pinned HOST
+buffers, host<->device copies inside the timed region.
+
+Prints ONE JSON line on rank 0.  N > 1: one process per GPU (torchrun), envs are independent so every
+rank runs its own batch of the same shape (different seed) with no data-path collective; the time is
+the max over ranks ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pixel-substeps/s"
+ALGO_BYTES_PER_PIXEL = 52          # per pixel per keyframe interval, DESIGN.md Sec. 6
+ALGO_BYTES_PER_EVENT = 16
+FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based, 1..4)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--path", default="auto", choices=["auto", "global", "tile"])
+    ap.add_argument("--envs", type=int, default=0, help="override the number of envs (0 = the config's)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=6)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    return ap.parse_args()
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for (_, r) in self.rows]
+        for r in rows:
+            c = [x.strip() for x in r.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx = float(c[1])
+            except ValueError:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline of our arm; the whole --impl reference arm)
+# ------------------------------------------------------------------------------------------------
+def time_oracle(spec, n_envs: int, n_steps: int, warmup: int):
+    """Run the CPU oracle (oracle/, as it stands, single thread) on the first `n_envs` envs of the
+    workload for warmup + n_steps keyframe intervals.  Returns (pixel-substeps/s, events/s, seconds
+    per step, events)."""
+    from oracle import evis_oracle as orc
+    from paper_2607_08098_b200 import scenes
+    sub = scenes.small(spec, num_envs=n_envs)
+    sc = scenes.make_scene(sub)
+    o = orc.Oracle(n_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps,
+                   spec.keyframe_dt)
+    kfs = [{a: b.numpy() for a, b in scenes.render_keyframe(sc, k).items()} for k in range(warmup + n_steps + 1)]
+    for k in range(warmup + 1):                        # keyframe 0 initialises; then `warmup` intervals
+        o.step(kfs[k]["rad"], kfs[k]["mv_bwd"], kfs[k]["depth"], kfs[k]["mv_fwd"])
+    ev = 0
+    t0 = time.perf_counter()
+    for k in range(warmup + 1, warmup + 1 + n_steps):
+        ev += len(o.step(kfs[k]["rad"], kfs[k]["mv_bwd"], kfs[k]["depth"], kfs[k]["mv_fwd"]))
+    dt = time.perf_counter() - t0
+    pxss = n_envs * spec.height * spec.width * spec.substeps * n_steps
+    return pxss / dt, ev / dt, dt / n_steps, ev
+
+
+def cpu_baseline(spec, seconds: float) -> dict:
+    """The oracle on a bounded sample of the same workload, sized for about `seconds` of CPU work."""
+    n_envs = min(spec.num_envs, 2)
+    rate, _, per_step, _ = time_oracle(spec, n_envs, 1, 0)          # probe: one interval
+    steps = max(1, min(60, int(seconds / max(per_step, 1e-3))))
+    rate, ev_rate, per_step, _ = time_oracle(spec, n_envs, steps, 0)
+    return {"value": rate, "unit": METRIC, "events_per_s": ev_rate, "cores": 1, "kind": "oracle",
+            "sample": f"oracle/evis_oracle.c single thread, first {n_envs} envs of {spec.name} at full "
+                      f"resolution, {steps} keyframe intervals ({per_step:.2f} s each)"}
+
+
+def run_reference(args, spec) -> None:
+    """--impl reference: there is no reference code (paper only), so the reference arm is the oracle,
+    timed as it stands on the host cores.  Rank 0 alone works."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_envs = min(spec.num_envs, 2)
+    steps = args.steps
+    rate, ev_rate, per_step, ev = time_oracle(spec, n_envs, steps, args.warmup)
+    sample = (f"oracle/evis_oracle.c single thread; each step = one keyframe interval of the first {n_envs} "
+              f"envs of {spec.name} at full resolution")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": METRIC, "n_gpus": args.gpus,
+        "steps": steps, "warmup": args.warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": workload_config(spec, "cpu-oracle"),
+        "events_per_s": ev_rate,
+        "cpu_baseline": {"value": rate, "unit": METRIC, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def workload_config(spec, path: str) -> dict:
+    return {"workload": spec.name, "envs": spec.num_envs, "height": spec.height, "width": spec.width,
+            "substeps": spec.substeps, "keyframe_hz": round(1.0 / spec.keyframe_dt, 3),
+            "c_pos": spec.c_pos, "c_neg": spec.c_neg, "log_eps": spec.log_eps, "path": path,
+            "l2": "inputs larger than L2 (one keyframe >= 126 MB), no flush" }
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+def run_ours(args, spec) -> None:
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2607_08098_b200 import binding, scenes
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    binding.load()                                     # fails loudly when libevis.so is missing
+
+    # every rank: its own batch of the same shape (envs are independent: no exchange step)
+    spec = scenes.small(spec, seed=spec.seed + 1000 * rank)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    K, Wm = args.steps, args.warmup
+    sc = scenes.make_scene(spec)
+    n_kf = Wm + K + 1
+    kfs = [scenes.render_keyframe(sc, k, device=dev) for k in range(n_kf)]
+    path = {"auto": binding.PATH_AUTO, "global": binding.PATH_GLOBAL, "tile": binding.PATH_TILE}[args.path]
+    cap = int(min(0x7FFFFFFF, max(1 << 22, 10 * E * H * W)))          # events stored per step
+    mk = lambda: binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                              max_motion_px=spec.max_motion_px(), path=path, device=local, event_capacity=cap)
+    ev = mk()
+    stream = torch.cuda.current_stream(dev)
+
+    def step(k):
+        f = kfs[k]
+        ev.step(f["rad"], f["mv_bwd"], f["depth"], mv_fwd=f["mv_fwd"], stream=stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing -------------------------------------------------------------------
+    for k in range(Wm + 1):                             # keyframe 0 initialises, then W warm-up intervals
+        step(k)
+    barrier()
+    i0 = ev.info()
+    clk = ClockSampler(local)
+    clk.start()
+    time.sleep(0.25)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.time()
+    e0.record(stream)
+    for k in range(Wm + 1, Wm + 1 + K):
+        step(k)
+    e1.record(stream)
+    barrier()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    clocks = clk.stop(t0, t1)
+    i1 = ev.info()
+    if i1.last_overflow:
+        raise SystemExit("bench.py: event capacity overflow in the timed region")
+    events = i1.total_events - i0.total_events
+    launches = i1.kernel_launches - i0.kernel_launches
+    path_used = {binding.PATH_GLOBAL: "global", binding.PATH_TILE: "tile"}[i1.path]
+
+    # ---- per-stage device time of the same steps (second pass over the same keyframes, CUDA events
+    #      recorded by the library on the launching stream) -> dominant kernel for the roofline -------
+    ev.destroy()
+    ev = mk()
+    for k in range(Wm + 1):
+        step(k)
+    torch.cuda.synchronize(dev)
+    ev.profile_enable(True)
+    for k in range(Wm + 1, Wm + 1 + K):
+        step(k)
+    prof = ev.profile_read()
+    ev.profile_enable(False)
+    ev.destroy()
+
+    if world > 1:
+        t = torch.tensor([ms, float(events), float(launches)], device=dev, dtype=torch.float64)
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms, events, launches = float(tmax[0]), float(tsum[1]), int(tsum[2])
+    pxss_rank = E * H * W * S * K
+    value = world * pxss_rank / (ms * 1e-3)
+
+    # ---- roofline of the dominant stage ---------------------------------------------------------------
+    peak, peak_src = hbm_peak()
+    stage_ms = {k: v / K for k, v in prof["ms"].items()}
+    dom = max(stage_ms, key=stage_ms.get)
+    ev_per_step = events / world / K
+    algo_bytes_step = ALGO_BYTES_PER_PIXEL * E * H * W + ALGO_BYTES_PER_EVENT * ev_per_step
+    # the dominant stage is charged the WHOLE step's algorithmic bytes (the other stages are its
+    # helpers: with a fully fused path there is only one kernel); its duration is its own.
+    achieved = algo_bytes_step / (stage_ms[dom] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_step": algo_bytes_step,
+                "stage_ms_per_step": stage_ms, "stage_launches_per_step": {k: v / K for k, v in prof["launches"].items()},
+                "whole_step_frac": algo_bytes_step / (ms / K * 1e-3) / 1e9 / peak}
+
+    out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": K, "warmup": Wm,
+           "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic", "config": workload_config(spec, path_used),
+           "events_per_s": events / (ms * 1e-3), "events_per_step": ev_per_step,
+           "x_realtime": spec.keyframe_dt / (ms / K * 1e-3),
+           "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+
+    # ---- e2e: HOST buffers through evis_step_host + evis_read_events -------------------------------------
+    if not args.no_e2e:
+        Ke = max(1, min(args.e2e_steps, K))
+        hk = []
+        for k in range(Wm + 1 + Ke):
+            hk.append({a: b.cpu().pin_memory() for a, b in kfs[k].items()})
+        del kfs
+        torch.cuda.empty_cache()
+        ev = mk()
+        hbuf = torch.empty((cap, 16), dtype=torch.uint8).pin_memory()
+        harr = hbuf.numpy().view(binding.EVENT_DTYPE).reshape(-1)
+        for k in range(Wm + 1):
+            f = hk[k]
+            ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
+        barrier()
+        tt0 = time.perf_counter()
+        got = 0
+        for k in range(Wm + 1, Wm + 1 + Ke):
+            f = hk[k]
+            ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
+            got += ev.read_events_into(harr)
+        barrier()
+        dt = time.perf_counter() - tt0
+        ev.destroy()
+        if world > 1:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t[0])
+        out["e2e"] = {"value": world * E * H * W * S * Ke / dt, "unit": METRIC, "steps": Ke,
+                      "h2d_bytes_per_step": int(E * H * W * 32), "d2h_bytes_per_step": int(16 * got / Ke),
+                      "ms_per_step": dt / Ke * 1e3,
+                      "api": "evis_step_host (pinned host keyframes) + evis_read_events (pinned host stream)"}
+
+    if rank == 0 and not args.no_cpu:
+        out["cpu_baseline"] = cpu_baseline(scenes.small(spec, seed=spec.seed - 1000 * rank), args.cpu_seconds)
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    from paper_2607_08098_b200 import scenes
+    spec = scenes.config(args.config)
+    if args.envs:
+        spec = scenes.small(spec, num_envs=args.envs, name=f"{spec.name}_E{args.envs}")
+    if args.impl == "reference":
+        run_reference(args, spec)
+    else:
+        run_ours(args, spec)
+
+
+if __name__ == "__main__":
+    main()

@@ -81,7 +81,23 @@ typedef struct {
     int32_t  last_overflow;     /* 1 if the last step overflowed event_capacity                  */
     int32_t  last_motion_violation; /* 1 if a motion vector exceeded the tile-path bound         */
     uint64_t device_bytes;      /* device memory owned by the context                            */
+    uint64_t total_events;      /* true event count summed over every step so far                */
 } evis_info;
+
+/* Per-stage device time, measured with CUDA events on the stream evis_step was given (test and
+ * bench instrumentation; off by default).  Stages: */
+enum { EVIS_STAGE_PREP = 0,     /* a1 + a9: log-luminance, keyframe take-over                     */
+       EVIS_STAGE_CLEAR = 1,    /* global path: z-buffer / directory clears                       */
+       EVIS_STAGE_SPLAT = 2,    /* global path: a2-a4                                             */
+       EVIS_STAGE_RESOLVE = 3,  /* global path: a5-a8 (resolve, event model, compaction)          */
+       EVIS_STAGE_ORDER = 4,    /* a8: deterministic ordering                                     */
+       EVIS_STAGE_TILE = 5,     /* tile path: a2-a8 fused                                         */
+       EVIS_NUM_STAGES = 8 };
+typedef struct {
+    uint64_t steps;                       /* evis_step calls accumulated since enable / last read */
+    uint64_t launches[EVIS_NUM_STAGES];   /* kernels + memsets per stage                          */
+    double   ms[EVIS_NUM_STAGES];         /* device milliseconds per stage, summed                 */
+} evis_profile;
 
 /* Create a context: validates the configuration, allocates all device state.  *out is set only
  * on success.  Errors: INVALID_ARG, CUDA, OOM. */
@@ -123,6 +139,10 @@ int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_st
 
 /* Counters and geometry (synchronises the last step's stream). */
 int evis_get_info(evis_ctx *ctx, evis_info *info);
+
+/* Stage timing: enable/disable (resets the accumulators), read (synchronises, then resets). */
+int evis_profile_enable(evis_ctx *ctx, int on);
+int evis_profile_read(evis_ctx *ctx, evis_profile *out);
 
 /* State access for tests and checkpointing: the carried reference level L_ref and the last
  * warped log frame L_prev, each [E,H,W] float32, to/from HOST memory.  Either may be NULL. */

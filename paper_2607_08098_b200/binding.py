@@ -39,12 +39,20 @@ class evis_info(C.Structure):
     _fields_ = [("path", C.c_int32), ("tile_w", C.c_int32), ("tile_h", C.c_int32), ("halo", C.c_int32),
                 ("steps", C.c_uint64), ("last_events", C.c_uint64), ("last_holes", C.c_uint64),
                 ("kernel_launches", C.c_uint64), ("last_overflow", C.c_int32),
-                ("last_motion_violation", C.c_int32), ("device_bytes", C.c_uint64)]
+                ("last_motion_violation", C.c_int32), ("device_bytes", C.c_uint64), ("total_events", C.c_uint64)]
+
+
+NUM_STAGES = 8
+STAGE_NAMES = ["prep", "clear", "splat", "resolve", "order", "tile", "s6", "s7"]
+
+
+class evis_profile(C.Structure):
+    _fields_ = [("steps", C.c_uint64), ("launches", C.c_uint64 * NUM_STAGES), ("ms", C.c_double * NUM_STAGES)]
 
 
 # every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
-           "evis_get_info", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
+           "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
            "evis_strerror", "evis_last_cuda_error", "evis_version"]
 
 _lib = None
@@ -66,6 +74,8 @@ def load() -> C.CDLL:
     L.evis_read_events.argtypes = [vp, vp, C.c_int, C.c_uint64, u64p]
     L.evis_events_device.argtypes = [vp, C.POINTER(vp), u64p]
     L.evis_get_info.argtypes = [vp, C.POINTER(evis_info)]
+    L.evis_profile_enable.argtypes = [vp, C.c_int]
+    L.evis_profile_read.argtypes = [vp, C.POINTER(evis_profile)]
     L.evis_get_state.argtypes = [vp, vp, vp]
     L.evis_set_state.argtypes = [vp, vp, vp]
     L.evis_debug_read.argtypes = [vp, vp, vp, vp]
@@ -185,6 +195,17 @@ class Evis:
         i = evis_info()
         _check(self._lib.evis_get_info(self._ctx, C.byref(i)), "evis_get_info")
         return i
+
+    def profile_enable(self, on: bool = True) -> None:
+        _check(self._lib.evis_profile_enable(self._ctx, int(on)), "evis_profile_enable")
+
+    def profile_read(self) -> dict:
+        """{'steps': n, 'ms': {stage: device ms summed}, 'launches': {stage: count}} since the last read."""
+        p = evis_profile()
+        _check(self._lib.evis_profile_read(self._ctx, C.byref(p)), "evis_profile_read")
+        return {"steps": int(p.steps),
+                "ms": {STAGE_NAMES[i]: float(p.ms[i]) for i in range(NUM_STAGES) if p.launches[i]},
+                "launches": {STAGE_NAMES[i]: int(p.launches[i]) for i in range(NUM_STAGES) if p.launches[i]}}
 
     def get_state(self) -> Tuple[np.ndarray, np.ndarray]:
         shp = (self.E, self.H, self.W)

@@ -4,13 +4,14 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "kernels.h"
 
 using namespace evis;
 
 static_assert(sizeof(evis_event) == 16, "evis_event is a 16-byte record");
-static_assert(sizeof(evis_config) == 64 && sizeof(evis_info) == 64, "ABI struct layout (binding.py mirrors it)");
+static_assert(sizeof(evis_config) == 64 && sizeof(evis_info) == 72, "ABI struct layout (binding.py mirrors it)");
 
 struct evis_ctx {
     evis_config cfg;
@@ -48,6 +49,13 @@ struct evis_ctx {
     uint64_t last_events, last_holes;
     int last_overflow, last_motion;
     bool have_events;
+
+    // stage timing (evis_profile_*)
+    bool prof_on;
+    struct ProfSpan { int stage; cudaEvent_t a, b; };
+    std::vector<ProfSpan> prof_spans;     // recorded, not yet read
+    std::vector<cudaEvent_t> prof_free;   // event pool
+    evis_profile prof_acc;
 };
 
 namespace {
@@ -82,6 +90,49 @@ cudaError_t dalloc(evis_ctx *ctx, T **p, size_t count)
     return e;
 }
 
+cudaEvent_t prof_event(evis_ctx *ctx)
+{
+    cudaEvent_t e = nullptr;
+    if (!ctx->prof_free.empty()) { e = ctx->prof_free.back(); ctx->prof_free.pop_back(); }
+    else if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return e;
+}
+
+// drain recorded spans into the accumulators (synchronises on the spans' events)
+void prof_drain(evis_ctx *ctx)
+{
+    for (auto &sp : ctx->prof_spans) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(sp.b) == cudaSuccess && cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess)
+            ctx->prof_acc.ms[sp.stage] += (double)ms;
+        else cudaGetLastError();
+        ctx->prof_free.push_back(sp.a);
+        ctx->prof_free.push_back(sp.b);
+    }
+    ctx->prof_spans.clear();
+}
+
+// RAII span: records an event pair around the launches of one stage when profiling is on
+struct Span {
+    evis_ctx *ctx; cudaStream_t st; int stage; cudaEvent_t a;
+    Span(evis_ctx *c, cudaStream_t s, int stg, int launches) : ctx(c), st(s), stage(stg), a(nullptr)
+    {
+        ctx->launches += launches;
+        if (!ctx->prof_on) return;
+        ctx->prof_acc.launches[stage] += launches;
+        a = prof_event(ctx);
+        if (a) cudaEventRecord(a, st);
+    }
+    ~Span()
+    {
+        if (!a) return;
+        cudaEvent_t b = prof_event(ctx);
+        if (!b) { ctx->prof_free.push_back(a); return; }
+        cudaEventRecord(b, st);
+        ctx->prof_spans.push_back({stage, a, b});
+    }
+};
+
 size_t env_size_mb(const char *name, size_t dflt)
 {
     const char *v = getenv(name);
@@ -100,6 +151,9 @@ void free_all(evis_ctx *ctx)
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
     cudaFree(ctx->st_rad); cudaFree(ctx->st_mv); cudaFree(ctx->st_fwd); cudaFree(ctx->st_depth);
     if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
+    prof_drain(ctx);
+    for (cudaEvent_t e : ctx->prof_free) cudaEventDestroy(e);
+    ctx->prof_free.clear();
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
 }
 
@@ -235,9 +289,8 @@ int evis_create(const evis_config *cfg, evis_ctx **out)
     if (cfg->device < 0 || cfg->device >= ndev) return EVIS_ERR_INVALID_ARG;
     DeviceGuard guard(cfg->device);
     if (!guard.ok) return EVIS_ERR_CUDA;
-    evis_ctx *ctx = new (std::nothrow) evis_ctx();
+    evis_ctx *ctx = new (std::nothrow) evis_ctx();     // value-initialised: every POD member is zero
     if (!ctx) return EVIS_ERR_OOM;
-    memset(ctx, 0, sizeof *ctx);
     ctx->cfg = *cfg;
     const int rc = create_impl(ctx);
     if (rc != EVIS_OK) { free_all(ctx); delete ctx; return rc; }
@@ -272,9 +325,12 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     }
     B.has_fwd = mv_fwd != nullptr;
     const bool first = ctx->steps == 0;
-    CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, B.L, B.mv, B.fwd, B.Z,
-                   first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr, st));
-    ctx->launches += 1;
+    if (ctx->prof_on) { ctx->prof_acc.steps += 1; if (ctx->prof_spans.size() > 8192) prof_drain(ctx); }
+    {
+        Span sp(ctx, st, EVIS_STAGE_PREP, 1);
+        CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, B.L, B.mv, B.fwd, B.Z,
+                       first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr, st));
+    }
     ctx->last_stream = st;
     if (first) {
         ctx->h_counters[0] = ctx->h_counters[1] = ctx->h_counters[2] = 0;
@@ -287,9 +343,11 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
 
     ctx->ep.kf = (uint32_t)(ctx->steps - 1);
     EventSink sink{ctx->arrival, ctx->cfg.event_capacity, ctx->counters, ctx->directory};
-    CU(cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), st));
-    CU(cudaMemsetAsync(ctx->directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
-    ctx->launches += 2;
+    {
+        Span sp(ctx, st, EVIS_STAGE_CLEAR, 2);
+        CU(cudaMemsetAsync(ctx->counters, 0, 3 * sizeof(unsigned long long), st));   // [3] accumulates
+        CU(cudaMemsetAsync(ctx->directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
+    }
 
     if (ctx->path == EVIS_PATH_GLOBAL) {
         for (int e0 = 0; e0 < g.E; e0 += ctx->chunk_ne) {
@@ -301,21 +359,24 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 const size_t nd = (size_t)ctx->nset * ni * ne * g.HW, nc = (size_t)ctx->nset * ni * ne * g.HWc;
                 zc.zd = ctx->zmem;
                 zc.zc = ctx->zmem + nd;
-                CU(cudaMemsetAsync(ctx->zmem, 0xFF, (nd + nc) * 8u, st));
-                CU(launch_global_splat(g, zc, A, B, ctx->tab, st));
-                CU(launch_global_resolve(g, zc, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink,
-                                         ctx->counters + 1, ctx->dbg, st));
-                ctx->launches += 3;
+                { Span sp(ctx, st, EVIS_STAGE_CLEAR, 1); CU(cudaMemsetAsync(ctx->zmem, 0xFF, (nd + nc) * 8u, st)); }
+                { Span sp(ctx, st, EVIS_STAGE_SPLAT, 1); CU(launch_global_splat(g, zc, A, B, ctx->tab, st)); }
+                {
+                    Span sp(ctx, st, EVIS_STAGE_RESOLVE, 1);
+                    CU(launch_global_resolve(g, zc, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink,
+                                             ctx->counters + 1, ctx->dbg, st));
+                }
             }
         }
     } else {
+        Span sp(ctx, st, EVIS_STAGE_TILE, 1);
         CU(launch_tile(g, ctx->tile, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink, ctx->counters + 1,
                        ctx->counters + 2, ctx->dbg, st));
-        ctx->launches += 1;
     }
-    int nl = 0;
-    CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, st, &nl));
-    ctx->launches += nl;
+    {
+        Span sp(ctx, st, EVIS_STAGE_ORDER, 3);
+        CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->counters, st));
+    }
     CU(cudaMemcpyAsync(ctx->h_counters, ctx->counters, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     ctx->steps += 1;
     ctx->cur ^= 1;
@@ -401,6 +462,27 @@ int evis_get_info(evis_ctx *ctx, evis_info *info)
     info->last_overflow = ctx->last_overflow;
     info->last_motion_violation = ctx->last_motion;
     info->device_bytes = ctx->device_bytes;
+    info->total_events = ctx->h_counters[3];
+    return EVIS_OK;
+}
+
+int evis_profile_enable(evis_ctx *ctx, int on)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    prof_drain(ctx);
+    memset(&ctx->prof_acc, 0, sizeof ctx->prof_acc);
+    ctx->prof_on = on != 0;
+    return EVIS_OK;
+}
+
+int evis_profile_read(evis_ctx *ctx, evis_profile *out)
+{
+    if (!ctx || !out) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    prof_drain(ctx);
+    *out = ctx->prof_acc;
+    memset(&ctx->prof_acc, 0, sizeof ctx->prof_acc);
     return EVIS_OK;
 }
 

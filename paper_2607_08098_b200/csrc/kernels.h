@@ -68,7 +68,8 @@ cudaError_t launch_tile(const Geom &g, const TilePlan &plan, const Keyframe &A, 
 
 // ---- a8 ordering (order.cu) ----------------------------------------------------------------------
 // directory entry d = (arrival offset, count); ordered stream = chunks concatenated in d order.
+// counters[0] = events of this step; counters[3] += counters[0] (running total over all steps).
 cudaError_t launch_order(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out /*[n]*/,
-                         uint4 *ordered, cudaStream_t st, int *launches);
+                         uint4 *ordered, unsigned long long *counters, cudaStream_t st);
 
 }  // namespace evis

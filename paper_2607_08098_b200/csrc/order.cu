@@ -58,8 +58,9 @@ k_dir_blocksum(const uint2 *__restrict__ dir, uint32_t n, unsigned long long *__
 
 // single block: exclusive scan of the per-block sums in place
 __global__ void __launch_bounds__(1024)
-k_dir_scan_bsum(unsigned long long *__restrict__ bsum, uint32_t nb)
+k_dir_scan_bsum(unsigned long long *__restrict__ bsum, uint32_t nb, unsigned long long *__restrict__ counters)
 {
+    if (threadIdx.x == 0) counters[3] += counters[0];
     __shared__ unsigned long long s_w[33];
     const uint32_t per = (nb + blockDim.x - 1) / blockDim.x;
     const uint32_t lo = threadIdx.x * per, hi = min(lo + per, nb);
@@ -99,13 +100,12 @@ k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *
 }
 
 cudaError_t launch_order(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
-                         cudaStream_t st, int *launches)
+                         unsigned long long *counters, cudaStream_t st)
 {
     const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
     k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum);
-    k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb);
+    k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, counters);
     k_dir_copy<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, ordered, sink.capacity);
-    if (launches) *launches += 3;
     return cudaGetLastError();
 }
 

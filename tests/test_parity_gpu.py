@@ -146,7 +146,8 @@ def test_invariants_p7_p9_on_gpu_output():
             continue
         e = ev.read_events()
         i = e["substep"].astype(np.float64)
-        assert np.all(e["t_off"] >= (i - 1) * dt - 1e-9) and np.all(e["t_off"] <= i * dt + 1e-9)
+        # t_off is binary32: allow one ulp of the largest value (T = 16.7 ms -> ulp 1.9e-9)
+        assert np.all(e["t_off"] >= (i - 1) * dt - 4e-9) and np.all(e["t_off"] <= i * dt + 4e-9)
         w = np.where(e["p"] > 0, spec.c_pos, -spec.c_neg)
         np.add.at(net, (e["env"].astype(np.int64), e["y"].astype(np.int64), e["x"].astype(np.int64)), w)
     lref, lprev = ev.get_state()
