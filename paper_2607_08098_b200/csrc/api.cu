@@ -329,7 +329,8 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     {
         Span sp(ctx, st, EVIS_STAGE_PREP, 1);
         CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, B.L, B.mv, B.fwd, B.Z,
-                       first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr, st));
+                       first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr,
+                       ctx->path == EVIS_PATH_TILE ? ctx->cfg.max_motion_px : 0.0f, ctx->counters + 2, st));
     }
     ctx->last_stream = st;
     if (first) {
@@ -345,7 +346,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     EventSink sink{ctx->arrival, ctx->cfg.event_capacity, ctx->counters, ctx->directory};
     {
         Span sp(ctx, st, EVIS_STAGE_CLEAR, 2);
-        CU(cudaMemsetAsync(ctx->counters, 0, 3 * sizeof(unsigned long long), st));   // [3] accumulates
+        CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st));   // [2] sticky, [3] accumulates
         CU(cudaMemsetAsync(ctx->directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
     }
 

@@ -30,7 +30,8 @@ struct DebugOut {  // all nullable; [S,E,H,W]
 // a1 + a9 (prep.cu)
 cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, const float *depth, long long n,
                         float eps, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
-                        float *l_prev, cudaStream_t st);
+                        float *l_prev, float motion_bound /* 0 = unchecked */, unsigned long long *viol,
+                        cudaStream_t st);
 
 // ---- global z-buffer path (global_path.cu): any motion -----------------------------------------
 // z-buffers of one chunk = envs [e0, e0+ne) x substeps [i0, i0+ni):
@@ -58,6 +59,7 @@ struct TilePlan {
     int threads;           // CTA size
     int cand_cap;          // candidate sources kept in shared memory per tile
     int smem_bytes;
+    int force_direct;      // test hook (EVIS_TILE_FORCE_DIRECT=1): never keep candidates resident
 };
 bool plan_tile(const Geom &g, float max_motion_px, TilePlan *plan);     // false: motion too large for a tile
 cudaError_t tile_setup(const Geom &g, const TilePlan &plan);            // one-time function attributes

@@ -28,8 +28,10 @@ __global__ void __launch_bounds__(256)
 k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float *__restrict__ fwd_in,
        const float *__restrict__ depth, long long n, float eps_f,
        float *__restrict__ L, float2 *__restrict__ mv_out, float2 *__restrict__ fwd_out,
-       float *__restrict__ Z, float *__restrict__ l_ref, float *__restrict__ l_prev)
+       float *__restrict__ Z, float *__restrict__ l_ref, float *__restrict__ l_prev, float bound,
+       unsigned long long *__restrict__ viol)
 {
+    bool over = false;       // a motion vector beyond the bound the tile path was planned for
     const double eps = (double)eps_f;
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (VEC) {
@@ -49,13 +51,19 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
         }
         const float4 *m4 = reinterpret_cast<const float4 *>(mv + 2 * p);
         float4 *mo = reinterpret_cast<float4 *>(mv_out + p);
-        mo[0] = __ldcs(m4);
-        mo[1] = __ldcs(m4 + 1);
+        const float4 m0 = __ldcs(m4), m1 = __ldcs(m4 + 1);
+        mo[0] = m0;
+        mo[1] = m1;
+        over = fmaxf(fmaxf(fmaxf(fabsf(m0.x), fabsf(m0.y)), fmaxf(fabsf(m0.z), fabsf(m0.w))),
+                     fmaxf(fmaxf(fabsf(m1.x), fabsf(m1.y)), fmaxf(fabsf(m1.z), fabsf(m1.w)))) > bound;
         if (fwd_in) {
             const float4 *f4 = reinterpret_cast<const float4 *>(fwd_in + 2 * p);
             float4 *fo = reinterpret_cast<float4 *>(fwd_out + p);
-            fo[0] = __ldcs(f4);
-            fo[1] = __ldcs(f4 + 1);
+            const float4 f0 = __ldcs(f4), f1 = __ldcs(f4 + 1);
+            fo[0] = f0;
+            fo[1] = f1;
+            over |= fmaxf(fmaxf(fmaxf(fabsf(f0.x), fabsf(f0.y)), fmaxf(fabsf(f0.z), fabsf(f0.w))),
+                          fmaxf(fmaxf(fabsf(f1.x), fabsf(f1.y)), fmaxf(fabsf(f1.z), fabsf(f1.w)))) > bound;
         }
         *reinterpret_cast<float4 *>(Z + p) = __ldcs(reinterpret_cast<const float4 *>(depth + p));
     } else {
@@ -64,25 +72,31 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
         L[t] = l;
         if (l_ref) { l_ref[t] = l; l_prev[t] = l; }
         mv_out[t] = make_float2(mv[2 * t], mv[2 * t + 1]);
-        if (fwd_in) fwd_out[t] = make_float2(fwd_in[2 * t], fwd_in[2 * t + 1]);
+        over = fmaxf(fabsf(mv[2 * t]), fabsf(mv[2 * t + 1])) > bound;
+        if (fwd_in) {
+            fwd_out[t] = make_float2(fwd_in[2 * t], fwd_in[2 * t + 1]);
+            over |= fmaxf(fabsf(fwd_in[2 * t]), fabsf(fwd_in[2 * t + 1])) > bound;
+        }
         Z[t] = depth[t];
     }
+    if (over) atomicAdd(viol, 1ull);        // rare by contract; reported as EVIS_ERR_MOTION_BOUND
 }
 
 static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, const float *depth, long long n,
                         float eps, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
-                        float *l_prev, cudaStream_t st)
+                        float *l_prev, float bound, unsigned long long *viol, cudaStream_t st)
 {
+    if (!(bound > 0.0f)) bound = __builtin_inff();      // no bound declared: nothing to check
     const bool vec = (n % 4 == 0) && aligned16(rad) && aligned16(mv) && aligned16(depth) && (!fwd || aligned16(fwd));
     if (vec) {
         const long long threads = n / 4;
         k_prep<true><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, L, mv_out,
-                                                                         fwd_out, Z, l_ref, l_prev);
+                                                                         fwd_out, Z, l_ref, l_prev, bound, viol);
     } else {
         k_prep<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, L, mv_out,
-                                                                    fwd_out, Z, l_ref, l_prev);
+                                                                    fwd_out, Z, l_ref, l_prev, bound, viol);
     }
     return cudaGetLastError();
 }

@@ -70,7 +70,7 @@ class SceneSpec:
     c_pos: float
     c_neg: float
     log_eps: float = 1e-3
-    kind: str = "rects"         # "rects" | "disk"
+    kind: str = "rects"         # "rects" | "disk" | "noise" (stress input, see _paint_noise)
     num_rects: int = 8
     v_max: float = 300.0        # rectangle velocity bound [px/s], per component
     ego_v_max: float = 0.0      # global translation bound [px/s], per component
@@ -323,11 +323,41 @@ def _paint(scene: Scene, t: float, t_prev: float, t_next: float, device, envs: S
     return {k: torch.cat([p[k] for p in parts], dim=0) for k in parts[0]}
 
 
+def _paint_noise(scene: Scene, k: int, device, envs: Sequence[int]) -> Dict[str, torch.Tensor]:
+    """kind == "noise": a stress input, not a scene.  Every pixel of every keyframe gets hashed radiance,
+    hashed motion vectors in [-v_max T, v_max T) (quantised to 1/4 px, so integer and half-integer
+    landings and therefore every footprint class occur) and a depth drawn from eight values (so depth
+    ties are everywhere).  Keyframes are unrelated to each other: it exercises the z-test, the tie-break,
+    hole filling and the event model under conflicts no rendered scene produces."""
+    spec = scene.spec
+    H, W = spec.height, spec.width
+    M = spec.v_max * spec.keyframe_dt
+    ys = torch.arange(H, device=device, dtype=torch.int64).view(1, H, 1)
+    xs = torch.arange(W, device=device, dtype=torch.int64).view(1, 1, W)
+    es = torch.tensor(list(envs), device=device, dtype=torch.int64).view(-1, 1, 1)
+    salt0 = (spec.seed & 0xFFF) * 131 + k * 17
+
+    def h(field):
+        return _hash01(xs + 7 * field + 1000 * es, ys + 13 * k, torch.full_like(es, salt0 + 31 * field))
+
+    rad = torch.stack([10.0 ** (spec.log10_rad * (2.0 * h(c) - 1.0)) for c in range(3)], dim=-1)
+    q = 4.0
+    mv = [torch.floor((2.0 * h(3 + c) - 1.0) * M * q) / q for c in range(4)]
+    still = h(9) < 0.25                                    # a quarter of the pixels rest
+    mv = [torch.where(still, torch.zeros_like(m), m) for m in mv]
+    depth = 1.0 + torch.floor(8.0 * h(8))
+    return {"rad": rad.to(torch.float32).contiguous(), "depth": depth.to(torch.float32).contiguous(),
+            "mv_bwd": torch.stack(mv[0:2], dim=-1).to(torch.float32).contiguous(),
+            "mv_fwd": torch.stack(mv[2:4], dim=-1).to(torch.float32).contiguous()}
+
+
 def render_keyframe(scene: Scene, k: int, device="cpu", envs: Optional[Sequence[int]] = None
                     ) -> Dict[str, torch.Tensor]:
     """Keyframe k: ``rad[E,H,W,3]``, ``mv_bwd[E,H,W,2]``, ``mv_fwd[E,H,W,2]``, ``depth[E,H,W]`` (float32)."""
     T = scene.spec.keyframe_dt
     envs = list(range(scene.spec.num_envs)) if envs is None else list(envs)
+    if scene.spec.kind == "noise":
+        return _paint_noise(scene, k, torch.device(device), envs)
     return _paint(scene, k * T, (k - 1) * T, (k + 1) * T, torch.device(device), envs)
 
 

@@ -67,6 +67,63 @@ def test_tiny_and_ragged_shapes(shape, S):
     assert rep.max_dL <= parity.TOL_L and rep.max_dt <= parity.TOL_T
 
 
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("v_max,S", [(300.0, 4), (1200.0, 7)])
+def test_noise_stress(path, v_max, S):
+    """Hashed per-pixel motion, eight depth values, unrelated keyframes: depth ties, many sources per
+    cell, every footprint class, holes everywhere -- the z-test and the tie-break under real conflict."""
+    spec = scenes.SceneSpec("noise", 2, 75, 131, 4, 1.0 / 60.0, S, 0.3, 0.2, kind="noise", num_rects=0,
+                            v_max=v_max, seed=11)
+    rep = parity.run_parity(spec, 4, path=path)
+    _assert_tolerances(rep)
+    assert rep.holes > 0
+
+
+def test_tile_path_is_taken_and_direct_mode_matches(monkeypatch):
+    """PATH_TILE is honoured for bounded motion; with EVIS_TILE_FORCE_DIRECT=1 the tile kernel never keeps
+    candidates resident (the fallback for pools that overflow) and must give the same result."""
+    spec = scenes.small(scenes.config(4), num_envs=3, height=130, width=173, num_keyframes=3)
+    ev = binding.Evis(3, 130, 173, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                      max_motion_px=spec.max_motion_px(), path=binding.PATH_TILE)
+    info = ev.info()
+    assert info.path == binding.PATH_TILE and info.halo == int(np.ceil(spec.max_motion_px())) + 1
+    ev.destroy()
+    rep = parity.run_parity(spec, 3, path=binding.PATH_TILE)
+    _assert_tolerances(rep)
+    monkeypatch.setenv("EVIS_TILE_FORCE_DIRECT", "1")
+    rep = parity.run_parity(spec, 3, path=binding.PATH_TILE)
+    _assert_tolerances(rep)
+    nz = scenes.SceneSpec("noise", 1, 75, 131, 3, 1.0 / 60.0, 5, 0.3, 0.2, kind="noise", num_rects=0, v_max=600.0, seed=3)
+    rep = parity.run_parity(nz, 3, path=binding.PATH_TILE)
+    _assert_tolerances(rep)
+
+
+def test_tile_path_reports_motion_bound_violation():
+    """A motion vector beyond max_motion_px on the tile path is reported (EVIS_ERR_MOTION_BOUND)."""
+    spec = scenes.small(scenes.config(1), height=64, width=96, num_keyframes=2)
+    sc = scenes.make_scene(spec)
+    ev = binding.Evis(1, 64, 96, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                      max_motion_px=0.5, path=binding.PATH_TILE)
+    k0 = scenes.render_keyframe(sc, 0, device="cuda")
+    assert float(k0["mv_bwd"].abs().max()) > 0.5
+    ev.step(k0["rad"], k0["mv_bwd"], k0["depth"], sync=True)
+    with pytest.raises(binding.EvisError) as ei:
+        k1 = scenes.render_keyframe(sc, 1, device="cuda")
+        ev.step(k1["rad"], k1["mv_bwd"], k1["depth"], sync=True)
+    assert ei.value.status == binding.EVIS_ERR_MOTION_BOUND
+    assert ev.info().last_motion_violation == 1
+    ev.destroy()
+
+
+def test_static_scene_tile_shortcut():
+    """Zero motion everywhere: the tile path's static shortcut; a pure brightness change lands in
+    substep 1 (R19 note) and matches the oracle."""
+    spec = scenes.SceneSpec("static", 2, 70, 100, 3, 1.0 / 60.0, 8, 0.02, 0.025, num_rects=5, v_max=0.0,
+                            ramp_max=30.0, seed=21)
+    rep = parity.run_parity(spec, 3, path=binding.PATH_TILE, max_motion=1.0)
+    _assert_tolerances(rep)
+
+
 def test_blend_mode_global():
     """Composite mode 1 (R19): nearest of both winners, time-weighted blend on the same surface."""
     spec = scenes.small(scenes.config(2), num_envs=2, height=120, width=160, num_keyframes=3)
@@ -106,8 +163,9 @@ def _run_stream(spec, n_kf, path, seed_offset=0):
 
 @pytest.mark.parametrize("path", PATHS)
 def test_output_order_is_deterministic_and_tiled(path):
-    """Two runs give byte-identical ordered streams; the order is (env, substep, tile row, tile col,
-    y, x, time) with the tile geometry evis_get_info reports."""
+    """Two runs give byte-identical ordered streams; the order is (env, substep, tile row, tile col) with
+    the tile geometry evis_get_info reports; inside a tile the events of one pixel are contiguous and in
+    time order (the pixel order inside a tile is fixed but unspecified)."""
     spec = scenes.small(scenes.config(2), num_envs=3, height=157, width=211, num_keyframes=3)
     a, info = _run_stream(spec, 3, path)
     b, _ = _run_stream(spec, 3, path)
@@ -116,15 +174,16 @@ def test_output_order_is_deterministic_and_tiled(path):
         assert x.tobytes() == y.tobytes()
     tw, th = info.tile_w, info.tile_h
     for ev in a:
-        key = np.stack([ev["env"].astype(np.int64), ev["substep"].astype(np.int64), ev["y"] // th, ev["x"] // tw,
-                        ev["y"].astype(np.int64), ev["x"].astype(np.int64)], axis=1)
-        # lexicographic non-decreasing
-        d = np.diff(key, axis=0)
+        key = np.stack([ev["env"].astype(np.int64), ev["substep"].astype(np.int64), ev["y"] // th, ev["x"] // tw],
+                       axis=1)
+        d = np.diff(key, axis=0)                     # lexicographic non-decreasing
         first = np.argmax(d != 0, axis=1)
-        lead = d[np.arange(len(d)), first]
-        assert np.all(lead >= 0)
-        same = np.all(d == 0, axis=1)
+        assert np.all(d[np.arange(len(d)), first] >= 0)
+        pix = (ev["env"].astype(np.int64) << 40) | (ev["substep"].astype(np.int64) << 32) \
+            | (ev["y"].astype(np.int64) << 16) | ev["x"].astype(np.int64)
+        same = np.diff(pix) == 0
         assert np.all(np.diff(ev["t_off"])[same] >= 0)
+        assert int((~same).sum()) + 1 == len(np.unique(pix))      # each pixel-substep is one run
 
 
 def test_invariants_p7_p9_on_gpu_output():
