@@ -38,8 +38,11 @@ struct evis_ctx {
     uint2 *directory;
     uint32_t dir_entries;
     unsigned long long *bsum;
-    unsigned long long *counters;     // device: [0] events, [1] holes, [2] motion violations
+    // device counters.  Reset every step: [0] events, [1] holes, [2] arrival slots handed out,
+    // [3] tile work counter.  Sticky: [4] motion-bound violations, [5] events over all steps.
+    unsigned long long *counters;
     unsigned long long *h_counters;   // pinned host mirror
+    unsigned long long arrival_cap;   // slots of the arrival buffer (capacity + slab slack)
     DebugOut dbg;
 
     // host-buffer entry point staging
@@ -59,6 +62,8 @@ struct evis_ctx {
 };
 
 namespace {
+
+enum { C_EVENTS = 0, C_HOLES = 1, C_ALLOC = 2, C_ITEM = 3, C_MOTION = 4, C_TOTAL = 5, NCOUNTERS = 6 };
 
 struct DeviceGuard {
     int prev;
@@ -223,29 +228,35 @@ int create_impl(evis_ctx *ctx)
     if (ent >= 0xFFFFFFFFull) return EVIS_ERR_INVALID_ARG;
     ctx->dir_entries = (uint32_t)ent;
     CU(dalloc(ctx, &ctx->directory, (size_t)ent));
-    CU(dalloc(ctx, &ctx->bsum, (size_t)(ent / 2048 + 2)));
-    CU(dalloc(ctx, &ctx->arrival, (size_t)c.event_capacity));
+    CU(dalloc(ctx, &ctx->bsum, (size_t)(ent / ORDER_ENTRIES_PER_BLOCK + 2)));
+    if (ctx->path == EVIS_PATH_TILE) CU(tile_setup(g, ctx->tile, c.device));
+    // arrival buffer: the global path packs chunks densely; the tile path hands out slabs, so each
+    // persistent CTA may leave one slab partly used and lose < one chunk at every slab change
+    ctx->arrival_cap = c.event_capacity;
+    if (ctx->path == EVIS_PATH_TILE)
+        ctx->arrival_cap += c.event_capacity / 8 + (unsigned long long)(ctx->tile.ctas + 1) * ctx->tile.slab;
+    if (ctx->arrival_cap > 0xFFFFFFF0ull) ctx->arrival_cap = 0xFFFFFFF0ull;
+    CU(dalloc(ctx, &ctx->arrival, (size_t)ctx->arrival_cap));
     CU(dalloc(ctx, &ctx->ordered, (size_t)c.event_capacity));
-    CU(dalloc(ctx, &ctx->counters, 4));
-    CU(cudaMemset(ctx->counters, 0, 4 * sizeof(unsigned long long)));
-    CU(cudaHostAlloc((void **)&ctx->h_counters, 4 * sizeof(unsigned long long), cudaHostAllocDefault));
-    memset(ctx->h_counters, 0, 4 * sizeof(unsigned long long));
+    CU(dalloc(ctx, &ctx->counters, NCOUNTERS));
+    CU(cudaMemset(ctx->counters, 0, NCOUNTERS * sizeof(unsigned long long)));
+    CU(cudaHostAlloc((void **)&ctx->h_counters, NCOUNTERS * sizeof(unsigned long long), cudaHostAllocDefault));
+    memset(ctx->h_counters, 0, NCOUNTERS * sizeof(unsigned long long));
     if (c.debug_capture) {
         CU(dalloc(ctx, &ctx->dbg.win, P * g.S));
         CU(dalloc(ctx, &ctx->dbg.dir, P * g.S));
         CU(dalloc(ctx, &ctx->dbg.l_hat, P * g.S));
     }
-    if (ctx->path == EVIS_PATH_TILE) CU(tile_setup(g, ctx->tile));
     return EVIS_OK;
 }
 
 int fetch_counters(evis_ctx *ctx)
 {
     if (ctx->last_stream || ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
-    ctx->last_events = ctx->h_counters[0];
-    ctx->last_holes = ctx->h_counters[1];
-    ctx->last_motion = ctx->h_counters[2] != 0;
-    ctx->last_overflow = ctx->last_events > ctx->cfg.event_capacity;
+    ctx->last_events = ctx->h_counters[C_EVENTS];
+    ctx->last_holes = ctx->h_counters[C_HOLES];
+    ctx->last_motion = ctx->h_counters[C_MOTION] != 0;
+    ctx->last_overflow = ctx->last_events > ctx->cfg.event_capacity || ctx->h_counters[C_ALLOC] > ctx->arrival_cap;
     return EVIS_OK;
 }
 
@@ -330,11 +341,11 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         Span sp(ctx, st, EVIS_STAGE_PREP, 1);
         CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, B.L, B.mv, B.fwd, B.Z,
                        first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr,
-                       ctx->path == EVIS_PATH_TILE ? ctx->cfg.max_motion_px : 0.0f, ctx->counters + 2, st));
+                       ctx->path == EVIS_PATH_TILE ? ctx->cfg.max_motion_px : 0.0f, ctx->counters + C_MOTION, st));
     }
     ctx->last_stream = st;
     if (first) {
-        ctx->h_counters[0] = ctx->h_counters[1] = ctx->h_counters[2] = 0;
+        ctx->h_counters[C_EVENTS] = ctx->h_counters[C_HOLES] = ctx->h_counters[C_ALLOC] = 0;
         ctx->steps = 1;
         ctx->cur ^= 1;
         ctx->have_events = true;
@@ -343,10 +354,10 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     }
 
     ctx->ep.kf = (uint32_t)(ctx->steps - 1);
-    EventSink sink{ctx->arrival, ctx->cfg.event_capacity, ctx->counters, ctx->directory};
+    EventSink sink{ctx->arrival, ctx->arrival_cap, ctx->counters + C_ALLOC, ctx->counters + C_EVENTS, ctx->directory};
     {
         Span sp(ctx, st, EVIS_STAGE_CLEAR, 2);
-        CU(cudaMemsetAsync(ctx->counters, 0, 2 * sizeof(unsigned long long), st));   // [2] sticky, [3] accumulates
+        CU(cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), st));   // the per-step counters
         CU(cudaMemsetAsync(ctx->directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
     }
 
@@ -365,20 +376,21 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 {
                     Span sp(ctx, st, EVIS_STAGE_RESOLVE, 1);
                     CU(launch_global_resolve(g, zc, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink,
-                                             ctx->counters + 1, ctx->dbg, st));
+                                             ctx->counters + C_HOLES, ctx->dbg, st));
                 }
             }
         }
     } else {
         Span sp(ctx, st, EVIS_STAGE_TILE, 1);
-        CU(launch_tile(g, ctx->tile, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink, ctx->counters + 1,
-                       ctx->counters + 2, ctx->dbg, st));
+        CU(launch_tile(g, ctx->tile, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink, ctx->counters + C_HOLES,
+                       ctx->counters + C_ITEM, ctx->dbg, st));
     }
     {
         Span sp(ctx, st, EVIS_STAGE_ORDER, 3);
-        CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->counters, st));
+        CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity, ctx->counters + C_EVENTS,
+                        ctx->counters + C_TOTAL, st));
     }
-    CU(cudaMemcpyAsync(ctx->h_counters, ctx->counters, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(ctx->h_counters, ctx->counters, NCOUNTERS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     ctx->steps += 1;
     ctx->cur ^= 1;
     ctx->have_events = true;
@@ -463,7 +475,7 @@ int evis_get_info(evis_ctx *ctx, evis_info *info)
     info->last_overflow = ctx->last_overflow;
     info->last_motion_violation = ctx->last_motion;
     info->device_bytes = ctx->device_bytes;
-    info->total_events = ctx->h_counters[3];
+    info->total_events = ctx->h_counters[C_TOTAL];
     return EVIS_OK;
 }
 

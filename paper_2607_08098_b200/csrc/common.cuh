@@ -28,12 +28,16 @@ struct EventParams {
     uint32_t kf;          // interval index of this step
 };
 
-// Where the compacted stream goes (a8).
+// Where the compacted stream goes (a8).  Space in the arrival buffer is handed out by `alloc`
+// (one atomicAdd per chunk on the global path, one per SLAB of events on the persistent tile path);
+// `counter` accumulates the true number of events.  directory[d] = (arrival offset, count) of chunk d;
+// order.cu lays the chunks out in d order.
 struct EventSink {
-    uint4 *arrival;                 // [capacity] events in arrival order
-    unsigned long long capacity;
+    uint4 *arrival;                 // [arrival_cap] events in arrival order
+    unsigned long long arrival_cap; // < 2^32
+    unsigned long long *alloc;      // next free arrival slot
     unsigned long long *counter;    // total events of this step
-    uint2 *directory;               // [num_entries] (arrival offset, count); capacity < 2^32; see order.cu
+    uint2 *directory;               // [num_entries] (arrival offset, count)
 };
 
 __device__ __forceinline__ unsigned long long umin64(unsigned long long a, unsigned long long b)
@@ -98,18 +102,6 @@ __device__ __forceinline__ int event_count(float l_hat, float l_ref, float c_pos
     return r >= 255.0f ? 255 : (int)r;
 }
 
-// 16-byte event record, layout of evis_event.
-__device__ __forceinline__ uint4 pack_event(int x, int y, int env, int pol, int substep, float t_off,
-                                            uint32_t kf)
-{
-    uint4 r;
-    r.x = (uint32_t)x | ((uint32_t)y << 16);
-    r.y = (uint32_t)env | (((uint32_t)pol & 0xFFu) << 16) | ((uint32_t)substep << 24);
-    r.z = __float_as_uint(t_off);
-    r.w = kf;
-    return r;
-}
-
 // Timestamp of the k-th crossing (R8): linear in log intensity between L_prev and L_hat.
 __device__ __forceinline__ float event_time(int k, int pol, float c, float l_ref, float l_prev, float l_hat,
                                             int substep, float dt)
@@ -122,60 +114,82 @@ __device__ __forceinline__ float event_time(int k, int pol, float c, float l_ref
     return __fmaf_rn(fr, dt, __fmul_rn((float)(substep - 1), dt));
 }
 
-// ---- a8: block-level compaction ------------------------------------------------------------------
-// Every thread of the block calls this once per (tile, substep) with its number of events n.
-// Warp shuffle scan -> block scan over warp totals -> ONE global atomic per block -> each thread
-// gets the arrival offset of its first event.  The (offset, count) of the block's chunk goes to
-// directory[dir_index]; order.cu later lays the chunks out in directory order, which makes the
-// stream deterministic although the atomics arrive in any order.
-// Returns the global arrival offset of this thread's first event; `any` tells whether the block
-// emitted anything (uniform across the block).  NT = threads per block (multiple of 32, <= 1024).
-template <int NT>
-__device__ __forceinline__ unsigned long long block_reserve(int n, const EventSink &sink, uint32_t dir_index,
-                                                            uint32_t *s_warp /* [NT/32 + 2] */, bool &any)
+// ---- a8: compaction ------------------------------------------------------------------------------
+// 16-byte event record from the crossing index k of one pixel-substep.
+__device__ __forceinline__ uint4 make_event(int k, int pol, float c, float l_ref, float l_prev, float l_hat,
+                                            uint32_t xy, int env, int substep, const EventParams &ep)
 {
-    constexpr int NW = NT / 32;
-    any = __syncthreads_or(n > 0) != 0;
-    if (!any) return 0;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint4 r;
+    r.x = xy;
+    r.y = (uint32_t)env | (((uint32_t)pol & 0xFFu) << 16) | ((uint32_t)substep << 24);
+    r.z = __float_as_uint(event_time(k, pol, c, l_ref, l_prev, l_hat, substep, ep.dt));
+    r.w = ep.kf;
+    return r;
+}
+
+// Warp-cooperative emission.  Every lane of a converged warp calls this with the n >= 0 crossings of
+// ITS pixel at this substep; the warp's events go to arrival[off ...] in (lane, k) order and the
+// number written is returned (warp-uniform).  n <= 1 everywhere: ballot/popc ranks, each firing lane
+// stores its own record.  Otherwise: shuffle scan of n, then the lanes take the warp's events 32 at a
+// time -- lane e finds its owner by a 5-step search over the scan and fetches the owner's values by
+// shuffle -- so a pixel with many crossings costs the warp one pass, not n divergent ones.
+__device__ __forceinline__ int warp_emit(const EventSink &sink, unsigned long long off, int n, int pol, float c,
+                                         float l_ref, float l_prev, float l_hat, uint32_t xy, int env, int substep,
+                                         const EventParams &ep)
+{
+    constexpr unsigned FULL = 0xFFFFFFFFu;
+    const unsigned fire = __ballot_sync(FULL, n > 0);
+    if (!fire) return 0;
+    const int lane = threadIdx.x & 31;
+    if (!__ballot_sync(FULL, n > 1)) {
+        const unsigned long long o = off + __popc(fire & ((1u << lane) - 1u));
+        if (n && o < sink.arrival_cap) sink.arrival[o] = make_event(1, pol, c, l_ref, l_prev, l_hat, xy, env, substep, ep);
+        return __popc(fire);
+    }
     int incl = n;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
-        const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+        const int v = __shfl_up_sync(FULL, incl, d);
         if (lane >= d) incl += v;
     }
-    if (lane == 31) s_warp[warp] = (uint32_t)incl;
-    __syncthreads();
-    __shared__ unsigned long long s_base;
-    if (warp == 0) {
-        uint32_t w = lane < NW ? s_warp[lane] : 0u;
-        uint32_t wi = w;
+    const int excl = incl - n, total = __shfl_sync(FULL, incl, 31);
+    const float cs = pol < 0 ? -c : c;                      // polarity rides on the sign of the threshold
+    for (int base = 0; base < total; base += 32) {
+        const int e = base + lane;
+        int s = 0;                                          // owner: the last lane whose first event is <= e
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, wi, d);
-            if (lane >= d) wi += v;
+        for (int d = 16; d >= 1; d >>= 1) {
+            const int t = __shfl_sync(FULL, excl, s + d);
+            if (t <= e) s += d;
         }
-        if (lane < NW) s_warp[lane] = wi - w;             // exclusive warp offsets
-        if (lane == 31) {
-            const unsigned long long base = atomicAdd(sink.counter, (unsigned long long)wi);
-            s_base = base;
-            // chunks that start beyond 2^32 lie beyond any capacity: mark them unreachable
-            sink.directory[dir_index] = make_uint2(base < 0xFFFFFFFFull ? (uint32_t)base : 0xFFFFFFFFu, wi);
-        }
+        const int k = e - __shfl_sync(FULL, excl, s) + 1;
+        const float ocs = __shfl_sync(FULL, cs, s), oref = __shfl_sync(FULL, l_ref, s);
+        const float oprev = __shfl_sync(FULL, l_prev, s), ohat = __shfl_sync(FULL, l_hat, s);
+        const uint32_t oxy = __shfl_sync(FULL, xy, s);
+        const unsigned long long o = off + e;
+        if (e < total && o < sink.arrival_cap)
+            sink.arrival[o] = make_event(k, ocs < 0.0f ? -1 : +1, fabsf(ocs), oref, oprev, ohat, oxy, env, substep, ep);
     }
-    __syncthreads();
-    return s_base + s_warp[warp] + (uint32_t)(incl - n);
+    return total;
 }
 
-__device__ __forceinline__ void write_events(const EventSink &sink, unsigned long long off, int n, int pol,
-                                             float c, float l_ref, float l_prev, float l_hat, int x, int y,
-                                             int env, int substep, const EventParams &ep)
+// Exclusive prefix of this warp among the per-warp event totals s_tot[0..NW) of a block, and the block
+// total.  Every warp computes both from the same array, so no second barrier is needed.
+template <int NW>
+__device__ __forceinline__ uint32_t warp_prefix(const volatile uint32_t *s_tot, uint32_t &block_total)
 {
-    for (int k = 1; k <= n; ++k, ++off) {
-        if (off < sink.capacity)
-            sink.arrival[off] = pack_event(x, y, env, pol, substep,
-                                           event_time(k, pol, c, l_ref, l_prev, l_hat, substep, ep.dt), ep.kf);
+    static_assert(NW <= 32, "one lane per warp");
+    constexpr unsigned FULL = 0xFFFFFFFFu;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t v = lane < NW ? s_tot[lane] : 0u;
+    uint32_t incl = v;
+#pragma unroll
+    for (int d = 1; d < NW; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(FULL, incl, d);
+        if (lane >= d) incl += u;
     }
+    block_total = __shfl_sync(FULL, incl, NW - 1);
+    return __shfl_sync(FULL, incl - v, warp);
 }
 
 }  // namespace evis

@@ -60,18 +60,23 @@ struct TilePlan {
     int cand_cap;          // candidate sources kept in shared memory per tile
     int smem_bytes;
     int force_direct;      // test hook (EVIS_TILE_FORCE_DIRECT=1): never keep candidates resident
+    int ctas;              // persistent grid: SMs x resident CTAs per SM (set by tile_setup)
+    int slab;              // events per arrival slab a CTA reserves with one global atomic
 };
 bool plan_tile(const Geom &g, float max_motion_px, TilePlan *plan);     // false: motion too large for a tile
-cudaError_t tile_setup(const Geom &g, const TilePlan &plan);            // one-time function attributes
+cudaError_t tile_setup(const Geom &g, TilePlan &plan, int device);      // function attributes, persistent grid size
+// next_item: device work counter, zero before the launch (the persistent CTAs draw (env, tile) items from it)
 cudaError_t launch_tile(const Geom &g, const TilePlan &plan, const Keyframe &A, const Keyframe &B,
                         const SubstepTable *tab_dev, float *l_ref, float *l_prev, const EventParams &ep,
-                        const EventSink &sink, unsigned long long *holes, unsigned long long *motion_viol,
+                        const EventSink &sink, unsigned long long *holes, unsigned long long *next_item,
                         const DebugOut &dbg, cudaStream_t st);
 
 // ---- a8 ordering (order.cu) ----------------------------------------------------------------------
-// directory entry d = (arrival offset, count); ordered stream = chunks concatenated in d order.
-// counters[0] = events of this step; counters[3] += counters[0] (running total over all steps).
+// directory entry d = (arrival offset, count); ordered stream = chunks concatenated in d order, cut at
+// `capacity` events.  *step_events = events of this step is added to *total_events (running total).
+constexpr int ORDER_ENTRIES_PER_BLOCK = 512;     // directory entries scanned and copied by one block
 cudaError_t launch_order(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out /*[n]*/,
-                         uint4 *ordered, unsigned long long *counters, cudaStream_t st);
+                         uint4 *ordered, unsigned long long capacity, const unsigned long long *step_events,
+                         unsigned long long *total_events, cudaStream_t st);
 
 }  // namespace evis

@@ -1,11 +1,12 @@
 // tile_path.cu -- rows a2-a8 fused per target tile, z-buffers in shared memory (bounded motion).
 //
-// One CTA owns one target tile (tw x th pixels, <= 64 x 32) of one env and runs ALL S substeps of
-// the keyframe interval, so the keyframes are read once, L_ref / L_prev stay in registers and only
-// events are written (north_star).  Sources that can reach the tile lie inside the tile grown by
-// the halo h = ceil(max_motion_px) + 1 ("halo sized from the motion bound").
+// Persistent kernel: one CTA per SM takes (env, tile) work items from a global counter.  For its
+// tile (tw x th <= 64 x 32 target pixels) a CTA runs ALL S substeps of the keyframe interval, so the
+// keyframes are read once, L_ref / L_prev stay in registers and only events are written
+// (north_star).  Sources that can reach the tile lie inside the tile grown by the halo
+// h = ceil(max_motion_px) + 1 ("halo sized from the motion bound").
 //
-//   stage      once per tile and direction: scan the halo region R, keep the sources whose swept
+//   stage      once per tile and direction: scan the halo region, keep the sources whose swept
 //              landing box can touch the tile ("candidates": position, displacement, own depth, far
 //              endpoint depth of Eq. 7) in shared memory.  Direction A is staged lazily, only when
 //              some substep of this tile has a pixel B does not reach (A fills holes).
@@ -18,29 +19,42 @@
 //              barrier, re-check; a round in which no thread had to store proves every cell holds
 //              the minimum of the keys offered to it (each thread only ever lowers a cell, and every
 //              candidate re-checks its own key after the last store).  Deterministic: the result is
-//              the minimum, whatever the interleaving.
+//              the minimum, whatever the interleaving.  Direction A only offers the candidates that
+//              land inside the bounding box of this substep's holes.
 //   resolve    per target pixel: minimum over zd and the four cells that can cover it, composite
 //              (the direction bit makes "B primary, A fills holes" a plain minimum), gather L.
-//   events     Eq. 4 + timestamps (R8) + block compaction with ONE global atomic per (tile, substep).
+//   events     Eq. 4 + timestamps (R8).  Per-warp totals -> one barrier -> every warp derives its own
+//              offset inside the (tile, substep) chunk; the chunk's space comes from a slab of the
+//              arrival buffer the CTA owns (one global atomic per T_SLAB events, not per chunk);
+//              warp-cooperative writes (common.cuh).  directory[(env, substep, tile)] records the
+//              chunk so that order.cu can lay the stream out deterministically.
 //
-// A tile whose candidates all have zero motion and valid depth is
-// static: every substep reproduces L_B, no splat is needed (bit-identical to the general path).
+// Barriers per substep in the common case (no hole, no z conflict): after the z clear, after the
+// optimistic stores, after check + gather + event count.
+//
+// A tile whose candidates all have zero motion and valid depth is static: every substep reproduces
+// L_B, no splat is needed (bit-identical to the general path).
 #include <cstdlib>
 
 #include "kernels.h"
 
 namespace evis {
 
-constexpr int T_NT = 512;            // threads per CTA
-constexpr int T_TPT = 4;             // targets per thread  (T_NT * T_TPT >= tw * th)
-constexpr int T_CAP = 3584;          // resident candidates per direction
-constexpr int T_CPT = T_CAP / T_NT;  // candidates per thread (7)
+constexpr int T_NT = 512;                       // threads per CTA
+constexpr int T_NW = T_NT / 32;
 constexpr int T_MAX_TW = 64, T_MAX_TH = 32;
+constexpr int T_TPT = T_MAX_TW * T_MAX_TH / T_NT;   // targets per thread (4)
+constexpr int T_CAP = 4608;                     // resident candidates per direction
+constexpr int T_CPT = T_CAP / T_NT;             // candidates per thread (9)
+constexpr int T_SLAB = 8192;                    // events per arrival slab
 constexpr uint32_t A_NONE = 0xFFFFFFFFu;
+static_assert(T_CAP % T_NT == 0 && T_TPT * T_NT == T_MAX_TW * T_MAX_TH, "tile constants");
 
 struct TileArgs {
     Geom g;
     int tw, th, halo, tiles_x, tiles_y, force_direct;
+    uint32_t num_items;                 // E * tiles_y * tiles_x
+    unsigned long long *next_item;      // work counter (reset every step)
     const float *LA, *LB, *ZA, *ZB;
     const float2 *mvA, *fwdA, *mvB;     // fwdA nullable (R12)
     const SubstepTable *tab;
@@ -69,7 +83,6 @@ struct TileGeo {
 
 __device__ __forceinline__ bool zput(volatile unsigned long long *z, uint32_t a, unsigned long long key)
 {
-    if (a == A_NONE) return false;
     const unsigned long long cur = z[a];
     if (key < cur) { z[a] = key; return true; }
     return false;
@@ -116,11 +129,13 @@ __device__ __forceinline__ bool candidate(const TileArgs &a, const TileGeo &t, s
     return true;
 }
 
-__device__ __forceinline__ bool land_dir(int dir, float x, float y, float dx, float dy, float zo, float zf, float f,
-                                         float g, uint32_t src, int W, int H, Landing &L)
+// q of Eq. 5 for a candidate of direction DIR at time weights (f, g): B moves by g m_B, A by f d_A.
+template <int DIR>
+__device__ __forceinline__ bool land_dir(float x, float y, float dx, float dy, float zo, float zf, float f, float g,
+                                         uint32_t src, int W, int H, Landing &L)
 {
     // B: q = p + (1-f) m_B, Za = far, Zb = own.   A: q = p + f d_A, Za = own, Zb = far.   (Eq. 5, 7)
-    if (dir == 0) return land(x, y, dx, dy, g, f, g, zf, zo, src, 0ull, W, H, L);
+    if (DIR == 0) return land(x, y, dx, dy, g, f, g, zf, zo, src, 0ull, W, H, L);
     return land(x, y, dx, dy, f, f, g, zo, zf, src, KEY_DIR_A, W, H, L);
 }
 
@@ -180,47 +195,57 @@ __device__ int stage(const TileArgs &a, const TileGeo &t, size_t eoff, int dir, 
     return (int)*s_count;
 }
 
-// ---- splat of one direction at one substep --------------------------------------------------------
+// ---- splat of one resident direction at one substep: optimistic stores, then the re-checks ---------
+// Hole box of direction A (float, inclusive): only sources with q inside it can cover a hole.
+struct Box { float x0, y0, x1, y1; };
+
 template <int DIR>
-__device__ __forceinline__ void splat_resident(volatile unsigned long long *z, const Pool &pool, int base, int n,
-                                               float f, float g, const TileGeo &t)
+__device__ __forceinline__ void splat_store(volatile unsigned long long *z, const Pool &pool, int base, int n, float f,
+                                            float g, const TileGeo &t, const Box &box, unsigned long long (&key)[T_CPT],
+                                            uint32_t (&adr)[T_CPT])
 {
-    unsigned long long key[T_CPT];
-    uint32_t adr[T_CPT];                       // a0 | a1 << 16, 0xFFFF = none
 #pragma unroll
     for (int j = 0; j < T_CPT; ++j) {
         const int s = j * T_NT + threadIdx.x;
-        adr[j] = 0xFFFFFFFFu;
+        adr[j] = 0xFFFFFFFFu;                   // a0 | a1 << 16, 0xFFFF = none
         key[j] = KEY_EMPTY;
         if (s < n) {
             const uint32_t pos = pool.pos[base + s];
             const int x = (int)(pos & 0xFFFFu), y = (int)(pos >> 16);
+            const float dx = pool.dx[base + s], dy = pool.dy[base + s];
+            if (DIR == 1) {                     // cheap reject: lands outside the hole box (same q as land())
+                const float qx = __fmaf_rn(f, dx, (float)x), qy = __fmaf_rn(f, dy, (float)y);
+                if (!(qx >= box.x0 && qx <= box.x1 && qy >= box.y0 && qy <= box.y1)) continue;
+            }
             Landing L;
-            if (land_dir(DIR, (float)x, (float)y, pool.dx[base + s], pool.dy[base + s], pool.zo[base + s],
-                         pool.zf[base + s], f, g, (uint32_t)(y * t.W + x), t.W, t.H, L)) {
+            if (land_dir<DIR>((float)x, (float)y, dx, dy, pool.zo[base + s], pool.zf[base + s], f, g,
+                              (uint32_t)(y * t.W + x), t.W, t.H, L)) {
                 uint32_t a0, a1;
                 tile_addr(L, t, a0, a1);
                 adr[j] = (a0 & 0xFFFFu) | (a1 << 16);
                 key[j] = L.key;
-                zput(z, a0, L.key);
-                zput(z, a1, L.key);
+                if (a0 != A_NONE) zput(z, a0, L.key);
+                if (a1 != A_NONE) zput(z, a1, L.key);
             }
         }
     }
-    bool fail;
-    do {
-        __syncthreads();
-        fail = false;
+}
+
+__device__ __forceinline__ bool splat_check(volatile unsigned long long *z, const unsigned long long (&key)[T_CPT],
+                                            const uint32_t (&adr)[T_CPT])
+{
+    bool fail = false;
 #pragma unroll
-        for (int j = 0; j < T_CPT; ++j) {
-            const uint32_t a0 = adr[j] & 0xFFFFu, a1 = adr[j] >> 16;
-            if (a0 != 0xFFFFu) fail |= zput(z, a0, key[j]);
-            if (a1 != 0xFFFFu) fail |= zput(z, a1, key[j]);
-        }
-    } while (__syncthreads_or(fail));
+    for (int j = 0; j < T_CPT; ++j) {
+        const uint32_t a0 = adr[j] & 0xFFFFu, a1 = adr[j] >> 16;
+        if (a0 != 0xFFFFu) fail |= zput(z, a0, key[j]);
+        if (a1 != 0xFFFFu) fail |= zput(z, a1, key[j]);
+    }
+    return fail;
 }
 
 // Non-resident direction (more candidates than the pool holds): walk the halo region every round.
+// Leaves the final minima in z (ends with a barrier).
 template <int DIR>
 __device__ void splat_direct(volatile unsigned long long *z, const TileArgs &a, const TileGeo &t, size_t eoff,
                              float f, float g)
@@ -236,11 +261,11 @@ __device__ void splat_direct(volatile unsigned long long *z, const TileArgs &a, 
             float dx, dy, zo, zf;
             if (!candidate(a, t, eoff, DIR, x, y, dx, dy, zo, zf)) continue;
             Landing L;
-            if (!land_dir(DIR, (float)x, (float)y, dx, dy, zo, zf, f, g, (uint32_t)(y * t.W + x), t.W, t.H, L)) continue;
+            if (!land_dir<DIR>((float)x, (float)y, dx, dy, zo, zf, f, g, (uint32_t)(y * t.W + x), t.W, t.H, L)) continue;
             uint32_t a0, a1;
             tile_addr(L, t, a0, a1);
-            fail |= zput(z, a0, L.key);
-            fail |= zput(z, a1, L.key);
+            if (a0 != A_NONE) fail |= zput(z, a0, L.key);
+            if (a1 != A_NONE) fail |= zput(z, a1, L.key);
         }
     } while (__syncthreads_or(fail));
 }
@@ -249,19 +274,13 @@ __device__ void splat_direct(volatile unsigned long long *z, const TileArgs &a, 
 __global__ void __launch_bounds__(T_NT, 1) k_tile(const TileArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ uint32_t s_warp[T_NT / 32 + 2];
-    __shared__ uint32_t s_count, s_holes;
+    __shared__ uint32_t s_tot[2][T_NW];         // per-warp event totals (parity of the substep)
+    __shared__ uint32_t s_flag[2][2];           // [parity][0 = a z re-check stored, 1 = a target is a hole]
+    __shared__ int s_box[4];                    // hole bounding box of the substep (tile coordinates)
+    __shared__ uint32_t s_count;
+    __shared__ unsigned long long s_item, s_slab;
 
-    TileGeo t;
-    t.W = a.g.W; t.H = a.g.H;
-    t.tw = a.tw; t.th = a.th;
-    t.X0 = blockIdx.x * a.tw; t.Y0 = blockIdx.y * a.th;
-    t.RX0 = max(t.X0 - a.halo, 0); t.RY0 = max(t.Y0 - a.halo, 0);
-    t.RW = min(t.X0 + a.tw + a.halo, t.W) - t.RX0;
-    t.RH = min(t.Y0 + a.th + a.halo, t.H) - t.RY0;
-    t.zc_off = a.tw * a.th; t.zc_w = a.tw + 1;
-    const int zn = t.zc_off + (a.tw + 1) * (a.th + 1);
-
+    const int zn = a.tw * a.th + (a.tw + 1) * (a.th + 1);
     volatile unsigned long long *z = reinterpret_cast<volatile unsigned long long *>(smem_raw);
     Pool pool;
     {
@@ -272,104 +291,200 @@ __global__ void __launch_bounds__(T_NT, 1) k_tile(const TileArgs a)
         pool.zo = reinterpret_cast<float *>(p); p += 2 * T_CAP * 4;
         pool.zf = reinterpret_cast<float *>(p);
     }
-    const int env = blockIdx.z;
-    const size_t eoff = (size_t)env * a.g.HW;
-    const float *la = a.LA + eoff, *lb = a.LB + eoff;
-    if (threadIdx.x == 0) s_holes = 0;
-
-    // my target pixels (lane-consecutive: conflict-free shared-memory access)
-    int tx[T_TPT], ty[T_TPT], tp[T_TPT];
-    bool in[T_TPT];
-    float l_ref[T_TPT], l_prev[T_TPT];
-    int n_in = 0;
-#pragma unroll
-    for (int j = 0; j < T_TPT; ++j) {
-        const int tt = j * T_NT + threadIdx.x;
-        ty[j] = tt / a.tw; tx[j] = tt - ty[j] * a.tw;
-        in[j] = tt < t.zc_off && t.X0 + tx[j] < t.W && t.Y0 + ty[j] < t.H;
-        tp[j] = (t.Y0 + ty[j]) * t.W + t.X0 + tx[j];
-        l_ref[j] = l_prev[j] = 0.f;
-        if (in[j]) { l_ref[j] = a.l_ref[eoff + tp[j]]; l_prev[j] = a.l_prev[eoff + tp[j]]; ++n_in; }
-    }
-
-    uint32_t flags = 0;
-    int nB = stage(a, t, eoff, 0, pool, 0, &s_count, flags);
-    if (a.force_direct) nB = T_CAP + 1;
-    int nA = -1;
-    // static tile: every candidate rests (zero displacement, ordinary depth).  Then each pixel of the
-    // tile is reached by itself alone (single-pixel footprint, R14), at every substep: L_hat = L_B.
-    const bool is_static = !__syncthreads_or((int)flags);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr unsigned FULL = 0xFFFFFFFFu;
+    // arrival slab owned by this CTA: [cursor, slab_end); replicated in every thread (block-uniform)
+    unsigned long long cursor = 0, slab_end = 0;
     uint32_t my_holes = 0;
+    const uint32_t tiles_per_env = (uint32_t)(a.tiles_x * a.tiles_y);
 
-    for (int i = 1; i <= a.g.S; ++i) {
-        const float f = a.tab->f[i], g = a.tab->g[i];
-        unsigned long long key[T_TPT];
-        if (is_static) {
+    for (;;) {
+        if (threadIdx.x == 0) s_item = atomicAdd(a.next_item, 1ull);
+        __syncthreads();
+        const unsigned long long item64 = s_item;
+        if (item64 >= a.num_items) break;
+        const uint32_t item = (uint32_t)item64;
+        const int env = (int)(item / tiles_per_env);
+        const uint32_t tile_id = item - (uint32_t)env * tiles_per_env;
+        const int by = (int)(tile_id / (uint32_t)a.tiles_x), bx = (int)(tile_id - (uint32_t)by * a.tiles_x);
+
+        TileGeo t;
+        t.W = a.g.W; t.H = a.g.H;
+        t.tw = a.tw; t.th = a.th;
+        t.X0 = bx * a.tw; t.Y0 = by * a.th;
+        t.RX0 = max(t.X0 - a.halo, 0); t.RY0 = max(t.Y0 - a.halo, 0);
+        t.RW = min(t.X0 + a.tw + a.halo, t.W) - t.RX0;
+        t.RH = min(t.Y0 + a.th + a.halo, t.H) - t.RY0;
+        t.zc_off = a.tw * a.th; t.zc_w = a.tw + 1;
+        const size_t eoff = (size_t)env * a.g.HW;
+        const float *la = a.LA + eoff, *lb = a.LB + eoff;
+
+        // my target pixels (lane-consecutive: conflict-free shared-memory access)
+        int tx[T_TPT], ty[T_TPT], tp[T_TPT];
+        bool in[T_TPT];
+        float l_ref[T_TPT], l_prev[T_TPT];
 #pragma unroll
-            for (int j = 0; j < T_TPT; ++j) key[j] = in[j] ? (unsigned long long)(uint32_t)tp[j] : KEY_EMPTY;
-        } else {
-            for (int k = threadIdx.x; k < zn; k += T_NT) z[k] = KEY_EMPTY;
-            __syncthreads();
-            if (nB <= T_CAP) splat_resident<0>(z, pool, 0, nB, f, g, t);
-            else splat_direct<0>(z, a, t, eoff, f, g);
-            bool hole = false;
+        for (int j = 0; j < T_TPT; ++j) {
+            const int tt = j * T_NT + threadIdx.x;
+            ty[j] = tt / a.tw; tx[j] = tt - ty[j] * a.tw;
+            in[j] = tt < t.zc_off && t.X0 + tx[j] < t.W && t.Y0 + ty[j] < t.H;
+            tp[j] = (t.Y0 + ty[j]) * t.W + t.X0 + tx[j];
+            l_ref[j] = l_prev[j] = 0.f;
+            if (in[j]) { l_ref[j] = a.l_ref[eoff + tp[j]]; l_prev[j] = a.l_prev[eoff + tp[j]]; }
+        }
+
+        uint32_t flags = 0;
+        int nB = stage(a, t, eoff, 0, pool, 0, &s_count, flags);
+        if (a.force_direct) nB = T_CAP + 1;
+        int nA = -1;
+        // static tile: every candidate rests (zero displacement, ordinary depth).  Then each pixel of the
+        // tile is reached by itself alone (single-pixel footprint, R14), at every substep: L_hat = L_B.
+        const bool is_static = !__syncthreads_or((int)flags);
+
+        for (int i = 1; i <= a.g.S; ++i) {
+            const int par = i & 1;
+            const float f = a.tab->f[i], g = a.tab->g[i];
+            unsigned long long key[T_TPT];
+            bool any_hole = false;
+            if (is_static) {
+#pragma unroll
+                for (int j = 0; j < T_TPT; ++j) key[j] = in[j] ? (unsigned long long)(uint32_t)tp[j] : KEY_EMPTY;
+            } else {
+                for (int k = threadIdx.x; k < zn; k += T_NT) z[k] = KEY_EMPTY;
+                if (threadIdx.x == 0) {
+                    s_flag[par][0] = 0u; s_flag[par][1] = 0u;
+                    s_box[0] = 0x7FFFFFFF; s_box[1] = 0x7FFFFFFF; s_box[2] = -1; s_box[3] = -1;
+                }
+                __syncthreads();
+                bool fail = false;
+                if (nB <= T_CAP) {
+                    unsigned long long ck[T_CPT];
+                    uint32_t ca[T_CPT];
+                    const Box none = {0.f, 0.f, 0.f, 0.f};
+                    splat_store<0>(z, pool, 0, nB, f, g, t, none, ck, ca);
+                    __syncthreads();
+                    fail = splat_check(z, ck, ca);
+                    if (fail) s_flag[par][0] = 1u;
+                    // gather optimistically: final unless some re-check stored (then redone below)
+                    bool hole = false;
+#pragma unroll
+                    for (int j = 0; j < T_TPT; ++j) {
+                        key[j] = in[j] ? tile_gather(z, t, tx[j], ty[j]) : 0ull;
+                        hole |= key[j] == KEY_EMPTY;
+                    }
+                    if (hole) s_flag[par][1] = 1u;
+                    __syncthreads();
+                    if (s_flag[par][0]) {                       // rare: finish the fixed point, gather again
+                        do { fail = splat_check(z, ck, ca); } while (__syncthreads_or(fail));
+                        hole = false;
+#pragma unroll
+                        for (int j = 0; j < T_TPT; ++j) {
+                            key[j] = in[j] ? tile_gather(z, t, tx[j], ty[j]) : 0ull;
+                            hole |= key[j] == KEY_EMPTY;
+                        }
+                        any_hole = __syncthreads_or(hole) != 0;
+                    } else any_hole = s_flag[par][1] != 0u;
+                } else {
+                    splat_direct<0>(z, a, t, eoff, f, g);
+                    bool hole = false;
+#pragma unroll
+                    for (int j = 0; j < T_TPT; ++j) {
+                        key[j] = in[j] ? tile_gather(z, t, tx[j], ty[j]) : 0ull;
+                        hole |= key[j] == KEY_EMPTY;
+                    }
+                    any_hole = __syncthreads_or(hole) != 0;
+                }
+                if (any_hole) {                                 // A fills only B's holes
+                    if (nA < 0) { nA = stage(a, t, eoff, 1, pool, T_CAP, &s_count, flags); if (a.force_direct) nA = T_CAP + 1; }
+                    // bounding box of the holes (tile coordinates)
+                    int hx0 = 0x7FFFFFFF, hy0 = 0x7FFFFFFF, hx1 = -1, hy1 = -1;
+#pragma unroll
+                    for (int j = 0; j < T_TPT; ++j)
+                        if (in[j] && key[j] == KEY_EMPTY) {
+                            hx0 = min(hx0, tx[j]); hx1 = max(hx1, tx[j]); hy0 = min(hy0, ty[j]); hy1 = max(hy1, ty[j]);
+                        }
+                    hx0 = __reduce_min_sync(FULL, hx0); hy0 = __reduce_min_sync(FULL, hy0);
+                    hx1 = __reduce_max_sync(FULL, hx1); hy1 = __reduce_max_sync(FULL, hy1);
+                    if (lane == 0 && hx1 >= 0) {
+                        atomicMin(&s_box[0], hx0); atomicMin(&s_box[1], hy0); atomicMax(&s_box[2], hx1); atomicMax(&s_box[3], hy1);
+                    }
+                    __syncthreads();
+                    if (nA <= T_CAP) {
+                        // a source covers pixel h iff floor(q) is h-1 or h: q in [h-1, h+1)
+                        const Box box = {(float)(t.X0 + s_box[0] - 1), (float)(t.Y0 + s_box[1] - 1),
+                                         (float)(t.X0 + s_box[2] + 1), (float)(t.Y0 + s_box[3] + 1)};
+                        unsigned long long ck[T_CPT];
+                        uint32_t ca[T_CPT];
+                        splat_store<1>(z, pool, T_CAP, nA, f, g, t, box, ck, ca);
+                        do { __syncthreads(); fail = splat_check(z, ck, ca); } while (__syncthreads_or(fail));
+                    } else splat_direct<1>(z, a, t, eoff, f, g);
+#pragma unroll
+                    for (int j = 0; j < T_TPT; ++j)
+                        if (in[j] && key[j] == KEY_EMPTY) key[j] = tile_gather(z, t, tx[j], ty[j]);
+                }
+            }
+            // composite (a5) + event model (a6)
+            float l_hat[T_TPT], c[T_TPT];
+            int n[T_TPT], pol[T_TPT], n_tot = 0;
 #pragma unroll
             for (int j = 0; j < T_TPT; ++j) {
-                key[j] = in[j] ? tile_gather(z, t, tx[j], ty[j]) : 0ull;
-                hole |= key[j] == KEY_EMPTY;
+                n[j] = 0; pol[j] = 0; c[j] = 1.f; l_hat[j] = l_prev[j];
+                if (!in[j]) continue;
+                uint32_t widx = IDX_NONE;
+                int wdir = 3;
+                if (key[j] != KEY_EMPTY) {
+                    widx = (uint32_t)key[j];
+                    wdir = (int)(key[j] >> 63);
+                    l_hat[j] = __ldg((wdir ? la : lb) + widx);
+                } else ++my_holes;                            // R20: hold the previous value
+                if (a.dbg.win) {
+                    const size_t o = ((size_t)(i - 1) * a.g.E + env) * a.g.HW + tp[j];
+                    a.dbg.win[o] = widx; a.dbg.dir[o] = (uint8_t)wdir; a.dbg.l_hat[o] = l_hat[j];
+                }
+                n[j] = event_count(l_hat[j], l_ref[j], a.ep.c_pos, a.ep.c_neg, pol[j], c[j]);   // Eq. 4
+                n_tot += n[j];
             }
-            if (__syncthreads_or(hole)) {               // A fills only B's holes
-                if (nA < 0) { nA = stage(a, t, eoff, 1, pool, T_CAP, &s_count, flags); if (a.force_direct) nA = T_CAP + 1; }
-                if (nA <= T_CAP) splat_resident<1>(z, pool, T_CAP, nA, f, g, t);
-                else splat_direct<1>(z, a, t, eoff, f, g);
+            // a8: per-warp totals -> one barrier -> offsets inside the (tile, substep) chunk
+            const uint32_t wtot = (uint32_t)__reduce_add_sync(FULL, n_tot);
+            if (lane == 0) s_tot[par][warp] = wtot;
+            __syncthreads();
+            uint32_t btot;
+            const uint32_t wbase = warp_prefix<T_NW>(s_tot[par], btot);
+            if (btot) {                                         // block-uniform
+                if (cursor + btot > slab_end) {                 // block-uniform: take a new slab
+                    const unsigned long long want = btot > (uint32_t)T_SLAB ? btot : (unsigned long long)T_SLAB;
+                    if (threadIdx.x == 0) s_slab = atomicAdd(a.sink.alloc, want);
+                    __syncthreads();
+                    cursor = s_slab; slab_end = cursor + want;
+                }
+                unsigned long long off = cursor + wbase;
+                if (threadIdx.x == 0) {
+                    const uint32_t dir_index = ((uint32_t)env * a.g.S + (i - 1)) * tiles_per_env + tile_id;
+                    a.sink.directory[dir_index] = make_uint2(cursor < 0xFFFFFFFFull ? (uint32_t)cursor : 0xFFFFFFFFu, btot);
+                    atomicAdd(a.sink.counter, (unsigned long long)btot);
+                }
+                cursor += btot;
+                if (wtot) {                                     // warp-uniform
 #pragma unroll
-                for (int j = 0; j < T_TPT; ++j)
-                    if (in[j] && key[j] == KEY_EMPTY) key[j] = tile_gather(z, t, tx[j], ty[j]);
+                    for (int j = 0; j < T_TPT; ++j) {
+                        off += warp_emit(a.sink, off, n[j], pol[j], c[j], l_ref[j], l_prev[j], l_hat[j],
+                                         (uint32_t)(t.X0 + tx[j]) | ((uint32_t)(t.Y0 + ty[j]) << 16), env, i, a.ep);
+                        if (n[j] > 0) l_ref[j] = __fmaf_rn((float)(pol[j] * n[j]), c[j], l_ref[j]);
+                    }
+                }
             }
-        }
-        // composite (a5) + event model (a6)
-        float l_hat[T_TPT], c[T_TPT];
-        int n[T_TPT], pol[T_TPT], n_tot = 0;
 #pragma unroll
-        for (int j = 0; j < T_TPT; ++j) {
-            n[j] = 0; pol[j] = 0; c[j] = 1.f; l_hat[j] = l_prev[j];
-            if (!in[j]) continue;
-            uint32_t widx = IDX_NONE;
-            int wdir = 3;
-            if (key[j] != KEY_EMPTY) {
-                widx = (uint32_t)key[j];
-                wdir = (int)(key[j] >> 63);
-                l_hat[j] = __ldg((wdir ? la : lb) + widx);
-            } else ++my_holes;                            // R20: hold the previous value
-            if (a.dbg.win) {
-                const size_t o = ((size_t)(i - 1) * a.g.E + env) * a.g.HW + tp[j];
-                a.dbg.win[o] = widx; a.dbg.dir[o] = (uint8_t)wdir; a.dbg.l_hat[o] = l_hat[j];
-            }
-            n[j] = event_count(l_hat[j], l_ref[j], a.ep.c_pos, a.ep.c_neg, pol[j], c[j]);   // Eq. 4
-            n_tot += n[j];
+            for (int j = 0; j < T_TPT; ++j) l_prev[j] = l_hat[j];
+            // static tile: once a substep is silent nothing changes any more (same L_hat, same L_ref)
+            if (is_static && !btot && !a.dbg.win) break;
         }
-        const uint32_t dir_index = (((uint32_t)env * a.g.S + (i - 1)) * a.tiles_y + blockIdx.y) * a.tiles_x + blockIdx.x;
-        bool any;
-        unsigned long long off = block_reserve<T_NT>(n_tot, a.sink, dir_index, s_warp, any);
 #pragma unroll
-        for (int j = 0; j < T_TPT; ++j) {
-            if (n[j] > 0) {
-                write_events(a.sink, off, n[j], pol[j], c[j], l_ref[j], l_prev[j], l_hat[j], t.X0 + tx[j], t.Y0 + ty[j],
-                             env, i, a.ep);
-                off += n[j];
-                l_ref[j] = __fmaf_rn((float)(pol[j] * n[j]), c[j], l_ref[j]);
-            }
-            l_prev[j] = l_hat[j];
-        }
-        // static tile: once a substep is silent nothing changes any more (same L_hat, same L_ref)
-        if (is_static && !any && !a.dbg.win) break;
+        for (int j = 0; j < T_TPT; ++j)
+            if (in[j]) { a.l_ref[eoff + tp[j]] = l_ref[j]; a.l_prev[eoff + tp[j]] = l_prev[j]; }
+        __syncthreads();        // s_item, s_tot, the pool and z are reused by the next item
     }
-#pragma unroll
-    for (int j = 0; j < T_TPT; ++j)
-        if (in[j]) { a.l_ref[eoff + tp[j]] = l_ref[j]; a.l_prev[eoff + tp[j]] = l_prev[j]; }
-    if (my_holes) atomicAdd(&s_holes, my_holes);
-    __syncthreads();
-    if (threadIdx.x == 0 && s_holes) atomicAdd(a.holes, (unsigned long long)s_holes);
+    my_holes = __reduce_add_sync(FULL, my_holes);
+    if (lane == 0 && my_holes) atomicAdd(a.holes, (unsigned long long)my_holes);
 }
 
 // ---- host side ----------------------------------------------------------------------------------------
@@ -400,29 +515,41 @@ bool plan_tile(const Geom &g, float max_motion_px, TilePlan *plan)
     plan->threads = T_NT;
     plan->cand_cap = T_CAP;
     plan->smem_bytes = tile_smem_bytes(plan->tw, plan->th);
+    plan->slab = T_SLAB;
     const char *fd = getenv("EVIS_TILE_FORCE_DIRECT");
     plan->force_direct = fd && fd[0] == '1';
     return true;
 }
 
-cudaError_t tile_setup(const Geom &, const TilePlan &plan)
+cudaError_t tile_setup(const Geom &, TilePlan &plan, int device)
 {
-    return cudaFuncSetAttribute(k_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
+    cudaError_t e = cudaFuncSetAttribute(k_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.smem_bytes);
+    if (e != cudaSuccess) return e;
+    int sms = 0, per_sm = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tile, T_NT, plan.smem_bytes);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    plan.ctas = sms * per_sm;                       // persistent: every CTA is resident
+    return cudaSuccess;
 }
 
 cudaError_t launch_tile(const Geom &g, const TilePlan &plan, const Keyframe &A, const Keyframe &B,
                         const SubstepTable *tab, float *l_ref, float *l_prev, const EventParams &ep,
-                        const EventSink &sink, unsigned long long *holes, unsigned long long *,
+                        const EventSink &sink, unsigned long long *holes, unsigned long long *next_item,
                         const DebugOut &dbg, cudaStream_t st)
 {
     TileArgs a;
     a.g = g;
     a.tw = plan.tw; a.th = plan.th; a.halo = plan.halo; a.tiles_x = plan.tiles_x; a.tiles_y = plan.tiles_y;
     a.force_direct = plan.force_direct;
+    a.num_items = (uint32_t)g.E * (uint32_t)plan.tiles_x * (uint32_t)plan.tiles_y;
+    a.next_item = next_item;
     a.LA = A.L; a.LB = B.L; a.ZA = A.Z; a.ZB = B.Z;
     a.mvA = A.mv; a.fwdA = A.has_fwd ? A.fwd : nullptr; a.mvB = B.mv;
     a.tab = tab; a.l_ref = l_ref; a.l_prev = l_prev; a.ep = ep; a.sink = sink; a.holes = holes; a.dbg = dbg;
-    dim3 grid(plan.tiles_x, plan.tiles_y, g.E);
+    const unsigned grid = a.num_items < (uint32_t)plan.ctas ? a.num_items : (uint32_t)plan.ctas;
     k_tile<<<grid, T_NT, plan.smem_bytes, st>>>(a);
     return cudaGetLastError();
 }
