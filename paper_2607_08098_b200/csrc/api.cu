@@ -26,12 +26,15 @@ struct evis_ctx {
     int cur;                          // kf[cur] receives the next keyframe; kf[cur^1] is A
     float *l_ref, *l_prev;
     SubstepTable *tab;                // device
+    SubstepTable h_tab;               // host copy (kernel parameter of the global path)
     EventParams ep;
 
     // global path z-buffers
     unsigned long long *zmem;
     size_t zmem_bytes;
     int chunk_ne, chunk_ni, nset;
+    int idx_bits;                     // 24: tagged keys (H*W <= 2^24), 32: untagged
+    int ztag;                         // tag of the last chunk; 0 or less: the buffers must be cleared
 
     // event stream
     uint4 *arrival, *ordered;
@@ -181,7 +184,7 @@ int create_impl(evis_ctx *ctx)
     CU(dalloc(ctx, &ctx->l_prev, P));
 
     // substep weights f_i = i/S, g_i = 1 - f_i in IEEE binary32 (same expression as the paper's f = i/K)
-    SubstepTable h;
+    SubstepTable &h = ctx->h_tab;
     memset(&h, 0, sizeof h);
     for (int i = 0; i <= g.S; ++i) {
         volatile float f = (float)i / (float)g.S;
@@ -216,6 +219,9 @@ int create_impl(evis_ctx *ctx)
             ctx->chunk_ni = (int)(ni < 1 ? 1 : (ni > (size_t)g.S ? g.S : ni));
         }
         ctx->zmem_bytes = unit * ctx->chunk_ne * ctx->chunk_ni;
+        const char *nt = getenv("EVIS_NO_ZTAG");                      // test hook: force untagged keys
+        ctx->idx_bits = (g.HW <= (1 << 24) && !(nt && nt[0] == '1')) ? 24 : 32;
+        ctx->ztag = 0;
         CU(cudaMalloc((void **)&ctx->zmem, ctx->zmem_bytes));
         ctx->device_bytes += ctx->zmem_bytes;
         tiles_x = (g.W + G_TILE_W - 1) / G_TILE_W;
@@ -371,11 +377,25 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 const size_t nd = (size_t)ctx->nset * ni * ne * g.HW, nc = (size_t)ctx->nset * ni * ne * g.HWc;
                 zc.zd = ctx->zmem;
                 zc.zc = ctx->zmem + nd;
-                { Span sp(ctx, st, EVIS_STAGE_CLEAR, 1); CU(cudaMemsetAsync(ctx->zmem, 0xFF, (nd + nc) * 8u, st)); }
-                { Span sp(ctx, st, EVIS_STAGE_SPLAT, 1); CU(launch_global_splat(g, zc, A, B, ctx->tab, st)); }
+                zc.idx_bits = ctx->idx_bits;
+                zc.tag = 0;
+                if (ctx->idx_bits == 32) {
+                    Span sp(ctx, st, EVIS_STAGE_CLEAR, 1);
+                    CU(cudaMemsetAsync(ctx->zmem, 0xFF, (nd + nc) * 8u, st));
+                } else {
+                    // tagged keys: every chunk takes a smaller tag than all before it; stale entries lose
+                    // the atomicMin and fail the tag test, so one clear serves 255 chunks
+                    if (ctx->ztag <= 0) {
+                        Span sp(ctx, st, EVIS_STAGE_CLEAR, 1);
+                        CU(cudaMemsetAsync(ctx->zmem, 0xFF, ctx->zmem_bytes, st));
+                        ctx->ztag = 255;
+                    }
+                    zc.tag = (uint32_t)--ctx->ztag;
+                }
+                { Span sp(ctx, st, EVIS_STAGE_SPLAT, 1); CU(launch_global_splat(g, zc, A, B, ctx->h_tab, st)); }
                 {
                     Span sp(ctx, st, EVIS_STAGE_RESOLVE, 1);
-                    CU(launch_global_resolve(g, zc, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink,
+                    CU(launch_global_resolve(g, zc, A, B, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink,
                                              ctx->counters + C_HOLES, ctx->dbg, st));
                 }
             }

@@ -41,13 +41,16 @@ cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, con
 struct ZChunk {
     unsigned long long *zd, *zc;
     int e0, ne, i0, ni;
+    uint32_t tag;          // idx_bits == 24: tag of this chunk (254 .. 0, decreasing); else 0
+    int idx_bits;          // 32: untagged keys, buffers cleared before every chunk; 24: tagged keys
 };
 constexpr int G_TILE_W = 32, G_TILE_H = 8;     // ordering tile of the global path
 
+// tab: HOST copy of the substep table (passed to the kernels as a __grid_constant__ parameter)
 cudaError_t launch_global_splat(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B,
-                                const SubstepTable *tab_dev, cudaStream_t st);
+                                const SubstepTable &tab, cudaStream_t st);
 cudaError_t launch_global_resolve(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B,
-                                  const SubstepTable *tab_dev, float *l_ref, float *l_prev,
+                                  const SubstepTable &tab, float *l_ref, float *l_prev,
                                   const EventParams &ep, const EventSink &sink, unsigned long long *holes,
                                   const DebugOut &dbg, cudaStream_t st);
 

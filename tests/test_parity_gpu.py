@@ -145,6 +145,21 @@ def test_chunked_zbuffer_budget(monkeypatch):
     _assert_tolerances(rep)
 
 
+def test_untagged_keys_and_tag_wraparound(monkeypatch):
+    """Global path key layouts: EVIS_NO_ZTAG=1 forces the untagged 32-bit-index keys (cleared every chunk);
+    with tags, 64 one-substep chunks per step over 5 intervals run through the 255 tags and the re-clear."""
+    spec = scenes.small(scenes.config(4), num_envs=2, height=130, width=173, num_keyframes=3)
+    monkeypatch.setenv("EVIS_NO_ZTAG", "1")
+    rep = parity.run_parity(spec, 3, path=binding.PATH_GLOBAL)
+    _assert_tolerances(rep)
+    monkeypatch.delenv("EVIS_NO_ZTAG")
+    monkeypatch.setenv("EVIS_ZBUF_MB", "1")
+    spec = scenes.small(scenes.config(4), num_envs=4, num_keyframes=6)       # 1.45 MB per env-substep > 1 MB
+    rep = parity.run_parity(spec, 6, path=binding.PATH_GLOBAL)
+    _assert_tolerances(rep)
+    assert rep.steps == 5
+
+
 def _run_stream(spec, n_kf, path, seed_offset=0):
     sc = scenes.make_scene(spec)
     ev = binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg,
