@@ -218,6 +218,15 @@ int create_impl(evis_ctx *ctx)
             size_t ni = budget / unit;
             ctx->chunk_ni = (int)(ni < 1 ? 1 : (ni > (size_t)g.S ? g.S : ni));
         }
+        {   // experiment hooks: explicit chunk shape
+            const size_t ni = env_size_mb("EVIS_CHUNK_NI", 0), ne = env_size_mb("EVIS_CHUNK_NE", 0);
+            if (ni) ctx->chunk_ni = (int)(ni > (size_t)g.S ? g.S : ni);
+            if (ne) ctx->chunk_ne = (int)(ne > (size_t)g.E ? g.E : ne);
+            else if (ni) {
+                size_t n2 = budget / (unit * ctx->chunk_ni);
+                ctx->chunk_ne = (int)(n2 < 1 ? 1 : (n2 > (size_t)g.E ? g.E : n2));
+            }
+        }
         ctx->zmem_bytes = unit * ctx->chunk_ne * ctx->chunk_ni;
         const char *nt = getenv("EVIS_NO_ZTAG");                      // test hook: force untagged keys
         ctx->idx_bits = (g.HW <= (1 << 24) && !(nt && nt[0] == '1')) ? 24 : 32;
