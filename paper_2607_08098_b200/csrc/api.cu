@@ -200,7 +200,9 @@ int create_impl(evis_ctx *ctx)
     ctx->nset = g.mode == 0 ? 1 : 2;
     ctx->path = EVIS_PATH_GLOBAL;
     memset(&ctx->tile, 0, sizeof ctx->tile);
-    if (c.path != EVIS_PATH_GLOBAL && c.max_motion_px > 0.0f && plan_tile(g, c.max_motion_px, &ctx->tile))
+    // AUTO = the global z-buffer path: it is the faster one on every measured workload;
+    // the fused shared-memory tile path runs on request, for bounded motion
+    if (c.path == EVIS_PATH_TILE && c.max_motion_px > 0.0f && plan_tile(g, c.max_motion_px, &ctx->tile))
         ctx->path = EVIS_PATH_TILE;
     if (c.path == EVIS_PATH_TILE && ctx->path != EVIS_PATH_TILE) return EVIS_ERR_INVALID_ARG;
 
@@ -208,7 +210,8 @@ int create_impl(evis_ctx *ctx)
     if (ctx->path == EVIS_PATH_GLOBAL) {
         // chunk = envs x substeps whose z-buffers fit the budget (EVIS_ZBUF_MB, default 512 MiB)
         const size_t unit = (size_t)ctx->nset * 8u * ((size_t)g.HW + g.HWc);
-        const size_t budget = env_size_mb("EVIS_ZBUF_MB", 512) << 20;
+        size_t budget = env_size_mb("EVIS_ZBUF_MB", 512) << 20;
+        if (budget > ((size_t)8 << 30)) budget = (size_t)8 << 30;    // the kernels index a chunk with 32-bit offsets
         if (unit * g.S <= budget) {
             ctx->chunk_ni = g.S;
             size_t ne = budget / (unit * g.S);
@@ -416,8 +419,14 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     }
     {
         Span sp(ctx, st, EVIS_STAGE_ORDER, 3);
-        CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity, ctx->counters + C_EVENTS,
-                        ctx->counters + C_TOTAL, st));
+        if (ctx->path == EVIS_PATH_GLOBAL) {
+            const uint32_t tx = (g.W + G_TILE_W - 1) / G_TILE_W, ty = (g.H + G_TILE_H - 1) / G_TILE_H;
+            CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
+                             ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, ctx->ep, tx, tx * ty, (uint32_t)g.S, st));
+        } else {
+            CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
+                            ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, st));
+        }
     }
     CU(cudaMemcpyAsync(ctx->h_counters, ctx->counters, NCOUNTERS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     ctx->steps += 1;

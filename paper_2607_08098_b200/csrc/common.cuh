@@ -108,8 +108,11 @@ __device__ __forceinline__ float event_time(int k, int pol, float c, float l_ref
 {
     const float lev = __fmaf_rn((float)(pol * k), c, l_ref);
     const float den = __fsub_rn(l_hat, l_prev);
+    // timestamps decide nothing (compared within 1e-7 s; the step is ~1e-3 s): approximate division
+    // (2 ulp) unless the denominator is so small that the fast reciprocal would overflow
     float fr = 1.0f;
-    if (den != 0.0f) fr = __fdiv_rn(__fsub_rn(lev, l_prev), den);
+    if (fabsf(den) > 1e-30f) fr = __fdividef(__fsub_rn(lev, l_prev), den);
+    else if (den != 0.0f) fr = __fdiv_rn(__fsub_rn(lev, l_prev), den);
     fr = fminf(fmaxf(fr, 0.0f), 1.0f);          // NaN -> 0 like the oracle's !(fr >= 0)
     return __fmaf_rn(fr, dt, __fmul_rn((float)(substep - 1), dt));
 }

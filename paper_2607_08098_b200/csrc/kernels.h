@@ -44,7 +44,11 @@ struct ZChunk {
     uint32_t tag;          // idx_bits == 24: tag of this chunk (254 .. 0, decreasing); else 0
     int idx_bits;          // 32: untagged keys, buffers cleared before every chunk; 24: tagged keys
 };
-constexpr int G_TILE_W = 32, G_TILE_H = 8;     // ordering tile of the global path
+constexpr int G_TILE_W = 32, G_TILE_H = 16;    // ordering tile of the global path
+// The global path leaves RECORDS in the arrival buffer, one uint4 per firing pixel-substep:
+//   x, y, z = bits of L_ref (before the update), L_prev, L_hat;  w = raster position in the tile | n << 16
+// and directory entries (record offset, records | events << DIR_EV_SHIFT); order.cu expands them.
+constexpr int DIR_EV_SHIFT = 10;               // a tile has 512 pixels: records <= 512 < 2^10
 
 // tab: HOST copy of the substep table (passed to the kernels as a __grid_constant__ parameter)
 cudaError_t launch_global_splat(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B,
@@ -81,5 +85,11 @@ constexpr int ORDER_ENTRIES_PER_BLOCK = 512;     // directory entries scanned an
 cudaError_t launch_order(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out /*[n]*/,
                          uint4 *ordered, unsigned long long capacity, const unsigned long long *step_events,
                          unsigned long long *total_events, cudaStream_t st);
+// The same for the global path's records: chunks are expanded to events (a7: timestamps) on the way.
+// tiles_x, tiles = tiles per row / per frame of the G_TILE_W x G_TILE_H tiling; S = substeps.
+cudaError_t launch_expand(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out, uint4 *ordered,
+                          unsigned long long capacity, const unsigned long long *step_events,
+                          unsigned long long *total_events, const EventParams &ep, uint32_t tiles_x, uint32_t tiles,
+                          uint32_t S, cudaStream_t st);
 
 }  // namespace evis

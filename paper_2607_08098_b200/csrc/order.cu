@@ -43,15 +43,16 @@ __device__ __forceinline__ unsigned long long block_scan_excl(unsigned long long
     return r;
 }
 
+// shift: 0 = the entry's .y is an event count (tile path), DIR_EV_SHIFT = records | events << shift (global path)
 __global__ void __launch_bounds__(ORD_NT)
-k_dir_blocksum(const uint2 *__restrict__ dir, uint32_t n, unsigned long long *__restrict__ bsum)
+k_dir_blocksum(const uint2 *__restrict__ dir, uint32_t n, unsigned long long *__restrict__ bsum, int shift)
 {
     __shared__ unsigned long long s_w[33];
     const uint32_t base = blockIdx.x * ORD_PER_BLOCK + threadIdx.x * ORD_PER_THREAD;
     unsigned long long v = 0;
 #pragma unroll
     for (int j = 0; j < ORD_PER_THREAD; ++j)
-        if (base + j < n) v += dir[base + j].y;
+        if (base + j < n) v += dir[base + j].y >> shift;
     unsigned long long total;
     block_scan_excl(v, s_w, total);
     if (threadIdx.x == 0) bsum[blockIdx.x] = total;
@@ -128,12 +129,118 @@ k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *
     }
 }
 
+// ---- global path: records -> events ------------------------------------------------------------------
+// A block owns ORD_PER_BLOCK consecutive directory entries = one contiguous range of the ordered stream;
+// the directory holds each chunk's event count, so the block scan of those counts places every chunk.
+// Then the warps take chunks one at a time (shared counter): 32 records per pass -- one coalesced 16-byte
+// load per lane --, warp scan of the crossing counts n, and every lane writes the n events of its record
+// (a7: timestamp of the k-th crossing, R8: linear in log intensity between L_prev and L_hat).
+__global__ void __launch_bounds__(ORD_NT)
+k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__restrict__ bsum,
+         const uint4 *__restrict__ arrival, unsigned long long arrival_cap, uint4 *__restrict__ ordered,
+         unsigned long long cap, const EventParams ep, uint32_t tiles_x, uint32_t tiles, uint32_t S)
+{
+    constexpr unsigned FULL = 0xFFFFFFFFu;
+    __shared__ unsigned long long s_w[33];
+    __shared__ uint32_t s_rel[ORD_PER_BLOCK];         // first output position of chunk e, relative to the block
+    __shared__ uint2 s_dir[ORD_PER_BLOCK];            // its directory entry (arrival offset, records | events << shift)
+    __shared__ uint32_t s_next;
+    const uint32_t blk = blockIdx.x * ORD_PER_BLOCK;
+    const uint32_t base = blk + threadIdx.x * ORD_PER_THREAD;
+    constexpr uint32_t RMASK = (1u << DIR_EV_SHIFT) - 1u;
+    uint32_t cnt[ORD_PER_THREAD];
+    unsigned long long v = 0;
+#pragma unroll
+    for (int j = 0; j < ORD_PER_THREAD; ++j) {
+        uint2 e = make_uint2(0u, 0u);
+        if (base + j < n) e = dir[base + j];
+        cnt[j] = e.y >> DIR_EV_SHIFT;
+        v += cnt[j];
+        s_dir[threadIdx.x * ORD_PER_THREAD + j] = e;
+    }
+    if (threadIdx.x == 0) s_next = 0;
+    unsigned long long total;
+    unsigned long long run = block_scan_excl(v, s_w, total);
+    if (total == 0) return;
+#pragma unroll
+    for (int j = 0; j < ORD_PER_THREAD; ++j) { s_rel[threadIdx.x * ORD_PER_THREAD + j] = (uint32_t)run; run += cnt[j]; }
+    __syncthreads();
+    const unsigned long long out0 = bsum[blockIdx.x];
+    if (out0 >= cap) return;
+    const int lane = threadIdx.x & 31;
+    for (;;) {
+        uint32_t e = 0;
+        if (lane == 0) e = atomicAdd(&s_next, 1u);
+        e = __shfl_sync(FULL, e, 0);
+        if (e >= ORD_PER_BLOCK) break;
+        const uint2 de = s_dir[e];
+        const uint32_t nrec = de.y & RMASK;
+        if (nrec == 0) continue;
+        // chunk d = (env * S + substep - 1) * tiles + tile
+        const uint32_t d = blk + e;
+        const uint32_t es = d / tiles, tile = d - es * tiles;
+        const uint32_t env = es / S, sub = es - env * S + 1u;
+        const uint32_t ty = tile / tiles_x, tx = tile - ty * tiles_x;
+        const uint32_t org = (tx * G_TILE_W) | ((ty * G_TILE_H) << 16);
+        const float t0 = __fmul_rn((float)(sub - 1u), ep.dt);
+        unsigned long long first = out0 + s_rel[e];
+        for (uint32_t r0 = 0; r0 < nrec; r0 += 32) {
+            const uint32_t r = r0 + lane;
+            uint4 rec = make_uint4(0u, 0u, 0u, 0u);
+            const unsigned long long src = (unsigned long long)de.x + r;
+            if (r < nrec && de.x != 0xFFFFFFFFu && src < arrival_cap) rec = __ldcs(arrival + src);
+            const uint32_t nev = rec.w >> 16;
+            uint32_t incl = nev;
+#pragma unroll
+            for (int dd = 1; dd < 32; dd <<= 1) {
+                const uint32_t u = __shfl_up_sync(FULL, incl, dd);
+                if (lane >= dd) incl += u;
+            }
+            unsigned long long o = first + (incl - nev);
+            first += __shfl_sync(FULL, incl, 31);
+            if (nev) {
+                const float l_ref = __uint_as_float(rec.x), l_prev = __uint_as_float(rec.y), l_hat = __uint_as_float(rec.z);
+                const bool up = __fsub_rn(l_hat, l_ref) > 0.0f;
+                const float pc = up ? ep.c_pos : -ep.c_neg;                  // p C
+                const uint32_t pos = rec.w & 0xFFFFu;
+                const uint32_t xy = org + (pos % G_TILE_W) + ((pos / G_TILE_W) << 16);
+                const uint32_t w1 = env | ((up ? 0x01u : 0xFFu) << 16) | (sub << 24);
+                // fr_k = (L_ref + k p C - L_prev) / (L_hat - L_prev), clamped to [0, 1]; 1 when the denominator is 0.
+                // Timestamps decide nothing (compared within 1e-7 s; a substep is ~1e-3 s): reciprocal once per record.
+                const float den = __fsub_rn(l_hat, l_prev);
+                const bool flat = !(fabsf(den) > 1e-30f);
+                const float rden = flat ? 0.0f : __fdividef(1.0f, den);
+                float kf = 0.0f;
+                for (uint32_t k = 0; k < nev; ++k, ++o) {
+                    kf += 1.0f;
+                    float fr = __fmul_rn(__fsub_rn(__fmaf_rn(kf, pc, l_ref), l_prev), rden);
+                    fr = flat ? 1.0f : fminf(fmaxf(fr, 0.0f), 1.0f);
+                    if (o < cap) ordered[o] = make_uint4(xy, w1, __float_as_uint(__fmaf_rn(fr, ep.dt, t0)), ep.kf);
+                }
+            }
+        }
+    }
+}
+
+cudaError_t launch_expand(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
+                          unsigned long long capacity, const unsigned long long *step_events,
+                          unsigned long long *total_events, const EventParams &ep, uint32_t tiles_x, uint32_t tiles,
+                          uint32_t S, cudaStream_t st)
+{
+    const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
+    k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, DIR_EV_SHIFT);
+    k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events);
+    k_expand<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, sink.arrival_cap, ordered, capacity, ep,
+                                    tiles_x, tiles, S);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_order(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
                          unsigned long long capacity, const unsigned long long *step_events,
                          unsigned long long *total_events, cudaStream_t st)
 {
     const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
-    k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum);
+    k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, 0);
     k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events);
     k_dir_copy<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, sink.arrival_cap, ordered, capacity);
     return cudaGetLastError();

@@ -121,7 +121,7 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
 
 
 def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Sequence[int]] = None,
-               mode: int = 0, path: int = binding.PATH_AUTO, use_fwd: bool = True, debug: bool = True,
+               mode: int = 0, path: int = binding.PATH_GLOBAL, use_fwd: bool = True, debug: bool = True,
                capacity: int = 1 << 24, max_motion: Optional[float] = None) -> ParityReport:
     """GPU runs the whole batch; the oracle runs ``envs`` (default: all).  Returns the report after
     asserting every bit-exact criterion; tolerances are asserted by the caller on the report."""

@@ -11,7 +11,18 @@ from tests import parity
 
 pytestmark = pytest.mark.gpu
 
-PATHS = [binding.PATH_GLOBAL, binding.PATH_AUTO]
+PATHS = ["global", "tile"]
+TILE_MAX_MOTION = 23.0       # plan_tile() in tile_path.cu refuses larger motion bounds
+
+
+def _path(name, spec):
+    """EVIS_PATH_AUTO resolves to the global path (the faster one on every BASELINE config); the tile path
+    is requested explicitly and exists only for bounded motion."""
+    if name == "global":
+        return binding.PATH_GLOBAL
+    if spec.max_motion_px() > TILE_MAX_MOTION:
+        pytest.skip("motion bound too large for the tile path")
+    return binding.PATH_TILE
 
 
 def _assert_tolerances(rep):
@@ -28,7 +39,7 @@ def _assert_tolerances(rep):
 def test_config1_full(path):
     """BASELINE config 1 in full: 1 env, 346x260, S=16, C=0.2."""
     spec = scenes.config(1)
-    rep = parity.run_parity(spec, 3, path=path)
+    rep = parity.run_parity(spec, 3, path=_path(path, spec))
     _assert_tolerances(rep)
 
 
@@ -37,7 +48,7 @@ def test_config1_full(path):
 def test_config2_reduced(path, use_fwd):
     """Config 2 recipe (32 overlapping rectangles, occlusion every step) at 3 envs, 211x157 (ragged)."""
     spec = scenes.small(scenes.config(2), num_envs=3, height=157, width=211, num_keyframes=4)
-    rep = parity.run_parity(spec, 4, path=path, use_fwd=use_fwd)
+    rep = parity.run_parity(spec, 4, path=_path(path, spec), use_fwd=use_fwd)
     _assert_tolerances(rep)
     assert rep.holes > 0          # disocclusion actually happens in this workload
 
@@ -46,7 +57,7 @@ def test_config2_reduced(path, use_fwd):
 def test_config3_reduced_disk(path):
     """Config 3 recipe (rotating spoked disk, rotational MV, C+ != C-, S=33) at 2 envs, 320x200."""
     spec = scenes.small(scenes.config(3), num_envs=2, height=200, width=320, num_keyframes=3)
-    rep = parity.run_parity(spec, 3, path=path)
+    rep = parity.run_parity(spec, 3, path=_path(path, spec))
     _assert_tolerances(rep)
 
 
@@ -54,7 +65,7 @@ def test_config3_reduced_disk(path):
 def test_config4_reduced_rl(path):
     """Config 4 recipe (ego-motion + brightness ramp) at 5 envs, full 346x260 resolution."""
     spec = scenes.small(scenes.config(4), num_envs=5, num_keyframes=4)
-    rep = parity.run_parity(spec, 4, path=path)
+    rep = parity.run_parity(spec, 4, path=_path(path, spec))
     _assert_tolerances(rep)
 
 
@@ -74,7 +85,7 @@ def test_noise_stress(path, v_max, S):
     cell, every footprint class, holes everywhere -- the z-test and the tie-break under real conflict."""
     spec = scenes.SceneSpec("noise", 2, 75, 131, 4, 1.0 / 60.0, S, 0.3, 0.2, kind="noise", num_rects=0,
                             v_max=v_max, seed=11)
-    rep = parity.run_parity(spec, 4, path=path)
+    rep = parity.run_parity(spec, 4, path=_path(path, spec))
     _assert_tolerances(rep)
     assert rep.holes > 0
 
@@ -115,12 +126,13 @@ def test_tile_path_reports_motion_bound_violation():
     ev.destroy()
 
 
-def test_static_scene_tile_shortcut():
-    """Zero motion everywhere: the tile path's static shortcut; a pure brightness change lands in
-    substep 1 (R19 note) and matches the oracle."""
+@pytest.mark.parametrize("path", [binding.PATH_TILE, binding.PATH_GLOBAL])
+def test_static_scene_shortcuts(path):
+    """Zero motion everywhere: the tile path's static-tile shortcut and the global splat's static-source
+    loop; a pure brightness change lands in substep 1 (R19 note) and matches the oracle."""
     spec = scenes.SceneSpec("static", 2, 70, 100, 3, 1.0 / 60.0, 8, 0.02, 0.025, num_rects=5, v_max=0.0,
                             ramp_max=30.0, seed=21)
-    rep = parity.run_parity(spec, 3, path=binding.PATH_TILE, max_motion=1.0)
+    rep = parity.run_parity(spec, 3, path=path, max_motion=1.0)
     _assert_tolerances(rep)
 
 
@@ -182,8 +194,8 @@ def test_output_order_is_deterministic_and_tiled(path):
     the tile geometry evis_get_info reports; inside a tile the events of one pixel are contiguous and in
     time order (the pixel order inside a tile is fixed but unspecified)."""
     spec = scenes.small(scenes.config(2), num_envs=3, height=157, width=211, num_keyframes=3)
-    a, info = _run_stream(spec, 3, path)
-    b, _ = _run_stream(spec, 3, path)
+    a, info = _run_stream(spec, 3, _path(path, spec))
+    b, _ = _run_stream(spec, 3, _path(path, spec))
     assert sum(len(x) for x in a) > 1000
     for x, y in zip(a, b):
         assert x.tobytes() == y.tobytes()
