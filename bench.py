@@ -32,6 +32,22 @@ METRIC = "pixel-substeps/s"
 ALGO_BYTES_PER_PIXEL = 52          # per pixel per keyframe interval, DESIGN.md Sec. 6
 ALGO_BYTES_PER_EVENT = 16
 FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+ISSUE_PEAK = 148 * 4 * 32 * 1.965e9   # thread-instructions/s: SMs x schedulers x lanes x clocks.max.sm
+INSTR_PER_PXSS = 165.0                # issued thread-instructions per pixel-substep (ncu, profiles/r01_*.md)
+
+
+def ncu_traffic(workload: str, stage: str):
+    """DRAM bytes (read + write) per launch of the dominant kernel from the committed `ncu --set full`
+    capture (profiles/r01_dram_traffic.csv: workload,stage,bytes_per_launch), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) >= 3 and c[0] == workload and c[1] == stage:
+                    return float(c[2])
+    except OSError:
+        pass
+    return None
 
 
 def parse_args():
@@ -178,7 +194,7 @@ def run_ours(args, spec) -> None:
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2607_08098_b200 import binding, scenes
+    from paper_2607_08098_b200 import binding, scenes, sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -192,7 +208,7 @@ def run_ours(args, spec) -> None:
     binding.load()                                     # fails loudly when libevis.so is missing
 
     # every rank: its own batch of the same shape (envs are independent: no exchange step)
-    spec = scenes.small(spec, seed=spec.seed + 1000 * rank)
+    spec = scenes.small(spec, seed=sharding.rank_seed(spec.seed, rank))
     E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
     K, Wm = args.steps, args.warmup
     sc = scenes.make_scene(spec)
@@ -254,11 +270,8 @@ def run_ours(args, spec) -> None:
     ev.profile_enable(False)
     ev.destroy()
 
-    if world > 1:
-        t = torch.tensor([ms, float(events), float(launches)], device=dev, dtype=torch.float64)
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms, events, launches = float(tmax[0]), float(tsum[1]), int(tsum[2])
+    (ms,), (events, launches) = sharding.reduce_max_sum([ms], [float(events), float(launches)], dev)
+    launches = int(launches)
     pxss_rank = E * H * W * S * K
     value = world * pxss_rank / (ms * 1e-3)
 
@@ -269,13 +282,23 @@ def run_ours(args, spec) -> None:
     ev_per_step = events / world / K
     algo_bytes_step = ALGO_BYTES_PER_PIXEL * E * H * W + ALGO_BYTES_PER_EVENT * ev_per_step
     # the dominant stage is charged the WHOLE step's algorithmic bytes (the other stages are its
-    # helpers: with a fully fused path there is only one kernel); its duration is its own.
+    # helpers: with a fully fused path there is only one kernel); its duration is its own.  Per launch:
+    # bytes and duration are both divided by the stage's launches per step.
+    dom_launches = max(1.0, prof["launches"][dom] / K)
     achieved = algo_bytes_step / (stage_ms[dom] * 1e-3) / 1e9
+    pxss_step = E * H * W * S
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": ncu_traffic(spec.name, dom), "peak_source": peak_src,
                 "algorithmic_bytes_per_step": algo_bytes_step,
+                "algorithmic_bytes_per_launch": algo_bytes_step / dom_launches,
+                "launch_ms": stage_ms[dom] / dom_launches, "launches_per_step": dom_launches,
                 "stage_ms_per_step": stage_ms, "stage_launches_per_step": {k: v / K for k, v in prof["launches"].items()},
-                "whole_step_frac": algo_bytes_step / (ms / K * 1e-3) / 1e9 / peak}
+                "whole_step_frac": algo_bytes_step / (ms / K * 1e-3) / 1e9 / peak,
+                # the binding roof: issued thread-instructions, ~165 per pixel-substep
+                "issue_roof": {"bound": "alu", "unit": "thread-instr/s", "peak": ISSUE_PEAK,
+                               "instr_per_pixel_substep": INSTR_PER_PXSS,
+                               "achieved": INSTR_PER_PXSS * pxss_step / (ms / K * 1e-3),
+                               "frac": INSTR_PER_PXSS * pxss_step / (ms / K * 1e-3) / ISSUE_PEAK}}
 
     out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": K, "warmup": Wm,
            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -308,10 +331,7 @@ def run_ours(args, spec) -> None:
         barrier()
         dt = time.perf_counter() - tt0
         ev.destroy()
-        if world > 1:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t[0])
+        (dt,), _ = sharding.reduce_max_sum([dt], [], dev)
         out["e2e"] = {"value": world * E * H * W * S * Ke / dt, "unit": METRIC, "steps": Ke,
                       "h2d_bytes_per_step": int(E * H * W * 32), "d2h_bytes_per_step": int(16 * got / Ke),
                       "ms_per_step": dt / Ke * 1e3,
