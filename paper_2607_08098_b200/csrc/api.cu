@@ -33,6 +33,8 @@ struct evis_ctx {
     unsigned long long *zmem;
     size_t zmem_bytes;
     int chunk_ne, chunk_ni, nset;
+    alignas(64) unsigned char tmap_d[TMAP_BYTES], tmap_c[TMAP_BYTES];   // CUtensorMap of zd / zc (full-size chunk)
+    bool have_tmap;
     int idx_bits;                     // 24: tagged keys (H*W <= 2^24), 32: untagged
     int ztag;                         // tag of the last chunk; 0 or less: the buffers must be cleared
 
@@ -170,7 +172,9 @@ int create_impl(evis_ctx *ctx)
     const evis_config &c = ctx->cfg;
     Geom &g = ctx->g;
     g.E = c.num_envs; g.H = c.height; g.W = c.width; g.S = c.substeps;
-    g.HW = c.height * c.width; g.Wc = c.width + 1; g.HWc = (c.height + 1) * (c.width + 1);
+    g.HW = c.height * c.width;
+    g.Wd = (c.width + 1) & ~1; g.HWd = c.height * g.Wd;
+    g.Wc = (c.width + 2) & ~1; g.HWc = (c.height + 1) * g.Wc;
     g.mode = c.composite_mode;
     const size_t P = (size_t)g.E * g.HW;
 
@@ -209,7 +213,7 @@ int create_impl(evis_ctx *ctx)
     uint32_t tiles_x, tiles_y;
     if (ctx->path == EVIS_PATH_GLOBAL) {
         // chunk = envs x substeps whose z-buffers fit the budget (EVIS_ZBUF_MB, default 512 MiB)
-        const size_t unit = (size_t)ctx->nset * 8u * ((size_t)g.HW + g.HWc);
+        const size_t unit = (size_t)ctx->nset * 8u * ((size_t)g.HWd + g.HWc);
         size_t budget = env_size_mb("EVIS_ZBUF_MB", 512) << 20;
         if (budget > ((size_t)8 << 30)) budget = (size_t)8 << 30;    // the kernels index a chunk with 32-bit offsets
         if (unit * g.S <= budget) {
@@ -236,6 +240,12 @@ int create_impl(evis_ctx *ctx)
         ctx->ztag = 0;
         CU(cudaMalloc((void **)&ctx->zmem, ctx->zmem_bytes));
         ctx->device_bytes += ctx->zmem_bytes;
+        {
+            const size_t planes = (size_t)ctx->nset * ctx->chunk_ni * ctx->chunk_ne;
+            const char *nt2 = getenv("EVIS_NO_TMA");                  // test hook: direct loads in the resolve kernel
+            ctx->have_tmap = !(nt2 && nt2[0] == '1') &&
+                             make_z_tensor_maps(g, ctx->zmem, ctx->zmem + planes * g.HWd, planes, ctx->tmap_d, ctx->tmap_c);
+        }
         tiles_x = (g.W + G_TILE_W - 1) / G_TILE_W;
         tiles_y = (g.H + G_TILE_H - 1) / G_TILE_H;
     } else {
@@ -386,11 +396,16 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 const int ni = g.S + 1 - i0 < ctx->chunk_ni ? g.S + 1 - i0 : ctx->chunk_ni;
                 ZChunk zc;
                 zc.e0 = e0; zc.ne = ne; zc.i0 = i0; zc.ni = ni;
-                const size_t nd = (size_t)ctx->nset * ni * ne * g.HW, nc = (size_t)ctx->nset * ni * ne * g.HWc;
+                const size_t nd = (size_t)ctx->nset * ni * ne * g.HWd, nc = (size_t)ctx->nset * ni * ne * g.HWc;
                 zc.zd = ctx->zmem;
                 zc.zc = ctx->zmem + nd;
                 zc.idx_bits = ctx->idx_bits;
                 zc.tag = 0;
+                // the tensor maps describe the full-size chunk layout; a smaller chunk (last envs / substeps)
+                // has other plane strides between zd and zc, so it takes the direct-load kernel
+                const bool full = ne == ctx->chunk_ne && ni == ctx->chunk_ni;
+                zc.tmap_d = ctx->have_tmap && full ? ctx->tmap_d : nullptr;
+                zc.tmap_c = ctx->have_tmap && full ? ctx->tmap_c : nullptr;
                 if (ctx->idx_bits == 32) {
                     Span sp(ctx, st, EVIS_STAGE_CLEAR, 1);
                     CU(cudaMemsetAsync(ctx->zmem, 0xFF, (nd + nc) * 8u, st));

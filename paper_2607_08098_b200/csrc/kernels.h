@@ -17,7 +17,9 @@ struct Keyframe {
 struct Geom {
     int E, H, W, S;
     int HW;        // H*W
-    int Wc, HWc;   // class-11 cell grid: (W+1) x (H+1) cells, cell (x0+1, y0+1)
+    int Wd, HWd;   // z-buffer plane of direct targets: H rows of pitch Wd = W rounded up to even
+    int Wc, HWc;   // class-11 cell grid: (W+1) x (H+1) cells, cell (x0+1, y0+1); row pitch Wc = W+1 rounded up to
+                   // even (TMA needs 16-byte row pitches), HWc = (H+1) * Wc
     int mode;      // EVIS_COMPOSITE_*
 };
 
@@ -35,7 +37,7 @@ cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, con
 
 // ---- global z-buffer path (global_path.cu): any motion -----------------------------------------
 // z-buffers of one chunk = envs [e0, e0+ne) x substeps [i0, i0+ni):
-//   zd [nset][ni][ne][HW]   direct targets (footprints that are a single pixel or a 2-pixel edge)
+//   zd [nset][ni][ne][HWd]  direct targets (footprints that are a single pixel or a 2-pixel edge)
 //   zc [nset][ni][ne][HWc]  class-11 cells: the source covers the 2x2 block whose top-left is the cell
 // nset = 1 in composite mode 0 (direction folded into the key's top bit), 2 in mode 1.
 struct ZChunk {
@@ -43,7 +45,14 @@ struct ZChunk {
     int e0, ne, i0, ni;
     uint32_t tag;          // idx_bits == 24: tag of this chunk (254 .. 0, decreasing); else 0
     int idx_bits;          // 32: untagged keys, buffers cleared before every chunk; 24: tagged keys
+    const void *tmap_d, *tmap_c;   // HOST pointers to the CUtensorMap of zd / zc (3-D: x, y, plane), or null:
+                                   // the resolve kernel then loads the keys directly instead of staging them by TMA
 };
+constexpr int TMAP_BYTES = 128;    // sizeof(CUtensorMap)
+// Encode the tensor maps of a context's z-buffers ([planes][H][Wd] and [planes][H+1][Wc] of 64-bit keys, boxes
+// of one resolve tile).  Returns false when the driver entry point is unavailable.
+bool make_z_tensor_maps(const Geom &g, unsigned long long *zd, unsigned long long *zc, size_t planes, void *tmap_d,
+                        void *tmap_c);
 constexpr int G_TILE_W = 32, G_TILE_H = 16;    // ordering tile of the global path
 // The global path leaves RECORDS in the arrival buffer, one uint4 per firing pixel-substep:
 //   x, y, z = bits of L_ref (before the update), L_prev, L_hat;  w = raster position in the tile | n << 16
