@@ -154,7 +154,8 @@ size_t env_size_mb(const char *name, size_t dflt)
 void free_all(evis_ctx *ctx)
 {
     for (int k = 0; k < 2; ++k) {
-        cudaFree(ctx->kf[k].L); cudaFree(ctx->kf[k].mv); cudaFree(ctx->kf[k].fwd); cudaFree(ctx->kf[k].Z);
+        if (k == 0) cudaFree(ctx->kf[k].L);
+        cudaFree(ctx->kf[k].mv); cudaFree(ctx->kf[k].fwd); cudaFree(ctx->kf[k].Z);
     }
     cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->tab); cudaFree(ctx->zmem);
     cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
@@ -173,14 +174,16 @@ int create_impl(evis_ctx *ctx)
     Geom &g = ctx->g;
     g.E = c.num_envs; g.H = c.height; g.W = c.width; g.S = c.substeps;
     g.HW = c.height * c.width;
-    g.Wd = (c.width + 1) & ~1; g.HWd = c.height * g.Wd;
-    g.Wc = (c.width + 2) & ~1; g.HWc = (c.height + 1) * g.Wc;
+    g.Wp = (c.width + 2) & ~1; g.HWp = (c.height + 1) * g.Wp;
     g.mode = c.composite_mode;
     const size_t P = (size_t)g.E * g.HW;
+    if (P >= ((size_t)1 << 31)) return EVIS_ERR_INVALID_ARG;    // the kernels keep pixel offsets between planes in 32 bits
 
     CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+    // the two L planes share one allocation: the resolve kernel addresses the winner's value from one base
+    CU(dalloc(ctx, &ctx->kf[0].L, 2 * P));
+    ctx->kf[1].L = ctx->kf[0].L + P;
     for (int k = 0; k < 2; ++k) {
-        CU(dalloc(ctx, &ctx->kf[k].L, P));
         CU(dalloc(ctx, &ctx->kf[k].mv, P));
         CU(dalloc(ctx, &ctx->kf[k].Z, P));
     }
@@ -213,7 +216,7 @@ int create_impl(evis_ctx *ctx)
     uint32_t tiles_x, tiles_y;
     if (ctx->path == EVIS_PATH_GLOBAL) {
         // chunk = envs x substeps whose z-buffers fit the budget (EVIS_ZBUF_MB, default 512 MiB)
-        const size_t unit = (size_t)ctx->nset * 8u * ((size_t)g.HWd + g.HWc);
+        const size_t unit = (size_t)ctx->nset * 8u * 2u * (size_t)g.HWp;
         size_t budget = env_size_mb("EVIS_ZBUF_MB", 512) << 20;
         if (budget > ((size_t)8 << 30)) budget = (size_t)8 << 30;    // the kernels index a chunk with 32-bit offsets
         if (unit * g.S <= budget) {
@@ -244,7 +247,7 @@ int create_impl(evis_ctx *ctx)
             const size_t planes = (size_t)ctx->nset * ctx->chunk_ni * ctx->chunk_ne;
             const char *nt2 = getenv("EVIS_NO_TMA");                  // test hook: direct loads in the resolve kernel
             ctx->have_tmap = !(nt2 && nt2[0] == '1') &&
-                             make_z_tensor_maps(g, ctx->zmem, ctx->zmem + planes * g.HWd, planes, ctx->tmap_d, ctx->tmap_c);
+                             make_z_tensor_maps(g, ctx->zmem, ctx->zmem + planes * g.HWp, planes, ctx->tmap_d, ctx->tmap_c);
         }
         tiles_x = (g.W + G_TILE_W - 1) / G_TILE_W;
         tiles_y = (g.H + G_TILE_H - 1) / G_TILE_H;
@@ -396,19 +399,17 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 const int ni = g.S + 1 - i0 < ctx->chunk_ni ? g.S + 1 - i0 : ctx->chunk_ni;
                 ZChunk zc;
                 zc.e0 = e0; zc.ne = ne; zc.i0 = i0; zc.ni = ni;
-                const size_t nd = (size_t)ctx->nset * ni * ne * g.HWd, nc = (size_t)ctx->nset * ni * ne * g.HWc;
+                // every chunk uses the plane strides of the full chunk shape, so one pair of tensor maps serves all
+                zc.ne_alloc = ctx->chunk_ne; zc.ni_alloc = ctx->chunk_ni;
                 zc.zd = ctx->zmem;
-                zc.zc = ctx->zmem + nd;
+                zc.zc = ctx->zmem + (size_t)ctx->nset * ctx->chunk_ni * ctx->chunk_ne * g.HWp;
                 zc.idx_bits = ctx->idx_bits;
                 zc.tag = 0;
-                // the tensor maps describe the full-size chunk layout; a smaller chunk (last envs / substeps)
-                // has other plane strides between zd and zc, so it takes the direct-load kernel
-                const bool full = ne == ctx->chunk_ne && ni == ctx->chunk_ni;
-                zc.tmap_d = ctx->have_tmap && full ? ctx->tmap_d : nullptr;
-                zc.tmap_c = ctx->have_tmap && full ? ctx->tmap_c : nullptr;
+                zc.tmap_d = ctx->have_tmap ? ctx->tmap_d : nullptr;
+                zc.tmap_c = ctx->have_tmap ? ctx->tmap_c : nullptr;
                 if (ctx->idx_bits == 32) {
                     Span sp(ctx, st, EVIS_STAGE_CLEAR, 1);
-                    CU(cudaMemsetAsync(ctx->zmem, 0xFF, (nd + nc) * 8u, st));
+                    CU(cudaMemsetAsync(ctx->zmem, 0xFF, ctx->zmem_bytes, st));
                 } else {
                     // tagged keys: every chunk takes a smaller tag than all before it; stale entries lose
                     // the atomicMin and fail the tag test, so one clear serves 255 chunks

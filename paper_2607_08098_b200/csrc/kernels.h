@@ -17,9 +17,11 @@ struct Keyframe {
 struct Geom {
     int E, H, W, S;
     int HW;        // H*W
-    int Wd, HWd;   // z-buffer plane of direct targets: H rows of pitch Wd = W rounded up to even
-    int Wc, HWc;   // class-11 cell grid: (W+1) x (H+1) cells, cell (x0+1, y0+1); row pitch Wc = W+1 rounded up to
-                   // even (TMA needs 16-byte row pitches), HWc = (H+1) * Wc
+    int Wp, HWp;   // z-buffer plane: (H+1) rows of pitch Wp = W+1 rounded up to even (TMA needs 16-byte row
+                   // pitches), HWp = (H+1) * Wp.  Both kinds of plane use it with the same addressing: a source
+                   // whose q has floor (x0, y0), x0 >= -1, y0 >= -1, files itself at (y0+1) * Wp + (x0+1) -- in
+                   // the pixel plane zd that is target pixel (x0, y0) (row 0 / column 0 are a guard band for
+                   // coordinate -1, never read), in the cell plane zc it is the class-11 cell (x0+1, y0+1)
     int mode;      // EVIS_COMPOSITE_*
 };
 
@@ -37,19 +39,21 @@ cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, con
 
 // ---- global z-buffer path (global_path.cu): any motion -----------------------------------------
 // z-buffers of one chunk = envs [e0, e0+ne) x substeps [i0, i0+ni):
-//   zd [nset][ni][ne][HWd]  direct targets (footprints that are a single pixel or a 2-pixel edge)
-//   zc [nset][ni][ne][HWc]  class-11 cells: the source covers the 2x2 block whose top-left is the cell
-// nset = 1 in composite mode 0 (direction folded into the key's top bit), 2 in mode 1.
+//   zd [nset][ni_alloc][ne_alloc][HWp]  direct targets (footprints that are a single pixel or a 2-pixel edge)
+//   zc [nset][ni_alloc][ne_alloc][HWp]  class-11 cells: the source covers the 2x2 block whose top-left is the cell
+// nset = 1 in composite mode 0 (direction folded into the key's top bit), 2 in mode 1.  ni_alloc x ne_alloc is
+// the context's full chunk shape: a smaller last chunk keeps the same plane strides (and tensor maps).
 struct ZChunk {
     unsigned long long *zd, *zc;
     int e0, ne, i0, ni;
+    int ne_alloc, ni_alloc; // plane strides of the allocation (>= ne, ni)
     uint32_t tag;          // idx_bits == 24: tag of this chunk (254 .. 0, decreasing); else 0
     int idx_bits;          // 32: untagged keys, buffers cleared before every chunk; 24: tagged keys
     const void *tmap_d, *tmap_c;   // HOST pointers to the CUtensorMap of zd / zc (3-D: x, y, plane), or null:
                                    // the resolve kernel then loads the keys directly instead of staging them by TMA
 };
 constexpr int TMAP_BYTES = 128;    // sizeof(CUtensorMap)
-// Encode the tensor maps of a context's z-buffers ([planes][H][Wd] and [planes][H+1][Wc] of 64-bit keys, boxes
+// Encode the tensor maps of a context's z-buffers ([planes][H+1][Wp] of 64-bit keys each, boxes
 // of one resolve tile).  Returns false when the driver entry point is unavailable.
 bool make_z_tensor_maps(const Geom &g, unsigned long long *zd, unsigned long long *zc, size_t planes, void *tmap_d,
                         void *tmap_c);
