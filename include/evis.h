@@ -92,6 +92,9 @@ enum { EVIS_STAGE_PREP = 0,     /* a1 + a9: log-luminance, keyframe take-over   
        EVIS_STAGE_RESOLVE = 3,  /* global path: a5-a8 (resolve, event model, compaction)          */
        EVIS_STAGE_ORDER = 4,    /* a8: deterministic ordering                                     */
        EVIS_STAGE_TILE = 5,     /* tile path: a2-a8 fused                                         */
+       EVIS_STAGE_WARP = 6,     /* global path with concurrent z-buffer regions: a2-a8 of all chunks, from the
+                                   fork of the internal streams to their join (kernels overlap, so splat and
+                                   resolve are not timed apart)                                   */
        EVIS_NUM_STAGES = 8 };
 typedef struct {
     uint64_t steps;                       /* evis_step calls accumulated since enable / last read */

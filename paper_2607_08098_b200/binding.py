@@ -43,7 +43,7 @@ class evis_info(C.Structure):
 
 
 NUM_STAGES = 8
-STAGE_NAMES = ["prep", "clear", "splat", "resolve", "order", "tile", "s6", "s7"]
+STAGE_NAMES = ["prep", "clear", "splat", "resolve", "order", "tile", "splat+resolve", "s7"]
 
 
 class evis_profile(C.Structure):

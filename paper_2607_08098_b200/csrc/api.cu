@@ -30,13 +30,19 @@ struct evis_ctx {
     EventParams ep;
 
     // global path z-buffers
-    unsigned long long *zmem;
-    size_t zmem_bytes;
+    // nreg regions of zmem_bytes each; region r serves the env chunks c with c % nreg == r, on its own
+    // stream when nreg > 1, so that several chunks small enough for the L2 are in flight together
+    static constexpr int MAX_REG = 8;
+    unsigned long long *zmem;         // one allocation: nreg * zmem_bytes
+    size_t zmem_bytes;                // one region (a multiple of 256 bytes)
+    int nreg;
     int chunk_ne, chunk_ni, nset;
-    alignas(64) unsigned char tmap_d[TMAP_BYTES], tmap_c[TMAP_BYTES];   // CUtensorMap of zd / zc (full-size chunk)
+    alignas(64) unsigned char tmap_d[MAX_REG][TMAP_BYTES], tmap_c[MAX_REG][TMAP_BYTES];   // CUtensorMap of zd / zc per region
     bool have_tmap;
     int idx_bits;                     // 24: tagged keys (H*W <= 2^24), 32: untagged
-    int ztag;                         // tag of the last chunk; 0 or less: the buffers must be cleared
+    int ztag[MAX_REG];                // tag of the region's last chunk; 0 or less: the region must be cleared
+    cudaStream_t reg_stream[MAX_REG];
+    cudaEvent_t ev_fork, ev_join[MAX_REG];
 
     // event stream
     uint4 *arrival, *ordered;
@@ -125,10 +131,10 @@ void prof_drain(evis_ctx *ctx)
 // RAII span: records an event pair around the launches of one stage when profiling is on
 struct Span {
     evis_ctx *ctx; cudaStream_t st; int stage; cudaEvent_t a;
-    Span(evis_ctx *c, cudaStream_t s, int stg, int launches) : ctx(c), st(s), stage(stg), a(nullptr)
+    Span(evis_ctx *c, cudaStream_t s, int stg, int launches, bool timed = true) : ctx(c), st(s), stage(stg), a(nullptr)
     {
         ctx->launches += launches;
-        if (!ctx->prof_on) return;
+        if (!ctx->prof_on || !timed) return;
         ctx->prof_acc.launches[stage] += launches;
         a = prof_event(ctx);
         if (a) cudaEventRecord(a, st);
@@ -166,6 +172,11 @@ void free_all(evis_ctx *ctx)
     for (cudaEvent_t e : ctx->prof_free) cudaEventDestroy(e);
     ctx->prof_free.clear();
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    for (int r = 0; r < evis_ctx::MAX_REG; ++r) {
+        if (ctx->reg_stream[r]) cudaStreamDestroy(ctx->reg_stream[r]);
+        if (ctx->ev_join[r]) cudaEventDestroy(ctx->ev_join[r]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
 }
 
 int create_impl(evis_ctx *ctx)
@@ -215,9 +226,13 @@ int create_impl(evis_ctx *ctx)
 
     uint32_t tiles_x, tiles_y;
     if (ctx->path == EVIS_PATH_GLOBAL) {
-        // chunk = envs x substeps whose z-buffers fit the budget (EVIS_ZBUF_MB, default 512 MiB)
+        // chunk = envs x substeps whose z-buffers fit one region's budget.  Defaults (measured on B200, DESIGN.md
+        // Sec. 6): 4 regions on 4 streams; 24 MiB regions when one env's S substeps fit (the live keys stay in the
+        // L2 and small grids overlap across streams), else 128 MiB (substep chunks re-read the sources and carry
+        // L_ref / L_prev through memory, so they should be long).  EVIS_ZBUF_MB / EVIS_STREAMS override.
         const size_t unit = (size_t)ctx->nset * 8u * 2u * (size_t)g.HWp;
-        size_t budget = env_size_mb("EVIS_ZBUF_MB", 512) << 20;
+        const size_t default_regions = 4;
+        size_t budget = env_size_mb("EVIS_ZBUF_MB", unit * g.S <= ((size_t)24 << 20) ? 24 : 128) << 20;
         if (budget > ((size_t)8 << 30)) budget = (size_t)8 << 30;    // the kernels index a chunk with 32-bit offsets
         if (unit * g.S <= budget) {
             ctx->chunk_ni = g.S;
@@ -237,17 +252,35 @@ int create_impl(evis_ctx *ctx)
                 ctx->chunk_ne = (int)(n2 < 1 ? 1 : (n2 > (size_t)g.E ? g.E : n2));
             }
         }
-        ctx->zmem_bytes = unit * ctx->chunk_ne * ctx->chunk_ni;
+        ctx->zmem_bytes = (unit * ctx->chunk_ne * ctx->chunk_ni + 255) & ~(size_t)255;
+        {   // concurrent regions (EVIS_STREAMS): never more than there are env chunks
+            const size_t nchunks = ((size_t)g.E + ctx->chunk_ne - 1) / ctx->chunk_ne;
+            size_t nr = env_size_mb("EVIS_STREAMS", default_regions);
+            if (nr > (size_t)evis_ctx::MAX_REG) nr = evis_ctx::MAX_REG;
+            if (nr > nchunks) nr = nchunks;
+            ctx->nreg = (int)(nr < 1 ? 1 : nr);
+        }
         const char *nt = getenv("EVIS_NO_ZTAG");                      // test hook: force untagged keys
         ctx->idx_bits = (g.HW <= (1 << 24) && !(nt && nt[0] == '1')) ? 24 : 32;
-        ctx->ztag = 0;
-        CU(cudaMalloc((void **)&ctx->zmem, ctx->zmem_bytes));
-        ctx->device_bytes += ctx->zmem_bytes;
+        CU(cudaMalloc((void **)&ctx->zmem, ctx->zmem_bytes * ctx->nreg));
+        ctx->device_bytes += ctx->zmem_bytes * ctx->nreg;
         {
             const size_t planes = (size_t)ctx->nset * ctx->chunk_ni * ctx->chunk_ne;
             const char *nt2 = getenv("EVIS_NO_TMA");                  // test hook: direct loads in the resolve kernel
-            ctx->have_tmap = !(nt2 && nt2[0] == '1') &&
-                             make_z_tensor_maps(g, ctx->zmem, ctx->zmem + planes * g.HWp, planes, ctx->tmap_d, ctx->tmap_c);
+            ctx->have_tmap = !(nt2 && nt2[0] == '1');
+            for (int r = 0; r < ctx->nreg; ++r) {
+                unsigned long long *zr = ctx->zmem + (size_t)r * (ctx->zmem_bytes / 8);
+                ctx->ztag[r] = 0;
+                if (ctx->have_tmap && !make_z_tensor_maps(g, zr, zr + planes * g.HWp, planes, ctx->tmap_d[r], ctx->tmap_c[r]))
+                    ctx->have_tmap = false;
+            }
+        }
+        if (ctx->nreg > 1) {
+            CU(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+            for (int r = 0; r < ctx->nreg; ++r) {
+                CU(cudaStreamCreateWithFlags(&ctx->reg_stream[r], cudaStreamNonBlocking));
+                CU(cudaEventCreateWithFlags(&ctx->ev_join[r], cudaEventDisableTiming));
+            }
         }
         tiles_x = (g.W + G_TILE_W - 1) / G_TILE_W;
         tiles_y = (g.H + G_TILE_H - 1) / G_TILE_H;
@@ -393,41 +426,59 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     }
 
     if (ctx->path == EVIS_PATH_GLOBAL) {
-        for (int e0 = 0; e0 < g.E; e0 += ctx->chunk_ne) {
+        // nreg > 1: the env chunks are dealt round-robin to the regions' streams, which fork from `st` here and
+        // join it after the loop; the substep chunks of one env chunk stay on one stream (L_ref / L_prev carry)
+        const bool multi = ctx->nreg > 1;
+        const int nchunks_e = (g.E + ctx->chunk_ne - 1) / ctx->chunk_ne, nchunks_i = (g.S + ctx->chunk_ni - 1) / ctx->chunk_ni;
+        Span sp_all(ctx, st, EVIS_STAGE_WARP, multi ? 2 * nchunks_e * nchunks_i : 0, multi);
+        if (multi) {
+            CU(cudaEventRecord(ctx->ev_fork, st));
+            for (int r = 0; r < ctx->nreg; ++r) CU(cudaStreamWaitEvent(ctx->reg_stream[r], ctx->ev_fork, 0));
+        }
+        const size_t planes = (size_t)ctx->nset * ctx->chunk_ni * ctx->chunk_ne;
+        for (int e0 = 0, ce = 0; e0 < g.E; e0 += ctx->chunk_ne, ++ce) {
             const int ne = g.E - e0 < ctx->chunk_ne ? g.E - e0 : ctx->chunk_ne;
+            const int r = ce % ctx->nreg;
+            cudaStream_t cs = multi ? ctx->reg_stream[r] : st;
+            unsigned long long *zr = ctx->zmem + (size_t)r * (ctx->zmem_bytes / 8);
             for (int i0 = 1; i0 <= g.S; i0 += ctx->chunk_ni) {
                 const int ni = g.S + 1 - i0 < ctx->chunk_ni ? g.S + 1 - i0 : ctx->chunk_ni;
                 ZChunk zc;
                 zc.e0 = e0; zc.ne = ne; zc.i0 = i0; zc.ni = ni;
                 // every chunk uses the plane strides of the full chunk shape, so one pair of tensor maps serves all
                 zc.ne_alloc = ctx->chunk_ne; zc.ni_alloc = ctx->chunk_ni;
-                zc.zd = ctx->zmem;
-                zc.zc = ctx->zmem + (size_t)ctx->nset * ctx->chunk_ni * ctx->chunk_ne * g.HWp;
+                zc.zd = zr;
+                zc.zc = zr + planes * g.HWp;
                 zc.idx_bits = ctx->idx_bits;
                 zc.tag = 0;
-                zc.tmap_d = ctx->have_tmap ? ctx->tmap_d : nullptr;
-                zc.tmap_c = ctx->have_tmap ? ctx->tmap_c : nullptr;
+                zc.tmap_d = ctx->have_tmap ? ctx->tmap_d[r] : nullptr;
+                zc.tmap_c = ctx->have_tmap ? ctx->tmap_c[r] : nullptr;
                 if (ctx->idx_bits == 32) {
-                    Span sp(ctx, st, EVIS_STAGE_CLEAR, 1);
-                    CU(cudaMemsetAsync(ctx->zmem, 0xFF, ctx->zmem_bytes, st));
+                    Span sp(ctx, cs, EVIS_STAGE_CLEAR, 1, !multi);
+                    CU(cudaMemsetAsync(zr, 0xFF, ctx->zmem_bytes, cs));
                 } else {
-                    // tagged keys: every chunk takes a smaller tag than all before it; stale entries lose
-                    // the atomicMin and fail the tag test, so one clear serves 255 chunks
-                    if (ctx->ztag <= 0) {
-                        Span sp(ctx, st, EVIS_STAGE_CLEAR, 1);
-                        CU(cudaMemsetAsync(ctx->zmem, 0xFF, ctx->zmem_bytes, st));
-                        ctx->ztag = 255;
+                    // tagged keys: every chunk takes a smaller tag than all before it in its region; stale
+                    // entries lose the atomicMin and fail the tag test, so one clear serves 255 chunks
+                    if (ctx->ztag[r] <= 0) {
+                        Span sp(ctx, cs, EVIS_STAGE_CLEAR, 1, !multi);
+                        CU(cudaMemsetAsync(zr, 0xFF, ctx->zmem_bytes, cs));
+                        ctx->ztag[r] = 255;
                     }
-                    zc.tag = (uint32_t)--ctx->ztag;
+                    zc.tag = (uint32_t)--ctx->ztag[r];
                 }
-                { Span sp(ctx, st, EVIS_STAGE_SPLAT, 1); CU(launch_global_splat(g, zc, A, B, ctx->h_tab, st)); }
+                { Span sp(ctx, cs, EVIS_STAGE_SPLAT, multi ? 0 : 1, !multi); CU(launch_global_splat(g, zc, A, B, ctx->h_tab, cs)); }
                 {
-                    Span sp(ctx, st, EVIS_STAGE_RESOLVE, 1);
+                    Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 1, !multi);
                     CU(launch_global_resolve(g, zc, A, B, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink,
-                                             ctx->counters + C_HOLES, ctx->dbg, st));
+                                             ctx->counters + C_HOLES, ctx->dbg, cs));
                 }
             }
         }
+        if (multi)
+            for (int r = 0; r < ctx->nreg; ++r) {
+                CU(cudaEventRecord(ctx->ev_join[r], ctx->reg_stream[r]));
+                CU(cudaStreamWaitEvent(st, ctx->ev_join[r], 0));
+            }
     } else {
         Span sp(ctx, st, EVIS_STAGE_TILE, 1);
         CU(launch_tile(g, ctx->tile, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink, ctx->counters + C_HOLES,

@@ -166,10 +166,25 @@ def test_untagged_keys_and_tag_wraparound(monkeypatch):
     _assert_tolerances(rep)
     monkeypatch.delenv("EVIS_NO_ZTAG")
     monkeypatch.setenv("EVIS_ZBUF_MB", "1")
+    monkeypatch.setenv("EVIS_STREAMS", "1")                                  # one region sees all 320 chunks
     spec = scenes.small(scenes.config(4), num_envs=4, num_keyframes=6)       # 1.45 MB per env-substep > 1 MB
     rep = parity.run_parity(spec, 6, path=binding.PATH_GLOBAL)
     _assert_tolerances(rep)
     assert rep.steps == 5
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("streams,no_tma", [("1", "0"), ("3", "0"), ("8", "0"), ("4", "1")])
+def test_concurrent_regions_and_direct_loads(monkeypatch, streams, no_tma):
+    """Global path plumbing: the env chunks are dealt to EVIS_STREAMS z-buffer regions on their own streams
+    (default 4); EVIS_NO_TMA=1 makes the resolve kernel load the keys directly instead of through the TMA ring.
+    Every variant must match the oracle, with several env chunks per region and a ragged last chunk."""
+    monkeypatch.setenv("EVIS_STREAMS", streams)
+    monkeypatch.setenv("EVIS_NO_TMA", no_tma)
+    monkeypatch.setenv("EVIS_ZBUF_MB", "2")                                  # 2.8 MB per env: 1 env x 11 substeps per chunk
+    spec = scenes.small(scenes.config(4), num_envs=11, height=90, width=120, num_keyframes=4)
+    rep = parity.run_parity(spec, 4, path=binding.PATH_GLOBAL)
+    _assert_tolerances(rep)
 
 
 def _run_stream(spec, n_kf, path, seed_offset=0):
