@@ -21,7 +21,7 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 zero motion identity, P2 substep S reproduces
  * keyframe B, P3 integer translation, P4 8x8 gather-form brute force, P5 analytic two-rectangle
- * occlusion, P6-P10 event-count / residual / timestamp closed forms.  UNPINNED by paper or
+ * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8).  UNPINNED by paper or
  * mathematics (fixed by DESIGN.md readings only): log base R1, epsilon R2, initial reference
  * level R6, nearest-pixel depth lookup R16, hole handling R20, the composite choice R19.
  */
@@ -154,10 +154,15 @@ void evo_composite(int H, int W, int i, int S, int mode,
  * stamped by linear interpolation in log intensity between the previous and the current frame
  * value [R8]: level_k = Lref + p k C, fr = (level_k - Lprev) / (L - Lprev) clamped to [0,1].
  * Frame i covers ((i-1) T/S, i T/S].  Events are appended in (y, x, k) order.
+ * Threshold mismatch (Eq. 8): "the scalar threshold C is replaced by per-pixel ON/OFF
+ * thresholds ... sampled once per pixel".  The maps are INPUTS (the caller draws them); th_on[q] replaces C+
+ * and th_off[q] replaces C- at pixel q, everything else is unchanged [R25].
  * Returns the number of events this frame produced (all are counted; only those that fit are
  * stored).                                                                                        */
 int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
-                        float c_pos, float c_neg, const float *Lhat,
+                        float c_pos, float c_neg,
+                        const float *th_on, const float *th_off,   /* [H*W] or NULL (both): Eq. 8 maps */
+                        const float *Lhat,
                         float *Lref, float *Lprev,
                         evo_event *ev, int64_t cap, int64_t n_have,
                         float *dbg_dL /* [H*W] or NULL: dL = L - Lref before the update */)
@@ -171,8 +176,8 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
             const float d = L - Lref[q];
             if (dbg_dL) dbg_dL[q] = d;
             float C; int p;
-            if (d > 0.0f)      { C = c_pos; p = +1; }
-            else if (d < 0.0f) { C = c_neg; p = -1; }
+            if (d > 0.0f)      { C = th_on ? th_on[q] : c_pos; p = +1; }     /* theta_ON(u),  Eq. 8 */
+            else if (d < 0.0f) { C = th_off ? th_off[q] : c_neg; p = -1; }   /* theta_OFF(u), Eq. 8 */
             else               { C = 1.0f;  p = 0; }
             int n = 0;
             if (p != 0) {
@@ -205,6 +210,7 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
  * fwdA: displacement of A's pixels towards B: -m_A or the explicit forward field.
  * Optional debug outputs, each [S][H*W] or NULL: winners of each direction, composite, Lhat.     */
 int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, float c_pos, float c_neg,
+                     const float *th_on, const float *th_off,              /* [H*W] or NULL: Eq. 8 maps of this env */
                      const float *LA, const float *fwdA, const float *ZA,
                      const float *LB, const float *mB, const float *ZB,
                      float *Lref, float *Lprev,
@@ -228,7 +234,7 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, fl
             if (dbg_Lhat) dbg_Lhat[(int64_t)(i - 1) * P + q] = Lhat[q];
             if (holes && zA[q] == EVO_EMPTY && zB[q] == EVO_EMPTY) ++*holes;
         }
-        made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, Lhat, Lref, Lprev,
+        made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, th_on, th_off, Lhat, Lref, Lprev,
                                 ev, cap, n_have + made, dbg_dL ? dbg_dL + (int64_t)(i - 1) * P : 0);
     }
     return made;

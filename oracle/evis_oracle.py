@@ -33,10 +33,10 @@ def lib():
         L.evo_splat.restype = None
         L.evo_composite.argtypes = [C.c_int] * 5 + [u64p, u64p, fp, fp, fp, fp, u8p, u32p]
         L.evo_composite.restype = None
-        L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp, fp, C.c_void_p,
+        L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [fp, fp, fp, C.c_void_p,
                                                                         C.c_int64, C.c_int64, fp]
         L.evo_event_frame.restype = C.c_int64
-        L.evo_interval.argtypes = ([C.c_int] * 6 + [C.c_float] * 3 + [fp] * 8 + [u64p, u64p, fp]
+        L.evo_interval.argtypes = ([C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [fp] * 8 + [u64p, u64p, fp]
                                    + [C.c_void_p, C.c_int64, C.c_int64]
                                    + [u32p, u32p, u8p, u32p, fp, fp, C.POINTER(C.c_int64)])
         L.evo_interval.restype = C.c_int64
@@ -73,14 +73,19 @@ def splat(i: int, S: int, src_is_B: bool, disp: np.ndarray, Zsrc: np.ndarray, Zo
 
 
 def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float, T: float,
-                 Lref0: Optional[np.ndarray] = None):
+                 Lref0: Optional[np.ndarray] = None, theta_on: Optional[np.ndarray] = None,
+                 theta_off: Optional[np.ndarray] = None):
     """Event stage alone (Eq. 4): feed a sequence of S log frames [S,H,W] to one env.
+    theta_on / theta_off [H,W]: per-pixel thresholds replacing c_pos / c_neg (Eq. 8).
 
     Returns (events, Lref_final).  Lref and Lprev start at L0 (or Lref0 for the reference)."""
     frames = np.ascontiguousarray(frames, np.float32)
     S, H, W = frames.shape
     Lprev = np.ascontiguousarray(L0, np.float32).copy()
     Lref = Lprev.copy() if Lref0 is None else np.ascontiguousarray(Lref0, np.float32).copy()
+    ton = None if theta_on is None else np.ascontiguousarray(theta_on, np.float32)
+    toff = None if theta_off is None else np.ascontiguousarray(theta_off, np.float32)
+    assert (ton is None) == (toff is None)
     cap = 1 << 16
     while True:
         ev = np.zeros(cap, dtype=EVENT_DTYPE)
@@ -88,6 +93,7 @@ def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float,
         n = 0
         for i in range(1, S + 1):
             n += lib().evo_event_frame(H, W, 0, 0, i, S, float(T), float(c_pos), float(c_neg),
+                                       _f(ton) if ton is not None else None, _f(toff) if toff is not None else None,
                                        _f(frames[i - 1]), _f(lr), _f(lp), ev.ctypes.data, cap, n, None)
         if n <= cap:
             return ev[:n], lr
@@ -98,10 +104,15 @@ class Oracle:
     """Stateful oracle over E envs: ``step(keyframe)`` mirrors evis_step."""
 
     def __init__(self, num_envs: int, height: int, width: int, substeps: int, c_pos: float, c_neg: float,
-                 log_eps: float, keyframe_dt: float, composite_mode: int = 0, debug: bool = False):
+                 log_eps: float, keyframe_dt: float, composite_mode: int = 0, debug: bool = False,
+                 theta_on: Optional[np.ndarray] = None, theta_off: Optional[np.ndarray] = None):
         self.E, self.H, self.W, self.S = num_envs, height, width, substeps
         self.c_pos, self.c_neg, self.eps, self.T = c_pos, c_neg, log_eps, keyframe_dt
         self.mode = composite_mode
+        # Eq. 8: per-pixel ON / OFF thresholds [E,H,W] replacing c_pos / c_neg (both or neither)
+        assert (theta_on is None) == (theta_off is None)
+        self.th_on = None if theta_on is None else np.ascontiguousarray(theta_on, np.float32).reshape(num_envs, height, width)
+        self.th_off = None if theta_off is None else np.ascontiguousarray(theta_off, np.float32).reshape(num_envs, height, width)
         self.debug = debug
         self.calls = 0
         self.prev = None
@@ -150,6 +161,8 @@ class Oracle:
                 d = self.dbg
                 n += lib().evo_interval(
                     H, W, S, self.mode, e, kf, float(self.T), float(self.c_pos), float(self.c_neg),
+                    _f(self.th_on[e]) if self.th_on is not None else None,
+                    _f(self.th_off[e]) if self.th_off is not None else None,
                     _f(A["L"][e]), _f(A["fwd"][e]), _f(A["Z"][e]), _f(LB[e]), _f(mB[e]), _f(ZB[e]),
                     _f(Lref[e]), _f(Lprev[e]), _p(zA, C.c_uint64), _p(zB, C.c_uint64), _f(Lhat),
                     ev.ctypes.data, cap, n,

@@ -409,3 +409,41 @@ def test_event_count_cap_255():
     frames = np.array([100.0], np.float32).reshape(1, 1, 1)
     ev, lr = orc.event_frames(frames, np.zeros((1, 1), np.float32), 0.125, 0.125, 1.0)
     assert len(ev) == 255 and float(lr[0, 0]) == 255 * 0.125
+
+
+# ---- P11: threshold mismatch, Eq. 8: per-pixel theta_ON / theta_OFF ------------------------
+def test_p11_per_pixel_thresholds_closed_form():
+    """Every pixel follows Eq. 4 with ITS OWN thresholds: an up-ramp of D then a down-ramp back to 0 gives
+    floor(D / theta_on(u)) ON events and floor((D - r_on(u)) / theta_off(u)) OFF events, r_on the ON residual.
+    Dyadic thresholds and endpoints keep binary32 exact; the scalar c_pos / c_neg passed alongside are absurd
+    on purpose (a map that is ignored, or ON / OFF maps that are swapped, changes the counts)."""
+    th_on = np.array([[0.125, 0.25, 0.5], [0.25, 0.5, 0.125]], np.float32)
+    th_off = np.array([[0.5, 0.125, 0.25], [0.25, 0.25, 0.5]], np.float32)
+    H, W = th_on.shape
+    D = np.float32(2.1875)
+    up = np.linspace(0.0, float(D), 8, dtype=np.float64)[1:]
+    frames = np.concatenate([up, up[::-1][1:], [0.0]]).astype(np.float32)
+    frames = np.broadcast_to(frames[:, None, None], (len(frames), H, W)).copy()
+    ev, lr = orc.event_frames(frames, np.zeros((H, W), np.float32), 7.0, 9.0, 1.0, theta_on=th_on, theta_off=th_off)
+    for y in range(H):
+        for x in range(W):
+            on = sum(1 for e in ev if e["x"] == x and e["y"] == y and e["p"] > 0)
+            off = sum(1 for e in ev if e["x"] == x and e["y"] == y and e["p"] < 0)
+            n_on = math.floor(float(D) / float(th_on[y, x]))
+            top = n_on * float(th_on[y, x])                       # reference level after the up-ramp
+            n_off = math.floor(top / float(th_off[y, x]))
+            assert (on, off) == (n_on, n_off), (y, x, on, off, n_on, n_off)
+            assert float(lr[y, x]) == top - n_off * float(th_off[y, x])
+
+
+def test_p11b_constant_maps_equal_the_scalar_thresholds():
+    """Special case that reduces to Eq. 4 with one C: maps filled with (C+, C-) give the scalar result, event
+    for event (count, polarity, timestamp) and bit for bit in L_ref."""
+    r = _rng(11)
+    S, H, W = 12, 5, 6
+    frames = np.cumsum(r.normal(0, 0.3, size=(S, H, W)), axis=0).astype(np.float32)
+    L0 = np.zeros((H, W), np.float32)
+    ev0, lr0 = orc.event_frames(frames, L0, 0.2, 0.3, 1.0)
+    ev1, lr1 = orc.event_frames(frames, L0, 5.0, 5.0, 1.0, theta_on=np.full((H, W), 0.2, np.float32),
+                                theta_off=np.full((H, W), 0.3, np.float32))
+    assert len(ev0) == len(ev1) > 0 and np.array_equal(ev0, ev1) and np.array_equal(lr0, lr1)
