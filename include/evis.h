@@ -130,6 +130,16 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
 int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd,
                    const float *depth, uint64_t *n_events);
 
+/* Threshold mismatch (Eq. 8; R25): replace the scalar thresholds C+ / C- of the
+ * configuration by per-pixel maps theta_on, theta_off, each [E,H,W] float32, every value finite and > 0 (the
+ * caller samples them, e.g. max(N(C, sigma^2), theta_min), once per pixel).  DEVICE pointers if src_is_device != 0,
+ * else HOST.  The library copies the maps (the caller may free its buffers when the call returns; the call
+ * synchronises) and uses them from the next evis_step on: Eq. 4 at pixel u runs with theta_on(u) for dL > 0 and
+ * theta_off(u) for dL < 0.  Both NULL = back to the scalar thresholds.  Global path only.
+ * Errors: INVALID_ARG (exactly one pointer NULL; a value that is not finite and > 0 -- the previous thresholds
+ * stay in force), BAD_STATE (tile path), CUDA, OOM. */
+int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta_off, int src_is_device);
+
 /* Copy the events of the last step, in the deterministic order
  * (env, substep, tile row, tile column, y, x, crossing k), to `dst` (room for `max` events;
  * device pointer if dst_is_device != 0, else host).  Synchronises.  *n_out = events copied

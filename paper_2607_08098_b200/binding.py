@@ -53,7 +53,7 @@ class evis_profile(C.Structure):
 # every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
-           "evis_strerror", "evis_last_cuda_error", "evis_version"]
+           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds"]
 
 _lib = None
 
@@ -82,6 +82,7 @@ def load() -> C.CDLL:
     L.evis_destroy.argtypes = [vp]
     L.evis_strerror.argtypes = [C.c_int]
     L.evis_strerror.restype = C.c_char_p
+    L.evis_set_thresholds.argtypes = [vp, vp, vp, C.c_int]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
     for name in SYMBOLS:
@@ -152,6 +153,17 @@ class Evis:
                                  C.c_void_p(st), C.byref(n) if sync else None)
         _check(rc, "evis_step", allow)
         return int(n.value) if sync else None
+
+    def set_thresholds(self, theta_on: Optional[torch.Tensor], theta_off: Optional[torch.Tensor]) -> None:
+        """evis_set_thresholds (Eq. 8): per-pixel ON / OFF threshold maps [E,H,W] float32, CUDA tensors on this
+        context's device; both None = back to the scalar thresholds.  The library copies them."""
+        if theta_on is None and theta_off is None:
+            _check(self._lib.evis_set_thresholds(self._ctx, None, None, 1), "evis_set_thresholds")
+            return
+        E, H, W = self.E, self.H, self.W
+        p_on, p_off = _dev_ptr(theta_on, (E, H, W), "theta_on"), _dev_ptr(theta_off, (E, H, W), "theta_off")
+        torch.cuda.synchronize(self.device)                 # the library copies on its own stream
+        _check(self._lib.evis_set_thresholds(self._ctx, p_on, p_off, 1), "evis_set_thresholds")
 
     def step_host(self, rad, mv_bwd, depth, mv_fwd=None, allow=()) -> int:
         """evis_step_host: HOST buffers (numpy or CPU tensors); copies, runs and synchronises."""

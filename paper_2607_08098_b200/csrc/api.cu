@@ -25,6 +25,8 @@ struct evis_ctx {
     Keyframe kf[2];
     int cur;                          // kf[cur] receives the next keyframe; kf[cur^1] is A
     float *l_ref, *l_prev;
+    float *th_on, *th_off;            // Eq. 8 maps [E*H*W] (owned), in force when th_active
+    bool th_active;
     SubstepTable *tab;                // device
     SubstepTable h_tab;               // host copy (kernel parameter of the global path)
     EventParams ep;
@@ -163,7 +165,7 @@ void free_all(evis_ctx *ctx)
         if (k == 0) cudaFree(ctx->kf[k].L);
         cudaFree(ctx->kf[k].mv); cudaFree(ctx->kf[k].fwd); cudaFree(ctx->kf[k].Z);
     }
-    cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->tab); cudaFree(ctx->zmem);
+    cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->tab); cudaFree(ctx->zmem);
     cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
     cudaFree(ctx->st_rad); cudaFree(ctx->st_mv); cudaFree(ctx->st_fwd); cudaFree(ctx->st_depth);
@@ -419,6 +421,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
 
     ctx->ep.kf = (uint32_t)(ctx->steps - 1);
     EventSink sink{ctx->arrival, ctx->arrival_cap, ctx->counters + C_ALLOC, ctx->counters + C_EVENTS, ctx->directory};
+    const Thresholds th{ctx->th_active ? ctx->th_on : nullptr, ctx->th_active ? ctx->th_off : nullptr};
     {
         Span sp(ctx, st, EVIS_STAGE_CLEAR, 2);
         CU(cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), st));   // the per-step counters
@@ -469,7 +472,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 { Span sp(ctx, cs, EVIS_STAGE_SPLAT, multi ? 0 : 1, !multi); CU(launch_global_splat(g, zc, A, B, ctx->h_tab, cs)); }
                 {
                     Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 1, !multi);
-                    CU(launch_global_resolve(g, zc, A, B, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink,
+                    CU(launch_global_resolve(g, zc, A, B, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, th, sink,
                                              ctx->counters + C_HOLES, ctx->dbg, cs));
                 }
             }
@@ -489,7 +492,8 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         if (ctx->path == EVIS_PATH_GLOBAL) {
             const uint32_t tx = (g.W + G_TILE_W - 1) / G_TILE_W, ty = (g.H + G_TILE_H - 1) / G_TILE_H;
             CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
-                             ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, ctx->ep, tx, tx * ty, (uint32_t)g.S, st));
+                             ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, ctx->ep, th, (uint32_t)g.W,
+                             (uint32_t)g.HW, tx, tx * ty, (uint32_t)g.S, st));
         } else {
             CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
                             ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, st));
@@ -506,6 +510,48 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         if (ctx->last_overflow) return EVIS_ERR_OVERFLOW;
         if (ctx->last_motion) return EVIS_ERR_MOTION_BOUND;
     }
+    return EVIS_OK;
+}
+
+int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta_off, int src_is_device)
+{
+    if (!ctx || ((theta_on == nullptr) != (theta_off == nullptr))) return EVIS_ERR_INVALID_ARG;
+    if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    // work already enqueued keeps the thresholds it was launched with
+    if (ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    if (!theta_on) { ctx->th_active = false; return EVIS_OK; }
+    const size_t P = (size_t)ctx->g.E * ctx->g.HW;
+    float *on = nullptr, *off = nullptr;
+    unsigned long long *bad = nullptr, h_bad = 0;
+    int rc = EVIS_OK;
+    cudaError_t e = cudaMalloc((void **)&on, P * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&off, P * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&bad, sizeof *bad);
+    const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    cudaStream_t st = ctx->own_stream;
+    if (e == cudaSuccess) e = cudaMemsetAsync(bad, 0, sizeof *bad, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(on, theta_on, P * sizeof(float), kind, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(off, theta_off, P * sizeof(float), kind, st);
+    if (e == cudaSuccess) e = launch_check_positive(on, (long long)P, bad, st);
+    if (e == cudaSuccess) e = launch_check_positive(off, (long long)P, bad, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_bad, bad, sizeof h_bad, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        ctx->last_cuda = (int)e;
+        cudaGetLastError();
+        rc = e == cudaErrorMemoryAllocation ? EVIS_ERR_OOM : EVIS_ERR_CUDA;
+    } else if (h_bad) {
+        rc = EVIS_ERR_INVALID_ARG;                      // the previous thresholds stay in force
+    }
+    cudaFree(bad);
+    if (rc != EVIS_OK) { cudaFree(on); cudaFree(off); return rc; }
+    cudaFree(ctx->th_on); cudaFree(ctx->th_off);
+    if (!ctx->th_on) ctx->device_bytes += 2 * P * sizeof(float);
+    ctx->th_on = on; ctx->th_off = off;
+    ctx->th_active = true;
+    ctx->launches += 2;
     return EVIS_OK;
 }
 

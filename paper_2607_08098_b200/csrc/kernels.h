@@ -25,6 +25,12 @@ struct Geom {
     int mode;      // EVIS_COMPOSITE_*
 };
 
+// Eq. 8: per-pixel ON / OFF thresholds [E*H*W], device; both null = the scalar C+ / C- of
+// EventParams.
+struct Thresholds {
+    const float *on, *off;
+};
+
 struct DebugOut {  // all nullable; [S,E,H,W]
     uint32_t *win;
     uint8_t  *dir;
@@ -68,8 +74,8 @@ cudaError_t launch_global_splat(const Geom &g, const ZChunk &zc, const Keyframe 
                                 const SubstepTable &tab, cudaStream_t st);
 cudaError_t launch_global_resolve(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B,
                                   const SubstepTable &tab, float *l_ref, float *l_prev,
-                                  const EventParams &ep, const EventSink &sink, unsigned long long *holes,
-                                  const DebugOut &dbg, cudaStream_t st);
+                                  const EventParams &ep, const Thresholds &th, const EventSink &sink,
+                                  unsigned long long *holes, const DebugOut &dbg, cudaStream_t st);
 
 // ---- tile path (tile_path.cu): bounded motion, z-buffers in shared memory --------------------------
 struct TilePlan {
@@ -102,7 +108,9 @@ cudaError_t launch_order(const EventSink &sink, uint32_t num_entries, unsigned l
 // tiles_x, tiles = tiles per row / per frame of the G_TILE_W x G_TILE_H tiling; S = substeps.
 cudaError_t launch_expand(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out, uint4 *ordered,
                           unsigned long long capacity, const unsigned long long *step_events,
-                          unsigned long long *total_events, const EventParams &ep, uint32_t tiles_x, uint32_t tiles,
-                          uint32_t S, cudaStream_t st);
+                          unsigned long long *total_events, const EventParams &ep, const Thresholds &th, uint32_t W,
+                          uint32_t HW, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st);
+// number of values among theta[0..n) that are not (finite and > 0), added to *bad (prep.cu)
+cudaError_t launch_check_positive(const float *theta, long long n, unsigned long long *bad, cudaStream_t st);
 
 }  // namespace evis

@@ -101,4 +101,23 @@ cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, con
     return cudaGetLastError();
 }
 
+// Eq. 8 precondition: thresholds must be finite and > 0 (a zero threshold would fire without end)
+__global__ void __launch_bounds__(256) k_check_positive(const float *__restrict__ theta, long long n, unsigned long long *bad)
+{
+    unsigned int mine = 0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float v = theta[i];
+        if (!(v > 0.0f && v < __int_as_float(0x7f800000))) ++mine;
+    }
+    mine = __reduce_add_sync(0xFFFFFFFFu, mine);
+    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(bad, (unsigned long long)mine);
+}
+
+cudaError_t launch_check_positive(const float *theta, long long n, unsigned long long *bad, cudaStream_t st)
+{
+    const long long blocks = (n + 255) / 256;
+    k_check_positive<<<(unsigned)(blocks < 4096 ? (blocks < 1 ? 1 : blocks) : 4096), 256, 0, st>>>(theta, n, bad);
+    return cudaGetLastError();
+}
+
 }  // namespace evis

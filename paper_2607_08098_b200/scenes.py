@@ -23,7 +23,7 @@ from __future__ import annotations
 
 import math
 from dataclasses import dataclass, field, replace
-from typing import Dict, List, Optional, Sequence
+from typing import Dict, List, Optional, Sequence, Tuple
 
 import torch
 
@@ -349,6 +349,24 @@ def _paint_noise(scene: Scene, k: int, device, envs: Sequence[int]) -> Dict[str,
     return {"rad": rad.to(torch.float32).contiguous(), "depth": depth.to(torch.float32).contiguous(),
             "mv_bwd": torch.stack(mv[0:2], dim=-1).to(torch.float32).contiguous(),
             "mv_fwd": torch.stack(mv[2:4], dim=-1).to(torch.float32).contiguous()}
+
+
+def threshold_maps(spec: SceneSpec, sigma: float = 0.03, theta_min: float = 0.01, device="cpu"
+                   ) -> Tuple[torch.Tensor, torch.Tensor]:
+    """Seeded per-pixel ON / OFF threshold maps [E,H,W] float32 for evis_set_thresholds: the draw the paper
+    states for threshold mismatch, theta ~ max(N(C, sigma^2), theta_min), once per pixel (PAPER.md:137-142,
+    Eq. 8).  Input synthesis only (the method's arithmetic is not here): Box-Muller on the counter hash of
+    (pixel, salt), in float64 on the CPU so that the maps do not depend on the device."""
+    E, H, W = spec.num_envs, spec.height, spec.width
+    iy, ix = torch.meshgrid(torch.arange(E * H, dtype=torch.int64), torch.arange(W, dtype=torch.int64), indexing="ij")
+    out = []
+    for salt, c in ((0x51ED + spec.seed, spec.c_pos), (0xA7C3 + spec.seed, spec.c_neg)):
+        u1 = _hash01(ix, iy, salt).double().clamp_min(1e-12)
+        u2 = _hash01(ix, iy, salt + 1).double()
+        n = torch.sqrt(-2.0 * torch.log(u1)) * torch.cos(2.0 * math.pi * u2)
+        theta = torch.clamp(c + sigma * n, min=theta_min).float().reshape(E, H, W).contiguous()
+        out.append(theta.to(device))
+    return out[0], out[1]
 
 
 def render_keyframe(scene: Scene, k: int, device="cpu", envs: Optional[Sequence[int]] = None

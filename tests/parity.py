@@ -61,7 +61,7 @@ def _counts(ev, E, S, H, W, env_map=None):
 
 def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int, S: int, H: int, W: int,
                  c_pos: float, c_neg: float, rep: ParityReport, kf: int,
-                 gpu_dbg=None, env_sel: Optional[Sequence[int]] = None) -> None:
+                 gpu_dbg=None, env_sel: Optional[Sequence[int]] = None, thresholds=None) -> None:
     """Compare one step.  ``env_sel``: the oracle ran only these envs of the GPU batch (oracle env j =
     GPU env env_sel[j]); GPU events of other envs are ignored."""
     if env_sel is not None:
@@ -104,6 +104,8 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
             seen.add((e, y, x))
             dL = float(ora.dbg["dL"][e, s, y, x])
             C = c_pos if dL > 0 else c_neg
+            if thresholds is not None:              # Eq. 8: the pixel's own thresholds, [Eo,H,W] numpy
+                C = float((thresholds[0] if dL > 0 else thresholds[1])[e, y, x])
             k = round(abs(dL) / C)
             assert abs(abs(dL) - k * C) < TOL_TIE, \
                 f"event mismatch not at a tie: env {e} substep {s + 1} ({x},{y}) dL={dL} gpu={cg[e, s, y, x]} oracle={co[e, s, y, x]}"
@@ -122,7 +124,7 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
 
 def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Sequence[int]] = None,
                mode: int = 0, path: int = binding.PATH_GLOBAL, use_fwd: bool = True, debug: bool = True,
-               capacity: int = 1 << 24, max_motion: Optional[float] = None) -> ParityReport:
+               capacity: int = 1 << 24, max_motion: Optional[float] = None, thresholds=None) -> ParityReport:
     """GPU runs the whole batch; the oracle runs ``envs`` (default: all).  Returns the report after
     asserting every bit-exact criterion; tolerances are asserted by the caller on the report."""
     sc = scenes.make_scene(spec)
@@ -131,8 +133,13 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
     mm = spec.max_motion_px() if max_motion is None else max_motion
     ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, max_motion_px=mm,
                       composite_mode=mode, path=path, event_capacity=capacity, debug_capture=debug)
+    th_np = None
+    if thresholds is not None:                      # (theta_on, theta_off) CUDA tensors [E,H,W] (Eq. 8)
+        ev.set_thresholds(thresholds[0], thresholds[1])
+        th_np = (thresholds[0][sel].cpu().numpy(), thresholds[1][sel].cpu().numpy())
     ora = orc.Oracle(len(sel), H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
-                     composite_mode=mode, debug=True)
+                     composite_mode=mode, debug=True, theta_on=None if th_np is None else th_np[0],
+                     theta_off=None if th_np is None else th_np[1])
     rep = ParityReport()
     try:
         for k in range(n_keyframes):
@@ -148,7 +155,7 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
             assert len(ge) == n
             dbg = ev.debug_read() if debug else None
             compare_step(ge, oe, ora, E, S, H, W, spec.c_pos, spec.c_neg, rep, k - 1, dbg,
-                         None if envs is None else sel)
+                         None if envs is None else sel, th_np)
             lref, lprev = ev.get_state()
             if rep.ties == 0:
                 assert np.array_equal(lref[sel], ora.Lref), "carried L_ref differs"

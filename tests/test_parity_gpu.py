@@ -187,6 +187,75 @@ def test_concurrent_regions_and_direct_loads(monkeypatch, streams, no_tma):
     _assert_tolerances(rep)
 
 
+def test_threshold_maps_eq8():
+    """Threshold mismatch (Eq. 8): per-pixel theta_ON / theta_OFF maps drawn as
+    max(N(C, sigma^2), theta_min) by the seeded generator; events, counts, L_ref and timestamps must match the
+    oracle run with the same maps.  sigma is large so that neighbouring pixels really differ."""
+    spec = scenes.small(scenes.config(4), num_envs=3, height=130, width=173, num_keyframes=4)
+    th = scenes.threshold_maps(spec, sigma=0.05, theta_min=0.02, device="cuda")
+    assert float(th[0].std()) > 0.03 and float(th[0].min()) >= float(np.float32(0.02))
+    rep = parity.run_parity(spec, 4, path=binding.PATH_GLOBAL, thresholds=th)
+    _assert_tolerances(rep)
+    assert rep.events_oracle > 0
+    # and the maps change the result: the scalar run of the same scene differs
+    rep0 = parity.run_parity(spec, 4, path=binding.PATH_GLOBAL)
+    assert rep0.events_oracle != rep.events_oracle
+
+
+def test_threshold_maps_api_contract():
+    """evis_set_thresholds: one NULL map or a non-positive value is INVALID_ARG and leaves the thresholds in
+    force; constant maps equal the scalar thresholds event for event; (NULL, NULL) restores the scalars; the tile
+    path refuses the maps."""
+    spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=3)
+    E, H, W = spec.num_envs, spec.height, spec.width
+    sc = scenes.make_scene(spec)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(3)]
+
+    def run(setup):
+        ev = binding.Evis(E, H, W, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                          path=binding.PATH_GLOBAL, event_capacity=1 << 22)
+        setup(ev)
+        out = []
+        for kf in kfs:
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+            out.append(ev.read_events().copy())
+        ev.destroy()
+        return np.concatenate(out)
+
+    on = torch.full((E, H, W), spec.c_pos, device="cuda")
+    off = torch.full((E, H, W), spec.c_neg, device="cuda")
+    base = run(lambda ev: None)
+    assert len(base) > 0
+    assert np.array_equal(base, run(lambda ev: ev.set_thresholds(on, off)))
+
+    def bad(ev):
+        with pytest.raises(binding.EvisError) as ei:
+            ev.set_thresholds(on, None)
+        assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+        z = on.clone(); z[0, 3, 5] = 0.0
+        with pytest.raises(binding.EvisError) as ei:
+            ev.set_thresholds(z, off)
+        assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+        z[0, 3, 5] = float("nan")
+        with pytest.raises(binding.EvisError) as ei:
+            ev.set_thresholds(on, z)
+        assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+    assert np.array_equal(base, run(bad))
+
+    def set_and_clear(ev):
+        ev.set_thresholds(on * 3.0, off * 3.0)
+        ev.set_thresholds(None, None)
+    assert np.array_equal(base, run(set_and_clear))
+    assert len(run(lambda ev: ev.set_thresholds(on * 3.0, off * 3.0))) < len(base)
+
+    ev = binding.Evis(E, H, W, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                      max_motion_px=spec.max_motion_px(), path=binding.PATH_TILE, event_capacity=1 << 22)
+    with pytest.raises(binding.EvisError) as ei:
+        ev.set_thresholds(on, off)
+    assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    ev.destroy()
+
+
 def _run_stream(spec, n_kf, path, seed_offset=0):
     sc = scenes.make_scene(spec)
     ev = binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg,
