@@ -63,6 +63,8 @@ def parse_args():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=6)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE.json config 5: one JSON line per (envs x resolution x S) point, device-resident")
     return ap.parse_args()
 
 
@@ -346,9 +348,61 @@ def run_ours(args, spec) -> None:
         dist.destroy_process_group()
 
 
+def run_sweep(args) -> None:
+    """BASELINE.json configs[4]: throughput at (roughly) fixed total pixels over envs x resolution x S, analytic
+    rectangle scenes as config 1.  One JSON line per point: pixel-substeps/s, events/s, fraction of the HBM
+    roofline (algorithmic bytes of the point / time / measured copy peak).  Single GPU, device-resident inputs."""
+    import torch
+    from paper_2607_08098_b200 import binding, scenes
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    binding.load()
+    peak, peak_src = hbm_peak()
+    K, Wm = args.steps, args.warmup
+    for spec in scenes.sweep_points():
+        E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+        sc = scenes.make_scene(spec)
+        kfs = [scenes.render_keyframe(sc, k, device=dev) for k in range(Wm + K + 1)]
+        ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                          max_motion_px=spec.max_motion_px(), path=binding.PATH_AUTO, device=0,
+                          event_capacity=int(min(0x7FFFFFFF, max(1 << 22, 10 * E * H * W))))
+        stream = torch.cuda.current_stream(dev)
+        for k in range(Wm + 1):
+            f = kfs[k]
+            ev.step(f["rad"], f["mv_bwd"], f["depth"], mv_fwd=f["mv_fwd"], stream=stream)
+        torch.cuda.synchronize(dev)
+        i0 = ev.info()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for k in range(Wm + 1, Wm + 1 + K):
+            f = kfs[k]
+            ev.step(f["rad"], f["mv_bwd"], f["depth"], mv_fwd=f["mv_fwd"], stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        ms = e0.elapsed_time(e1)
+        i1 = ev.info()
+        if i1.last_overflow:
+            raise SystemExit("bench.py: event capacity overflow in the sweep")
+        events = i1.total_events - i0.total_events
+        ev.destroy()
+        del kfs
+        torch.cuda.empty_cache()
+        algo = (ALGO_BYTES_PER_PIXEL * E * H * W) * K + ALGO_BYTES_PER_EVENT * events
+        print(json.dumps({"metric": METRIC, "workload": spec.name, "envs": E, "height": H, "width": W, "substeps": S,
+                          "value": E * H * W * S * K / (ms * 1e-3), "unit": METRIC, "events_per_s": events / (ms * 1e-3),
+                          "ms_per_step": ms / K, "steps": K, "warmup": Wm,
+                          "hbm_roofline_frac": algo / (ms * 1e-3) / 1e9 / peak, "hbm_peak_gbs": peak,
+                          "x_realtime": spec.keyframe_dt / (ms / K * 1e-3)}), flush=True)
+
+
 def main():
     args = parse_args()
     from paper_2607_08098_b200 import scenes
+    if args.sweep:
+        run_sweep(args)
+        return
     spec = scenes.config(args.config)
     if args.envs:
         spec = scenes.small(spec, num_envs=args.envs, name=f"{spec.name}_E{args.envs}")

@@ -187,6 +187,19 @@ def test_concurrent_regions_and_direct_loads(monkeypatch, streams, no_tma):
     _assert_tolerances(rep)
 
 
+@pytest.mark.parametrize("point", [2, 7, 11, 15, 18, 19])
+def test_config5_sweep_shapes_reduced(point):
+    """BASELINE.json config 5 (throughput sweep): the sweep's own scene recipe, resolutions and substep counts
+    (S = 8, 16, 33, 166), reduced to 2 envs (and a 1920-wide strip of 64 rows for the full-HD point) so that the
+    oracle finishes in seconds."""
+    spec = scenes.sweep_points()[point]
+    spec = scenes.small(spec, num_envs=min(2, spec.num_envs), height=min(spec.height, 64 if spec.width > 1000 else 10 ** 6),
+                        num_keyframes=3)
+    rep = parity.run_parity(spec, 3, path=binding.PATH_AUTO)
+    _assert_tolerances(rep)
+    assert rep.events_oracle > 0
+
+
 def test_threshold_maps_eq8():
     """Threshold mismatch (Eq. 8): per-pixel theta_ON / theta_OFF maps drawn as
     max(N(C, sigma^2), theta_min) by the seeded generator; events, counts, L_ref and timestamps must match the
