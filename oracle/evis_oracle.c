@@ -14,14 +14,15 @@
  * level that feeds the next count) is taken in the kernel's precision, IEEE binary32 with the
  * operation order written below (compile with -ffp-contract=off so that only the fmaf() calls
  * written here are fused).  The log-luminance is evaluated in binary64 and rounded once to
- * binary32.  Timestamps decide nothing and are computed in binary64.
+ * binary32.  Timestamps decide nothing and are computed in binary64 -- unless the refractory period
+ * is on: then they decide which crossings are emitted and are computed in binary32 [R26].
  *
  * Readings of the paper where it is silent or ambiguous are listed in DESIGN.md ("Readings");
  * the tag [Rn] below names the reading a line depends on.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 zero motion identity, P2 substep S reproduces
  * keyframe B, P3 integer translation, P4 8x8 gather-form brute force, P5 analytic two-rectangle
- * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8).  UNPINNED by paper or
+ * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8), P12 refractory period.  UNPINNED by paper or
  * mathematics (fixed by DESIGN.md readings only): log base R1, epsilon R2, initial reference
  * level R6, nearest-pixel depth lookup R16, hole handling R20, the composite choice R19.
  */
@@ -162,6 +163,7 @@ void evo_composite(int H, int W, int i, int S, int mode,
 int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
                         float c_pos, float c_neg,
                         const float *th_on, const float *th_off,   /* [H*W] or NULL (both): Eq. 8 maps */
+                        float tau_r, float *t_last,                /* refractory period (<= 0: off) and its state */
                         const float *Lhat,
                         float *Lref, float *Lprev,
                         evo_event *ev, int64_t cap, int64_t n_have,
@@ -184,7 +186,30 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
                 float r = floorf(fabsf(d) / C);
                 n = r >= 255.0f ? 255 : (int)r;
             }
-            for (int k = 1; k <= n; ++k) {
+            for (int k = 1; k <= n && tau_r > 0.0f; ++k) {
+                /* Refractory period [R26]: the crossing is stamped in binary32 (the stamp now
+                 * decides an integer: emitted or not) with the operation order below, and it is emitted iff
+                 * t - t_last >= tau_r, t_last = stamp of the pixel's last EMITTED event, kept relative to the
+                 * start of the current interval.  L_ref follows every crossing, emitted or not (Eq. 4).       */
+                const float dtf = T / (float)S;
+                const float lev = fmaf((float)(p * k), C, Lref[q]);
+                const float num = lev - Lprev[q], den = L - Lprev[q];
+                float fr = 1.0f;
+                if (den != 0.0f) fr = num / den;
+                if (!(fr >= 0.0f)) fr = 0.0f;
+                if (fr > 1.0f) fr = 1.0f;
+                const float t = fmaf(fr, dtf, (float)(i - 1) * dtf);
+                if (!(t - t_last[q] >= tau_r)) continue;              /* suppressed */
+                t_last[q] = t;
+                if (n_have + made < cap) {
+                    evo_event *o = &ev[n_have + made];
+                    o->env = env; o->x = x; o->y = y; o->p = p; o->substep = i; o->k = k;
+                    o->kf = kf; o->pad = 0;
+                    o->t_off = (double)t;
+                }
+                ++made;
+            }
+            for (int k = 1; k <= n && !(tau_r > 0.0f); ++k) {
                 const float lev = fmaf((float)(p * k), C, Lref[q]);
                 const double den = (double)L - (double)Lprev[q];
                 double fr = 1.0;
@@ -211,6 +236,7 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
  * Optional debug outputs, each [S][H*W] or NULL: winners of each direction, composite, Lhat.     */
 int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, float c_pos, float c_neg,
                      const float *th_on, const float *th_off,              /* [H*W] or NULL: Eq. 8 maps of this env */
+                     float tau_r, float *t_last,                           /* refractory period (<= 0: off), state [H*W] */
                      const float *LA, const float *fwdA, const float *ZA,
                      const float *LB, const float *mB, const float *ZB,
                      float *Lref, float *Lprev,
@@ -234,8 +260,11 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, fl
             if (dbg_Lhat) dbg_Lhat[(int64_t)(i - 1) * P + q] = Lhat[q];
             if (holes && zA[q] == EVO_EMPTY && zB[q] == EVO_EMPTY) ++*holes;
         }
-        made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, th_on, th_off, Lhat, Lref, Lprev,
+        made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, th_on, th_off, tau_r, t_last, Lhat, Lref, Lprev,
                                 ev, cap, n_have + made, dbg_dL ? dbg_dL + (int64_t)(i - 1) * P : 0);
     }
+    /* the next interval starts T later: keep t_last relative to its start (binary32, -inf stays -inf) [R26] */
+    if (tau_r > 0.0f)
+        for (int64_t q = 0; q < P; ++q) t_last[q] = t_last[q] - T;
     return made;
 }

@@ -33,10 +33,10 @@ def lib():
         L.evo_splat.restype = None
         L.evo_composite.argtypes = [C.c_int] * 5 + [u64p, u64p, fp, fp, fp, fp, u8p, u32p]
         L.evo_composite.restype = None
-        L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [fp, fp, fp, C.c_void_p,
+        L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [fp, fp, fp, C.c_void_p,
                                                                         C.c_int64, C.c_int64, fp]
         L.evo_event_frame.restype = C.c_int64
-        L.evo_interval.argtypes = ([C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [fp] * 8 + [u64p, u64p, fp]
+        L.evo_interval.argtypes = ([C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [fp] * 8 + [u64p, u64p, fp]
                                    + [C.c_void_p, C.c_int64, C.c_int64]
                                    + [u32p, u32p, u8p, u32p, fp, fp, C.POINTER(C.c_int64)])
         L.evo_interval.restype = C.c_int64
@@ -74,9 +74,11 @@ def splat(i: int, S: int, src_is_B: bool, disp: np.ndarray, Zsrc: np.ndarray, Zo
 
 def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float, T: float,
                  Lref0: Optional[np.ndarray] = None, theta_on: Optional[np.ndarray] = None,
-                 theta_off: Optional[np.ndarray] = None):
+                 theta_off: Optional[np.ndarray] = None, tau_r: float = 0.0, t_last0: Optional[np.ndarray] = None):
     """Event stage alone (Eq. 4): feed a sequence of S log frames [S,H,W] to one env.
     theta_on / theta_off [H,W]: per-pixel thresholds replacing c_pos / c_neg (Eq. 8).
+    tau_r > 0: refractory period; t_last0 [H,W] = stamps of the last emitted events relative to
+    the start of these frames (default -inf); the final t_last is returned as a third value.
 
     Returns (events, Lref_final).  Lref and Lprev start at L0 (or Lref0 for the reference)."""
     frames = np.ascontiguousarray(frames, np.float32)
@@ -86,17 +88,19 @@ def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float,
     ton = None if theta_on is None else np.ascontiguousarray(theta_on, np.float32)
     toff = None if theta_off is None else np.ascontiguousarray(theta_off, np.float32)
     assert (ton is None) == (toff is None)
+    tl0 = np.full((H, W), -np.inf, np.float32) if t_last0 is None else np.ascontiguousarray(t_last0, np.float32)
     cap = 1 << 16
     while True:
         ev = np.zeros(cap, dtype=EVENT_DTYPE)
         lr, lp = Lref.copy(), Lprev.copy()
+        tl = tl0.copy()
         n = 0
         for i in range(1, S + 1):
             n += lib().evo_event_frame(H, W, 0, 0, i, S, float(T), float(c_pos), float(c_neg),
                                        _f(ton) if ton is not None else None, _f(toff) if toff is not None else None,
-                                       _f(frames[i - 1]), _f(lr), _f(lp), ev.ctypes.data, cap, n, None)
+                                       float(tau_r), _f(tl), _f(frames[i - 1]), _f(lr), _f(lp), ev.ctypes.data, cap, n, None)
         if n <= cap:
-            return ev[:n], lr
+            return (ev[:n], lr, tl) if tau_r > 0.0 else (ev[:n], lr)
         cap = int(n)
 
 
@@ -105,7 +109,8 @@ class Oracle:
 
     def __init__(self, num_envs: int, height: int, width: int, substeps: int, c_pos: float, c_neg: float,
                  log_eps: float, keyframe_dt: float, composite_mode: int = 0, debug: bool = False,
-                 theta_on: Optional[np.ndarray] = None, theta_off: Optional[np.ndarray] = None):
+                 theta_on: Optional[np.ndarray] = None, theta_off: Optional[np.ndarray] = None,
+                 tau_r: float = 0.0):
         self.E, self.H, self.W, self.S = num_envs, height, width, substeps
         self.c_pos, self.c_neg, self.eps, self.T = c_pos, c_neg, log_eps, keyframe_dt
         self.mode = composite_mode
@@ -114,6 +119,9 @@ class Oracle:
         self.th_on = None if theta_on is None else np.ascontiguousarray(theta_on, np.float32).reshape(num_envs, height, width)
         self.th_off = None if theta_off is None else np.ascontiguousarray(theta_off, np.float32).reshape(num_envs, height, width)
         self.debug = debug
+        # refractory period: stamps of the last emitted events, relative to the current interval
+        self.tau_r = float(tau_r)
+        self.t_last = np.full((num_envs, height, width), -np.inf, np.float32)
         self.calls = 0
         self.prev = None
         self.Lref = None
@@ -155,6 +163,7 @@ class Oracle:
         while True:
             ev = np.zeros(cap, dtype=EVENT_DTYPE)
             Lref, Lprev = self.Lref.copy(), self.Lprev.copy()
+            t_last = self.t_last.copy()
             holes.value = 0
             n = 0
             for e in range(E):
@@ -163,6 +172,7 @@ class Oracle:
                     H, W, S, self.mode, e, kf, float(self.T), float(self.c_pos), float(self.c_neg),
                     _f(self.th_on[e]) if self.th_on is not None else None,
                     _f(self.th_off[e]) if self.th_off is not None else None,
+                    self.tau_r, _f(t_last[e]),
                     _f(A["L"][e]), _f(A["fwd"][e]), _f(A["Z"][e]), _f(LB[e]), _f(mB[e]), _f(ZB[e]),
                     _f(Lref[e]), _f(Lprev[e]), _p(zA, C.c_uint64), _p(zB, C.c_uint64), _f(Lhat),
                     ev.ctypes.data, cap, n,
@@ -172,7 +182,7 @@ class Oracle:
             if n <= cap:
                 break
             cap = int(n)
-        self.Lref, self.Lprev = Lref, Lprev
+        self.Lref, self.Lprev, self.t_last = Lref, Lprev, t_last
         self.holes = holes.value
         self.prev = cur
         self.calls += 1

@@ -447,3 +447,82 @@ def test_p11b_constant_maps_equal_the_scalar_thresholds():
     ev1, lr1 = orc.event_frames(frames, L0, 5.0, 5.0, 1.0, theta_on=np.full((H, W), 0.2, np.float32),
                                 theta_off=np.full((H, W), 0.3, np.float32))
     assert len(ev0) == len(ev1) > 0 and np.array_equal(ev0, ev1) and np.array_equal(lr0, lr1)
+
+
+# ---- P12: refractory period [R26] --------------------------------------------------------------
+def _greedy(times, tau, t_last=-math.inf):
+    out = []
+    for k, t in enumerate(times, start=1):
+        if t - t_last >= tau:
+            out.append(k)
+            t_last = t
+    return out
+
+
+@pytest.mark.parametrize("tau_num,expect_stride", [(2.5, 3), (3.0, 3), (3.0625, 4), (0.5, 1)])
+def test_p12_refractory_on_a_linear_ramp(tau_num, expect_stride):
+    """L rises by 4.0 = 32 C over one interval, sampled at S = 8 frames: the crossings fall at t_k = k / 32
+    (dyadic, exact in binary32).  With tau_r = tau_num / 32 the emitted crossings are the greedy subsequence
+    with gaps >= tau_r (>= : a gap of exactly tau_r is emitted), computed here on exact rationals; L_ref is the
+    same as without a refractory period (it follows every crossing)."""
+    C, S, T = 0.125, 8, 1.0
+    frames = (np.arange(1, S + 1, dtype=np.float32) * np.float32(0.5)).reshape(S, 1, 1)
+    L0 = np.zeros((1, 1), np.float32)
+    tau = tau_num / 32.0
+    ev, lr, tl = orc.event_frames(frames, L0, C, C, T, tau_r=tau)
+    ev0, lr0 = orc.event_frames(frames, L0, C, C, T)
+    assert len(ev0) == 32 and float(lr[0, 0]) == float(lr0[0, 0]) == 4.0
+    want = _greedy([k / 32.0 for k in range(1, 33)], tau)
+    assert want == list(range(1, 33, expect_stride))
+    got = [round(float(e["t_off"]) * 32) for e in ev]
+    assert got == want and all(abs(float(e["t_off"]) - k / 32.0) < 1e-7 for e, k in zip(ev, want))
+    assert all(int(e["p"]) == 1 for e in ev)
+    assert float(tl[0, 0]) == want[-1] / 32.0
+
+
+def test_p12b_refractory_state_carries_into_the_frames():
+    """t_last0 = -1/64 (an event 1/64 s before the interval started), tau_r = 3/64: the first crossing at
+    t = 1/32 = 2/64 has a gap of exactly 3/64 and is emitted; with t_last0 = -1/128 it is suppressed and the
+    second (t = 2/32) is the first one out."""
+    C, S, T = 0.125, 8, 1.0
+    frames = (np.arange(1, S + 1, dtype=np.float32) * np.float32(0.5)).reshape(S, 1, 1)
+    L0 = np.zeros((1, 1), np.float32)
+    for t0, first in ((-1.0 / 64, 1), (-1.0 / 128, 2)):
+        ev, lr, tl = orc.event_frames(frames, L0, C, C, T, tau_r=3.0 / 64, t_last0=np.full((1, 1), t0, np.float32))
+        times = [k / 32.0 for k in range(1, 33)]
+        want = _greedy(times, 3.0 / 64, t0)
+        assert want[0] == first
+        assert [round(float(e["t_off"]) * 32) for e in ev] == want
+
+
+def test_p12c_refractory_across_intervals_in_the_full_oracle():
+    """Whole oracle, three intervals of a flickering uniform scene (zero motion): consecutive emitted events of a
+    pixel are at least tau_r apart in absolute time, also across keyframes (t_last is carried, shifted by T);
+    events are a subset of the run without refractory period with the same stamps; L_ref is unchanged."""
+    E, H, W, S, T, C, tau = 1, 3, 4, 4, 1.0 / 60.0, 0.2, 0.004
+    r = _rng(12)
+    kfs = []
+    for k in range(4):
+        lum = np.exp(r.uniform(-2.0, 2.0, size=(E, H, W))).astype(np.float32)
+        kfs.append(dict(rad=np.repeat(lum[..., None], 3, axis=-1).copy(), mv=np.zeros((E, H, W, 2), np.float32),
+                        z=np.ones((E, H, W), np.float32)))
+    o_ref = orc.Oracle(E, H, W, S, C, C, 1e-3, T, tau_r=tau)
+    o_all = orc.Oracle(E, H, W, S, C, C, 1e-3, T)
+    ev_ref, ev_all = [], []
+    for kf in kfs:
+        ev_ref.append(o_ref.step(kf["rad"], kf["mv"], kf["z"]))
+        ev_all.append(o_all.step(kf["rad"], kf["mv"], kf["z"]))
+    assert np.array_equal(o_ref.Lref, o_all.Lref)
+    a, b = np.concatenate(ev_ref), np.concatenate(ev_all)
+    assert 0 < len(a) < len(b)
+    key = lambda e: (int(e["kf"]), int(e["y"]), int(e["x"]), int(e["substep"]), int(e["k"]))
+    tb = {key(e): float(e["t_off"]) for e in b}
+    assert all(key(e) in tb and abs(tb[key(e)] - float(e["t_off"])) < 1e-6 for e in a)
+    last = {}
+    for e in a:                                                   # stream order is time order per pixel
+        p, t = (int(e["y"]), int(e["x"])), int(e["kf"]) * T + float(e["t_off"])
+        if p in last:
+            assert t - last[p] >= tau - 1e-6
+        last[p] = t
+    for (y, x), t in last.items():                                # carried state = last stamp relative to the NEXT interval
+        assert abs(float(o_ref.t_last[0, y, x]) - (t - 3 * T)) < 1e-6
