@@ -140,6 +140,15 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
  * stay in force), BAD_STATE (tile path), CUDA, OOM. */
 int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta_off, int src_is_device);
 
+/* Refractory period (R26): with tau_r > 0 (seconds) a threshold crossing of a pixel is
+ * emitted only if its timestamp t satisfies t - t_last >= tau_r, t_last being the timestamp of the pixel's last
+ * EMITTED event (none before the call: every pixel starts free); suppressed crossings still move L_ref (Eq. 4 is
+ * unchanged).  The timestamps then decide which events exist, so they are computed in IEEE binary32 with a fixed
+ * operation order.  The state t_last is carried across steps.  tau_r = 0 switches the period off.  Calling it
+ * again with tau_r > 0 resets t_last.  Applies from the next evis_step on; synchronises.  Global path only.
+ * Errors: INVALID_ARG (negative or non-finite tau_r), BAD_STATE (tile path), CUDA, OOM. */
+int evis_set_refractory(evis_ctx *ctx, float tau_r);
+
 /* Copy the events of the last step, in the deterministic order
  * (env, substep, tile row, tile column, y, x, crossing k), to `dst` (room for `max` events;
  * device pointer if dst_is_device != 0, else host).  Synchronises.  *n_out = events copied

@@ -27,6 +27,8 @@ struct evis_ctx {
     float *l_ref, *l_prev;
     float *th_on, *th_off;            // Eq. 8 maps [E*H*W] (owned), in force when th_active
     bool th_active;
+    float *t_last;                    // refractory state [E*H*W] (owned), in force when tau_r > 0
+    float tau_r;
     SubstepTable *tab;                // device
     SubstepTable h_tab;               // host copy (kernel parameter of the global path)
     EventParams ep;
@@ -165,7 +167,7 @@ void free_all(evis_ctx *ctx)
         if (k == 0) cudaFree(ctx->kf[k].L);
         cudaFree(ctx->kf[k].mv); cudaFree(ctx->kf[k].fwd); cudaFree(ctx->kf[k].Z);
     }
-    cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->tab); cudaFree(ctx->zmem);
+    cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last); cudaFree(ctx->tab); cudaFree(ctx->zmem);
     cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
     cudaFree(ctx->st_rad); cudaFree(ctx->st_mv); cudaFree(ctx->st_fwd); cudaFree(ctx->st_depth);
@@ -423,6 +425,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     ctx->ep.kf = (uint32_t)(ctx->steps - 1);
     EventSink sink{ctx->arrival, ctx->arrival_cap, ctx->counters + C_ALLOC, ctx->counters + C_EVENTS, ctx->directory};
     const Thresholds th{ctx->th_active ? ctx->th_on : nullptr, ctx->th_active ? ctx->th_off : nullptr};
+    const Refractory rf{ctx->tau_r > 0.0f ? ctx->t_last : nullptr, ctx->tau_r, ctx->cfg.keyframe_dt};
     {
         Span sp(ctx, st, EVIS_STAGE_CLEAR, 2);
         CU(cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), st));   // the per-step counters
@@ -473,7 +476,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 { Span sp(ctx, cs, EVIS_STAGE_SPLAT, multi ? 0 : 1, !multi); CU(launch_global_splat(g, zc, A, B, ctx->h_tab, cs)); }
                 {
                     Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 1, !multi);
-                    CU(launch_global_resolve(g, zc, A, B, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, th, sink,
+                    CU(launch_global_resolve(g, zc, A, B, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, th, rf, sink,
                                              ctx->counters + C_HOLES, ctx->dbg, cs));
                 }
             }
@@ -490,7 +493,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     }
     {
         Span sp(ctx, st, EVIS_STAGE_ORDER, 3);
-        if (ctx->path == EVIS_PATH_GLOBAL) {
+        if (ctx->path == EVIS_PATH_GLOBAL && !rf.t_last) {
             const uint32_t tx = (g.W + G_TILE_W - 1) / G_TILE_W, ty = (g.H + G_TILE_H - 1) / G_TILE_H;
             CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
                              ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, ctx->ep, th, (uint32_t)g.W,
@@ -548,11 +551,30 @@ int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta
     }
     cudaFree(bad);
     if (rc != EVIS_OK) { cudaFree(on); cudaFree(off); return rc; }
-    cudaFree(ctx->th_on); cudaFree(ctx->th_off);
+    cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last);
     if (!ctx->th_on) ctx->device_bytes += 2 * P * sizeof(float);
     ctx->th_on = on; ctx->th_off = off;
     ctx->th_active = true;
     ctx->launches += 2;
+    return EVIS_OK;
+}
+
+int evis_set_refractory(evis_ctx *ctx, float tau_r)
+{
+    if (!ctx || !(tau_r >= 0.0f) || !(tau_r < 3.0e38f)) return EVIS_ERR_INVALID_ARG;
+    if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    if (tau_r > 0.0f) {
+        // (re)start with no event emitted yet: t_last = -inf at every pixel
+        const size_t P = (size_t)ctx->g.E * ctx->g.HW;
+        if (!ctx->t_last) CU(dalloc(ctx, &ctx->t_last, P));
+        CU(launch_fill(ctx->t_last, (long long)P, -INFINITY, ctx->own_stream));
+        CU(cudaStreamSynchronize(ctx->own_stream));
+        ctx->launches += 1;
+    }
+    ctx->tau_r = tau_r;
     return EVIS_OK;
 }
 

@@ -31,6 +31,15 @@ struct Thresholds {
     const float *on, *off;
 };
 
+// Refractory period (R26): t_last [E*H*W] = stamp of each pixel's last emitted event relative to
+// the start of the current interval (-inf: none yet), device, read and written by the resolve kernel; null = off.
+// With it on, the resolve kernel leaves EVENTS (not records) in the arrival buffer and order.cu copies them.
+struct Refractory {
+    float *t_last;
+    float tau_r;    // seconds, > 0
+    float T;        // keyframe period
+};
+
 struct DebugOut {  // all nullable; [S,E,H,W]
     uint32_t *win;
     uint8_t  *dir;
@@ -74,8 +83,10 @@ cudaError_t launch_global_splat(const Geom &g, const ZChunk &zc, const Keyframe 
                                 const SubstepTable &tab, cudaStream_t st);
 cudaError_t launch_global_resolve(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B,
                                   const SubstepTable &tab, float *l_ref, float *l_prev,
-                                  const EventParams &ep, const Thresholds &th, const EventSink &sink,
-                                  unsigned long long *holes, const DebugOut &dbg, cudaStream_t st);
+                                  const EventParams &ep, const Thresholds &th, const Refractory &rf,
+                                  const EventSink &sink, unsigned long long *holes, const DebugOut &dbg, cudaStream_t st);
+// fill n floats with v (prep.cu)
+cudaError_t launch_fill(float *p, long long n, float v, cudaStream_t st);
 
 // ---- tile path (tile_path.cu): bounded motion, z-buffers in shared memory --------------------------
 struct TilePlan {

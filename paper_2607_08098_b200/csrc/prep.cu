@@ -120,4 +120,16 @@ cudaError_t launch_check_positive(const float *theta, long long n, unsigned long
     return cudaGetLastError();
 }
 
+__global__ void __launch_bounds__(256) k_fill(float *__restrict__ p, long long n, float v)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) p[i] = v;
+}
+
+cudaError_t launch_fill(float *p, long long n, float v, cudaStream_t st)
+{
+    const long long blocks = (n + 255) / 256;
+    k_fill<<<(unsigned)(blocks < 4096 ? (blocks < 1 ? 1 : blocks) : 4096), 256, 0, st>>>(p, n, v);
+    return cudaGetLastError();
+}
+
 }  // namespace evis

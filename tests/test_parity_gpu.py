@@ -269,6 +269,64 @@ def test_threshold_maps_api_contract():
     ev.destroy()
 
 
+@pytest.mark.parametrize("tau_r,with_maps", [(0.0005, False), (0.003, False), (0.02, True)])
+def test_refractory_period(tau_r, with_maps, monkeypatch):
+    """Refractory period (R26): emitted events, their binary32 stamps, L_ref and the carried t_last
+    state match the oracle over several intervals (tau_r below a substep, a few substeps, longer than a keyframe
+    interval), also combined with the threshold maps and with substep chunks (state carried through memory)."""
+    if with_maps:
+        monkeypatch.setenv("EVIS_ZBUF_MB", "1")
+    spec = scenes.small(scenes.config(4), num_envs=3, height=97, width=131, num_keyframes=5)
+    th = scenes.threshold_maps(spec, sigma=0.04, theta_min=0.02, device="cuda") if with_maps else None
+    rep = parity.run_parity(spec, 5, path=binding.PATH_GLOBAL, thresholds=th, tau_r=tau_r)
+    assert rep.ties == 0, "a threshold tie would cascade through t_last: pick another seed"
+    _assert_tolerances(rep)
+    rep0 = parity.run_parity(spec, 5, path=binding.PATH_GLOBAL, thresholds=th)
+    assert 0 < rep.events_oracle < rep0.events_oracle and rep.events_gpu == rep.events_oracle
+
+
+def test_refractory_api_contract():
+    """evis_set_refractory: negative or non-finite tau_r is INVALID_ARG; tau_r = 0 restores the plain stream; the
+    tile path refuses it."""
+    spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=3)
+    E, H, W = spec.num_envs, spec.height, spec.width
+    sc = scenes.make_scene(spec)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(3)]
+
+    def run(setup, path=binding.PATH_GLOBAL):
+        ev = binding.Evis(E, H, W, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                          max_motion_px=spec.max_motion_px(), path=path, event_capacity=1 << 22)
+        setup(ev)
+        out = []
+        for kf in kfs:
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+            out.append(ev.read_events().copy())
+        ev.destroy()
+        return np.concatenate(out)
+
+    base = run(lambda ev: None)
+
+    def bad(ev):
+        for v in (-1.0, float("nan"), float("inf")):
+            with pytest.raises(binding.EvisError) as ei:
+                ev.set_refractory(v)
+            assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+    assert np.array_equal(base, run(bad))
+
+    def on_off(ev):
+        ev.set_refractory(0.01)
+        ev.set_refractory(0.0)
+    assert np.array_equal(base, run(on_off))
+    sup = run(lambda ev: ev.set_refractory(0.004))
+    assert 0 < len(sup) < len(base)
+
+    def tile(ev):
+        with pytest.raises(binding.EvisError) as ei:
+            ev.set_refractory(0.01)
+        assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    run(tile, path=binding.PATH_TILE)
+
+
 def _run_stream(spec, n_kf, path, seed_offset=0):
     sc = scenes.make_scene(spec)
     ev = binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg,
