@@ -43,6 +43,18 @@ def test_config1_full(path):
     _assert_tolerances(rep)
 
 
+@pytest.mark.parametrize("cfg,envs", [(2, [0, 8, 15]), (3, [0, 63]), (4, [0, 127, 255])])
+def test_full_size_configs_sampled_envs(cfg, envs):
+    """BASELINE configs 2, 3 and 4 at FULL size, in the launch configuration bench.py times (PATH_AUTO, default
+    regions and streams): the GPU runs the whole batch, the oracle the sampled envs (first, middle, last) -- envs
+    are independent, so an env's events are outputs the oracle can compute one by one.  Events, L_ref, L_prev and
+    timestamps of those envs must match as in the reduced cases."""
+    spec = scenes.small(scenes.config(cfg), num_keyframes=3)
+    cap = int(min(0x7FFFFFFF, 10 * spec.num_envs * spec.height * spec.width))
+    rep = parity.run_parity(spec, 3, envs=envs, path=binding.PATH_AUTO, debug=False, capacity=cap)
+    _assert_tolerances(rep)
+
+
 @pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("use_fwd", [True, False])
 def test_config2_reduced(path, use_fwd):
