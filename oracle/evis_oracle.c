@@ -233,8 +233,10 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
 /* ---- one keyframe interval of one env: A -> B, substeps i = 1..S ------------------------------
  * i < S are the paper's K-1 intermediates (f = i/K); i = S is keyframe B itself [R10].
  * fwdA: displacement of A's pixels towards B: -m_A or the explicit forward field.
- * Optional debug outputs, each [S][H*W] or NULL: winners of each direction, composite, Lhat.     */
-int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, float c_pos, float c_neg,
+ * Optional debug outputs, each [S][H*W] or NULL: winners of each direction, composite, Lhat.
+ * margin: H x W is the OVER-RENDERED frame (Supp. B 317-319); the warp runs on all of it and the
+ * caller crops `margin` pixels off each side afterwards (evis_oracle.py); here it only restricts the hole count. */
+int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, int margin, float T, float c_pos, float c_neg,
                      const float *th_on, const float *th_off,              /* [H*W] or NULL: Eq. 8 maps of this env */
                      float tau_r, float *t_last,                           /* refractory period (<= 0: off), state [H*W] */
                      const float *LA, const float *fwdA, const float *ZA,
@@ -258,7 +260,11 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, float T, fl
             if (dbg_winA) dbg_winA[(int64_t)(i - 1) * P + q] = zA[q] == EVO_EMPTY ? EVO_NONE : (uint32_t)zA[q];
             if (dbg_winB) dbg_winB[(int64_t)(i - 1) * P + q] = zB[q] == EVO_EMPTY ? EVO_NONE : (uint32_t)zB[q];
             if (dbg_Lhat) dbg_Lhat[(int64_t)(i - 1) * P + q] = Lhat[q];
-            if (holes && zA[q] == EVO_EMPTY && zB[q] == EVO_EMPTY) ++*holes;
+            if (holes && zA[q] == EVO_EMPTY && zB[q] == EVO_EMPTY) {
+                /* over-render margin [R27]: only the pixels kept by the crop count */
+                const int qx = (int)(q % W), qy = (int)(q / W);
+                if (qx >= margin && qx < W - margin && qy >= margin && qy < H - margin) ++*holes;
+            }
         }
         made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, th_on, th_off, tau_r, t_last, Lhat, Lref, Lprev,
                                 ev, cap, n_have + made, dbg_dL ? dbg_dL + (int64_t)(i - 1) * P : 0);

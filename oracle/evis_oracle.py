@@ -36,7 +36,7 @@ def lib():
         L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [fp, fp, fp, C.c_void_p,
                                                                         C.c_int64, C.c_int64, fp]
         L.evo_event_frame.restype = C.c_int64
-        L.evo_interval.argtypes = ([C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [fp] * 8 + [u64p, u64p, fp]
+        L.evo_interval.argtypes = ([C.c_int] * 7 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [fp] * 8 + [u64p, u64p, fp]
                                    + [C.c_void_p, C.c_int64, C.c_int64]
                                    + [u32p, u32p, u8p, u32p, fp, fp, C.POINTER(C.c_int64)])
         L.evo_interval.restype = C.c_int64
@@ -110,7 +110,7 @@ class Oracle:
     def __init__(self, num_envs: int, height: int, width: int, substeps: int, c_pos: float, c_neg: float,
                  log_eps: float, keyframe_dt: float, composite_mode: int = 0, debug: bool = False,
                  theta_on: Optional[np.ndarray] = None, theta_off: Optional[np.ndarray] = None,
-                 tau_r: float = 0.0):
+                 tau_r: float = 0.0, margin: int = 0):
         self.E, self.H, self.W, self.S = num_envs, height, width, substeps
         self.c_pos, self.c_neg, self.eps, self.T = c_pos, c_neg, log_eps, keyframe_dt
         self.mode = composite_mode
@@ -120,6 +120,11 @@ class Oracle:
         self.th_off = None if theta_off is None else np.ascontiguousarray(theta_off, np.float32).reshape(num_envs, height, width)
         self.debug = debug
         # refractory period: stamps of the last emitted events, relative to the current interval
+        # over-render margin (Supp. B): height x width is the over-rendered frame; the warp runs on
+        # all of it, then `margin` pixels are cropped off each side: events outside the crop are dropped and the
+        # others are reported in the cropped frame's coordinates [R27]
+        self.margin = int(margin)
+        assert 0 <= 2 * self.margin < min(height, width)
         self.tau_r = float(tau_r)
         self.t_last = np.full((num_envs, height, width), -np.inf, np.float32)
         self.calls = 0
@@ -169,7 +174,7 @@ class Oracle:
             for e in range(E):
                 d = self.dbg
                 n += lib().evo_interval(
-                    H, W, S, self.mode, e, kf, float(self.T), float(self.c_pos), float(self.c_neg),
+                    H, W, S, self.mode, e, kf, self.margin, float(self.T), float(self.c_pos), float(self.c_neg),
                     _f(self.th_on[e]) if self.th_on is not None else None,
                     _f(self.th_off[e]) if self.th_off is not None else None,
                     self.tau_r, _f(t_last[e]),
@@ -186,4 +191,11 @@ class Oracle:
         self.holes = holes.value
         self.prev = cur
         self.calls += 1
-        return ev[:n]
+        ev = ev[:n]
+        if self.margin:
+            M = self.margin
+            keep = (ev["x"] >= M) & (ev["x"] < W - M) & (ev["y"] >= M) & (ev["y"] < H - M)
+            ev = ev[keep].copy()
+            ev["x"] -= M
+            ev["y"] -= M
+        return ev

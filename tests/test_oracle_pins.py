@@ -526,3 +526,51 @@ def test_p12c_refractory_across_intervals_in_the_full_oracle():
         last[p] = t
     for (y, x), t in last.items():                                # carried state = last stamp relative to the NEXT interval
         assert abs(float(o_ref.t_last[0, y, x]) - (t - 3 * T)) < 1e-6
+
+
+# ---- P13: over-render margin and crop (Supp. B 317-319) [R27] ------------------------------------
+def test_p13_margin_removes_the_border_artifacts_of_a_translation():
+    """A textured plane translating by D = S d per keyframe (integer d, S a power of two).  On the plain frame the
+    strip that enters the field of view is seen by neither keyframe at some substeps (holes, held values); with a
+    margin >= |D| rendered around it and cropped after the warp, the events of the cropped frame are exactly those
+    of the ANALYTIC frame sequence L(t_i) fed to the event stage (which has its own pins), at the cropped
+    coordinates, and no hole is left inside the crop."""
+    H, W, S, dx, dy, M = 14, 18, 4, 2, -1, 8            # |D| = (8, 4) <= M
+    He, We = H + 2 * M, W + 2 * M
+    r = _rng(13)
+    big = r.uniform(-3, 3, size=(He + 96, We + 96)).astype(np.float32)
+    yse, xse = np.mgrid[0:He, 0:We]
+    tex_e = lambda px, py: big[yse - py + 48, xse - px + 48]          # extended frame, surface moved by (px, py)
+    crop = lambda a: a[..., M:M + H, M:M + W]
+    C = 0.25
+
+    def run(margin):
+        h, w = (He, We) if margin else (H, W)
+        o = orc.Oracle(1, h, w, S, C, C, 1e-3, 1.0, debug=True, margin=margin)
+        mv = np.empty((1, h, w, 2), np.float32)
+        mv[..., 0], mv[..., 1] = -S * dx, -S * dy
+        depth = np.full((1, h, w), 3.0, np.float32)
+        evs = []
+        for k in range(3):
+            L = tex_e(k * S * dx, k * S * dy)
+            L = L if margin else crop(L)
+            evs.append(o.step(_rad_from_L(L)[None], mv, depth))
+        return o, np.concatenate(evs)
+
+    o_m, ev_m = run(M)
+    o_0, ev_0 = run(0)
+    assert o_m.holes == 0 and o_0.holes > 0
+    # analytic sequence of the cropped frame: keyframes through the oracle's own log (same rounding), substeps exact
+    L0 = orc.log_luminance(_rad_from_L(tex_e(0, 0))[None], 1e-3)[0]
+    Lk = lambda k, i: crop(orc.log_luminance(_rad_from_L(tex_e((k * S + i) * dx, (k * S + i) * dy))[None], 1e-3)[0])
+    lref, lprev, want = crop(L0).copy(), crop(L0).copy(), []
+    for k in range(2):
+        frames = np.stack([Lk(k, i) for i in range(1, S + 1)])
+        e, lref = orc.event_frames(frames, lprev, C, C, 1.0, Lref0=lref)
+        lprev = frames[-1]
+        want += [(k, int(v["substep"]), int(v["y"]), int(v["x"]), int(v["p"])) for v in e]
+    got = [(int(v["kf"]), int(v["substep"]), int(v["y"]), int(v["x"]), int(v["p"])) for v in ev_m]
+    assert sorted(got) == sorted(want) and len(got) > 0
+    assert all(0 <= y < H and 0 <= x < W for (_, _, y, x, _) in got)
+    got0 = [(int(v["kf"]), int(v["substep"]), int(v["y"]), int(v["x"]), int(v["p"])) for v in ev_0]
+    assert sorted(got0) != sorted(want)                     # the plain frame does show the border artifact
