@@ -140,6 +140,14 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
  * stay in force), BAD_STATE (tile path), CUDA, OOM. */
 int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta_off, int src_is_device);
 
+/* Over-render margin (Supp. B 317-319; R27): the frames handed to evis_step (height x
+ * width of the configuration) were rendered with `margin` extra pixels on each side.  The warp uses all of them;
+ * the margin is cropped off afterwards: the event model runs and events exist only for the inner
+ * (height - 2 margin) x (width - 2 margin) pixels, x and y of an event are relative to that cropped frame, holes are
+ * counted inside it.  0 = no margin (default).  Applies from the next evis_step on; synchronises.  Global path only.
+ * Errors: INVALID_ARG (negative, or 2 margin >= min(height, width)), BAD_STATE (tile path), CUDA. */
+int evis_set_margin(evis_ctx *ctx, int margin);
+
 /* Refractory period (R26): with tau_r > 0 (seconds) a threshold crossing of a pixel is
  * emitted only if its timestamp t satisfies t - t_last >= tau_r, t_last being the timestamp of the pixel's last
  * EMITTED event (none before the call: every pixel starts free); suppressed crossings still move L_ref (Eq. 4 is

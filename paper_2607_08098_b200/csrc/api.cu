@@ -497,7 +497,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
             const uint32_t tx = (g.W + G_TILE_W - 1) / G_TILE_W, ty = (g.H + G_TILE_H - 1) / G_TILE_H;
             CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
                              ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, ctx->ep, th, (uint32_t)g.W,
-                             (uint32_t)g.HW, tx, tx * ty, (uint32_t)g.S, st));
+                             (uint32_t)g.HW, (uint32_t)g.margin, tx, tx * ty, (uint32_t)g.S, st));
         } else {
             CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
                             ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, st));
@@ -556,6 +556,18 @@ int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta
     ctx->th_on = on; ctx->th_off = off;
     ctx->th_active = true;
     ctx->launches += 2;
+    return EVIS_OK;
+}
+
+int evis_set_margin(evis_ctx *ctx, int margin)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    if (margin < 0 || 2 * (long long)margin >= (ctx->g.H < ctx->g.W ? ctx->g.H : ctx->g.W)) return EVIS_ERR_INVALID_ARG;
+    if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    ctx->g.margin = margin;
     return EVIS_OK;
 }
 

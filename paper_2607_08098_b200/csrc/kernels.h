@@ -23,6 +23,8 @@ struct Geom {
                    // the pixel plane zd that is target pixel (x0, y0) (row 0 / column 0 are a guard band for
                    // coordinate -1, never read), in the cell plane zc it is the class-11 cell (x0+1, y0+1)
     int mode;      // EVIS_COMPOSITE_*
+    int margin;    // over-render margin (R27): H x W is the over-rendered frame; events exist only for
+                   // pixels at least `margin` away from every side and carry coordinates relative to that crop
 };
 
 // Eq. 8: per-pixel ON / OFF thresholds [E*H*W], device; both null = the scalar C+ / C- of
@@ -120,7 +122,7 @@ cudaError_t launch_order(const EventSink &sink, uint32_t num_entries, unsigned l
 cudaError_t launch_expand(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out, uint4 *ordered,
                           unsigned long long capacity, const unsigned long long *step_events,
                           unsigned long long *total_events, const EventParams &ep, const Thresholds &th, uint32_t W,
-                          uint32_t HW, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st);
+                          uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st);
 // number of values among theta[0..n) that are not (finite and > 0), added to *bad (prep.cu)
 cudaError_t launch_check_positive(const float *theta, long long n, unsigned long long *bad, cudaStream_t st);
 

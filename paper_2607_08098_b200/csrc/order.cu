@@ -138,8 +138,8 @@ k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *
 __global__ void __launch_bounds__(ORD_NT)
 k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__restrict__ bsum,
          const uint4 *__restrict__ arrival, unsigned long long arrival_cap, uint4 *__restrict__ ordered,
-         unsigned long long cap, const EventParams ep, const Thresholds th, uint32_t W, uint32_t HW, uint32_t tiles_x,
-         uint32_t tiles, uint32_t S)
+         unsigned long long cap, const EventParams ep, const Thresholds th, uint32_t W, uint32_t HW, uint32_t margin,
+         uint32_t tiles_x, uint32_t tiles, uint32_t S)
 {
     constexpr unsigned FULL = 0xFFFFFFFFu;
     __shared__ unsigned long long s_w[33];
@@ -209,6 +209,7 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
                     const size_t pix = (size_t)env * HW + (size_t)(xy >> 16) * W + (xy & 0xFFFFu);
                     pc = up ? __ldg(th.on + pix) : -__ldg(th.off + pix);
                 }
+                const uint32_t xyc = xy - (margin | (margin << 16));         // coordinates in the cropped frame (R27)
                 const uint32_t w1 = env | ((up ? 0x01u : 0xFFu) << 16) | (sub << 24);
                 // fr_k = (L_ref + k p C - L_prev) / (L_hat - L_prev), clamped to [0, 1]; 1 when the denominator is 0.
                 // Timestamps decide nothing (compared within 1e-7 s; a substep is ~1e-3 s): reciprocal once per record.
@@ -220,7 +221,7 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
                     kf += 1.0f;
                     float fr = __fmul_rn(__fsub_rn(__fmaf_rn(kf, pc, l_ref), l_prev), rden);
                     fr = flat ? 1.0f : fminf(fmaxf(fr, 0.0f), 1.0f);
-                    if (o < cap) ordered[o] = make_uint4(xy, w1, __float_as_uint(__fmaf_rn(fr, ep.dt, t0)), ep.kf);
+                    if (o < cap) ordered[o] = make_uint4(xyc, w1, __float_as_uint(__fmaf_rn(fr, ep.dt, t0)), ep.kf);
                 }
             }
         }
@@ -230,13 +231,13 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
 cudaError_t launch_expand(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
                           unsigned long long capacity, const unsigned long long *step_events,
                           unsigned long long *total_events, const EventParams &ep, const Thresholds &th, uint32_t W,
-                          uint32_t HW, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st)
+                          uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st)
 {
     const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
     k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, DIR_EV_SHIFT);
     k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events);
     k_expand<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, sink.arrival_cap, ordered, capacity, ep, th,
-                                    W, HW, tiles_x, tiles, S);
+                                    W, HW, margin, tiles_x, tiles, S);
     return cudaGetLastError();
 }
 

@@ -61,7 +61,7 @@ def _counts(ev, E, S, H, W, env_map=None):
 
 def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int, S: int, H: int, W: int,
                  c_pos: float, c_neg: float, rep: ParityReport, kf: int,
-                 gpu_dbg=None, env_sel: Optional[Sequence[int]] = None, thresholds=None) -> None:
+                 gpu_dbg=None, env_sel: Optional[Sequence[int]] = None, thresholds=None, margin: int = 0) -> None:
     """Compare one step.  ``env_sel``: the oracle ran only these envs of the GPU batch (oracle env j =
     GPU env env_sel[j]); GPU events of other envs are ignored."""
     if env_sel is not None:
@@ -71,6 +71,9 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
         gpu_ev = gpu_ev[keep].copy()
         gpu_ev["env"] = env_map[gpu_ev["env"].astype(np.int64)].astype(np.uint16)
     Eo = E if env_sel is None else len(env_sel)
+    M = margin                                     # H, W: the over-rendered frame; events live in the crop (R27)
+    Hc, Wc = H - 2 * M, W - 2 * M
+    inner = (Ellipsis, slice(M, H - M), slice(M, W - M))
     assert np.all(gpu_ev["kf"] == kf)
     rep.steps += 1
     rep.events_gpu += len(gpu_ev)
@@ -81,17 +84,18 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
         win, d, lh = gpu_dbg                       # [S,E,H,W]
         if env_sel is not None:
             win, d, lh = win[:, env_sel], d[:, env_sel], lh[:, env_sel]
-        o_dir = np.transpose(ora.dbg["dir"], (1, 0, 2, 3))
-        o_idx = np.transpose(ora.dbg["idx"], (1, 0, 2, 3))
-        o_lh = np.transpose(ora.dbg["Lhat"], (1, 0, 2, 3))
+        o_dir = np.transpose(ora.dbg["dir"], (1, 0, 2, 3))[inner]
+        o_idx = np.transpose(ora.dbg["idx"], (1, 0, 2, 3))[inner]
+        o_lh = np.transpose(ora.dbg["Lhat"], (1, 0, 2, 3))[inner]
+        win, d, lh = win[inner], d[inner], lh[inner]
         bad = (d != o_dir) | (win != o_idx)
         rep.winner_mismatch += int(bad.sum())
         rep.max_dL = max(rep.max_dL, float(np.max(np.abs(lh.astype(np.float64) - o_lh))))
         rep.holes += int((o_dir == 3).sum())
 
     # --- events: multiset per (env, substep, y, x, polarity) -----------------------------------
-    cg = _counts(gpu_ev, Eo, S, H, W)
-    co = _counts(ora_ev, Eo, S, H, W)
+    cg = _counts(gpu_ev, Eo, S, Hc, Wc)
+    co = _counts(ora_ev, Eo, S, Hc, Wc)
     diff = np.argwhere(cg != co)
     if len(diff):
         # a disagreement is legitimate only at a threshold tie (R5): ||dL| - k C| < 1e-5.  It may
@@ -102,10 +106,10 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
             if (e, y, x) in seen:
                 continue
             seen.add((e, y, x))
-            dL = float(ora.dbg["dL"][e, s, y, x])
+            dL = float(ora.dbg["dL"][e, s, y + M, x + M])
             C = c_pos if dL > 0 else c_neg
             if thresholds is not None:              # Eq. 8: the pixel's own thresholds, [Eo,H,W] numpy
-                C = float((thresholds[0] if dL > 0 else thresholds[1])[e, y, x])
+                C = float((thresholds[0] if dL > 0 else thresholds[1])[e, y + M, x + M])
             k = round(abs(dL) / C)
             assert abs(abs(dL) - k * C) < TOL_TIE, \
                 f"event mismatch not at a tie: env {e} substep {s + 1} ({x},{y}) dL={dL} gpu={cg[e, s, y, x]} oracle={co[e, s, y, x]}"
@@ -125,7 +129,7 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
 def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Sequence[int]] = None,
                mode: int = 0, path: int = binding.PATH_GLOBAL, use_fwd: bool = True, debug: bool = True,
                capacity: int = 1 << 24, max_motion: Optional[float] = None, thresholds=None,
-               tau_r: float = 0.0) -> ParityReport:
+               tau_r: float = 0.0, margin: int = 0) -> ParityReport:
     """GPU runs the whole batch; the oracle runs ``envs`` (default: all).  Returns the report after
     asserting every bit-exact criterion; tolerances are asserted by the caller on the report."""
     sc = scenes.make_scene(spec)
@@ -140,9 +144,12 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
         th_np = (thresholds[0][sel].cpu().numpy(), thresholds[1][sel].cpu().numpy())
     if tau_r > 0.0:                                 # refractory period
         ev.set_refractory(tau_r)
+    if margin:                                      # over-render margin: spec = the over-rendered frame
+        ev.set_margin(margin)
+    inner = (Ellipsis, slice(margin, H - margin), slice(margin, W - margin))
     ora = orc.Oracle(len(sel), H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
                      composite_mode=mode, debug=True, theta_on=None if th_np is None else th_np[0],
-                     theta_off=None if th_np is None else th_np[1], tau_r=tau_r)
+                     theta_off=None if th_np is None else th_np[1], tau_r=tau_r, margin=margin)
     rep = ParityReport()
     try:
         for k in range(n_keyframes):
@@ -158,11 +165,11 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
             assert len(ge) == n
             dbg = ev.debug_read() if debug else None
             compare_step(ge, oe, ora, E, S, H, W, spec.c_pos, spec.c_neg, rep, k - 1, dbg,
-                         None if envs is None else sel, th_np)
+                         None if envs is None else sel, th_np, margin)
             lref, lprev = ev.get_state()
             if rep.ties == 0:
-                assert np.array_equal(lref[sel], ora.Lref), "carried L_ref differs"
-            assert np.allclose(lprev[sel], ora.Lprev, atol=TOL_L, rtol=0)
+                assert np.array_equal(lref[sel][inner], ora.Lref[inner]), "carried L_ref differs"
+            assert np.allclose(lprev[sel][inner], ora.Lprev[inner], atol=TOL_L, rtol=0)
             info = ev.info()
             if envs is None:
                 assert info.last_holes == ora.holes

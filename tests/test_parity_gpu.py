@@ -297,6 +297,69 @@ def test_refractory_period(tau_r, with_maps, monkeypatch):
     assert 0 < rep.events_oracle < rep0.events_oracle and rep.events_gpu == rep.events_oracle
 
 
+@pytest.mark.parametrize("margin,extra", [(20, False), (7, True)])
+def test_over_render_margin(margin, extra, monkeypatch):
+    """Over-render margin (Supp. B; R27): the frames carry `margin` extra pixels per side, the warp
+    uses them, events exist only inside the crop, with cropped coordinates; holes are counted inside the crop.
+    Config 4 recipe (ego-motion up to ~18 px per keyframe: the border is where the artifacts are).  Second case:
+    together with threshold maps, a refractory period and substep chunks."""
+    spec = scenes.small(scenes.config(4), num_envs=3, height=110 + 2 * margin, width=150 + 2 * margin, num_keyframes=4)
+    th, tau = None, 0.0
+    if extra:
+        monkeypatch.setenv("EVIS_ZBUF_MB", "1")
+        th = scenes.threshold_maps(spec, sigma=0.04, theta_min=0.02, device="cuda")
+        tau = 0.002
+    rep = parity.run_parity(spec, 4, path=binding.PATH_GLOBAL, margin=margin, thresholds=th, tau_r=tau)
+    _assert_tolerances(rep)
+
+
+def test_margin_api_contract():
+    """evis_set_margin: negative or too large margins are INVALID_ARG; margin 0 is the plain frame; coordinates
+    of a margin run stay inside the cropped frame; the tile path refuses it."""
+    spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=3)
+    E, H, W = spec.num_envs, spec.height, spec.width
+    sc = scenes.make_scene(spec)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(3)]
+
+    def run(setup, path=binding.PATH_GLOBAL):
+        ev = binding.Evis(E, H, W, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                          max_motion_px=spec.max_motion_px(), path=path, event_capacity=1 << 22)
+        setup(ev)
+        out = []
+        for kf in kfs:
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+            out.append(ev.read_events().copy())
+        ev.destroy()
+        return np.concatenate(out)
+
+    base = run(lambda ev: None)
+
+    def bad(ev):
+        for m in (-1, 33, 1000):                   # 2 * 33 >= 65
+            with pytest.raises(binding.EvisError) as ei:
+                ev.set_margin(m)
+            assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+        ev.set_margin(5)
+        ev.set_margin(0)
+    assert np.array_equal(base, run(bad))
+    crop = run(lambda ev: ev.set_margin(10))
+    assert 0 < len(crop) < len(base)
+    assert crop["x"].max() < W - 20 and crop["y"].max() < H - 20
+    # the cropped stream is the plain one restricted to the crop and shifted (pixels are independent)
+    keep = (base["x"] >= 10) & (base["x"] < W - 10) & (base["y"] >= 10) & (base["y"] < H - 10)
+    ref = base[keep].copy()
+    ref["x"] -= 10
+    ref["y"] -= 10
+    key = lambda a: np.sort(a, order=["kf", "env", "substep", "y", "x", "t_off"])
+    assert np.array_equal(key(ref), key(crop))
+
+    def tile(ev):
+        with pytest.raises(binding.EvisError) as ei:
+            ev.set_margin(4)
+        assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    run(tile, path=binding.PATH_TILE)
+
+
 def test_refractory_api_contract():
     """evis_set_refractory: negative or non-finite tau_r is INVALID_ARG; tau_r = 0 restores the plain stream; the
     tile path refuses it."""
