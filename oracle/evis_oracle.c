@@ -48,6 +48,18 @@ static uint32_t f32_bits(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
 /* ---- Eq. 3 + log -----------------------------------------------------------
  * I = 0.2126 R + 0.7152 G + 0.0722 B ;  L = log(I + eps), natural log [R1], I clamped at 0 [R3].
  * binary64, products and sums each rounded (no fma), summed left to right, one rounding to f32. */
+/* Colour events: "Replacing I with individual R, G, B channels and applying the event model to each
+ * independently produces color events."  channel = 0, 1, 2: I = that channel of the radiance, same clamp, same
+ * log; everything downstream is unchanged, one independent run per channel [R28].                              */
+void evo_log_channel(const float *rad /* [n][3] */, int64_t n, float eps, int channel, float *L /* [n] */)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        double I = (double)rad[3 * i + channel];
+        if (!(I > 0.0)) I = 0.0;
+        L[i] = (float)log(I + (double)eps);
+    }
+}
+
 void evo_log_luminance(const float *rad /* [n][3] */, int64_t n, float eps, float *L /* [n] */)
 {
     for (int64_t i = 0; i < n; ++i) {

@@ -29,6 +29,8 @@ def lib():
                                C.POINTER(C.c_uint8))
         L.evo_log_luminance.argtypes = [fp, C.c_int64, C.c_float, fp]
         L.evo_log_luminance.restype = None
+        L.evo_log_channel.argtypes = [fp, C.c_int64, C.c_float, C.c_int, fp]
+        L.evo_log_channel.restype = None
         L.evo_splat.argtypes = [C.c_int] * 5 + [fp, fp, fp, u64p]
         L.evo_splat.restype = None
         L.evo_composite.argtypes = [C.c_int] * 5 + [u64p, u64p, fp, fp, fp, fp, u8p, u32p]
@@ -53,11 +55,16 @@ def _p(a, t):
     return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
 
 
-def log_luminance(rad: np.ndarray, eps: float) -> np.ndarray:
-    """Eq. 3 + log (PAPER.md:94-99).  rad [...,3] float32 -> L [...] float32."""
+def log_luminance(rad: np.ndarray, eps: float, channel: Optional[int] = None) -> np.ndarray:
+    """Eq. 3 + log (PAPER.md:94-99).  rad [...,3] float32 -> L [...] float32.
+    channel = 0 / 1 / 2: colour events: the log of that channel instead of the luminance."""
     rad = np.ascontiguousarray(rad, dtype=np.float32)
     out = np.empty(rad.shape[:-1], dtype=np.float32)
-    lib().evo_log_luminance(_f(rad), out.size, float(eps), _f(out))
+    if channel is None:
+        lib().evo_log_luminance(_f(rad), out.size, float(eps), _f(out))
+    else:
+        assert channel in (0, 1, 2)
+        lib().evo_log_channel(_f(rad), out.size, float(eps), int(channel), _f(out))
     return out
 
 
@@ -110,7 +117,7 @@ class Oracle:
     def __init__(self, num_envs: int, height: int, width: int, substeps: int, c_pos: float, c_neg: float,
                  log_eps: float, keyframe_dt: float, composite_mode: int = 0, debug: bool = False,
                  theta_on: Optional[np.ndarray] = None, theta_off: Optional[np.ndarray] = None,
-                 tau_r: float = 0.0, margin: int = 0):
+                 tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None):
         self.E, self.H, self.W, self.S = num_envs, height, width, substeps
         self.c_pos, self.c_neg, self.eps, self.T = c_pos, c_neg, log_eps, keyframe_dt
         self.mode = composite_mode
@@ -123,6 +130,7 @@ class Oracle:
         # over-render margin (Supp. B): height x width is the over-rendered frame; the warp runs on
         # all of it, then `margin` pixels are cropped off each side: events outside the crop are dropped and the
         # others are reported in the cropped frame's coordinates [R27]
+        self.channel = channel                     # colour events: None = luminance, 0/1/2 = R/G/B
         self.margin = int(margin)
         assert 0 <= 2 * self.margin < min(height, width)
         self.tau_r = float(tau_r)
@@ -143,7 +151,7 @@ class Oracle:
         rad = np.ascontiguousarray(rad, np.float32).reshape(E, H, W, 3)
         mB = np.ascontiguousarray(mv_bwd, np.float32).reshape(E, H, W, 2)
         ZB = np.ascontiguousarray(depth, np.float32).reshape(E, H, W)
-        LB = log_luminance(rad, self.eps)
+        LB = log_luminance(rad, self.eps, self.channel)
         fwd = -mB if mv_fwd is None else np.ascontiguousarray(mv_fwd, np.float32).reshape(E, H, W, 2)
         fwd = np.ascontiguousarray(fwd)
         cur = dict(L=LB, m=mB, Z=ZB, fwd=fwd)

@@ -574,3 +574,40 @@ def test_p13_margin_removes_the_border_artifacts_of_a_translation():
     assert all(0 <= y < H and 0 <= x < W for (_, _, y, x, _) in got)
     got0 = [(int(v["kf"]), int(v["substep"]), int(v["y"]), int(v["x"]), int(v["p"])) for v in ev_0]
     assert sorted(got0) != sorted(want)                     # the plain frame does show the border artifact
+
+
+# ---- P14: colour events [R28] ---------------------------------------------------------------------
+def test_p14_channel_log_is_the_log_of_that_channel_alone():
+    """"Replacing I with individual R, G, B channels": L = log(channel + eps) by math.log in double, rounded once
+    to binary32; the other two channels do not matter (they hold absurd values), negative values clamp to 0."""
+    r = _rng(14)
+    n, eps = 200, 1e-3
+    for ch in (0, 1, 2):
+        rad = r.uniform(-1e6, 1e6, size=(n, 3)).astype(np.float32)
+        rad[:, ch] = np.exp(r.uniform(-7, 7, size=n)).astype(np.float32)
+        rad[:5, ch] = [-1.0, 0.0, 1e-30, 1.0, 1e6]
+        L = orc.log_luminance(rad, eps, channel=ch)
+        for i in range(n):
+            c = max(float(rad[i, ch]), 0.0)
+            assert L[i] == np.float32(math.log(c + float(np.float32(eps))))
+    # a grey pixel has the same log in every channel, and its luminance log is within rounding of it
+    g = np.full((1, 3), 0.37, np.float32)
+    Ls = [float(orc.log_luminance(g, eps, channel=c)[0]) for c in (0, 1, 2)]
+    assert Ls[0] == Ls[1] == Ls[2] and abs(Ls[0] - float(orc.log_luminance(g, eps)[0])) < 1e-6
+
+
+def test_p14b_colour_events_are_three_independent_runs():
+    """A scene whose RED channel alone changes between keyframes: the R run fires, the G and B runs stay silent,
+    and the R run equals the luminance run of the grey image made of that channel (same warp, same Eq. 4)."""
+    E, H, W, S, T, C = 1, 4, 5, 4, 1.0 / 60.0, 0.2
+    r = _rng(15)
+    base = np.exp(r.uniform(-1, 1, size=(E, H, W, 3))).astype(np.float32)
+    nxt = base.copy()
+    nxt[..., 0] *= np.float32(3.0)
+    mv, z = np.zeros((E, H, W, 2), np.float32), np.ones((E, H, W), np.float32)
+    n_ev = []
+    for ch in (0, 1, 2):
+        o = orc.Oracle(E, H, W, S, C, C, 1e-3, T, channel=ch)
+        o.step(base, mv, z)
+        n_ev.append(len(o.step(nxt, mv, z)))
+    assert n_ev[0] == H * W * math.floor(math.log(3.0) / C) and n_ev[1] == n_ev[2] == 0
