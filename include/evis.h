@@ -140,6 +140,13 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
  * stay in force), BAD_STATE (tile path), CUDA, OOM. */
 int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta_off, int src_is_device);
 
+/* Colour events ("Replacing I with individual R, G, B channels and applying the event model to each
+ * independently produces color events"; R28): channel = 0, 1 or 2 makes this context take
+ * L = log(channel + eps) of the radiance's R, G or B instead of the Rec.709 luminance; -1 = luminance (default).
+ * A colour sensor is three contexts fed the same keyframes, one per channel.  Applies to the keyframes given to
+ * later evis_step calls: set it before the first one.  Both paths.  Errors: INVALID_ARG. */
+int evis_set_channel(evis_ctx *ctx, int channel);
+
 /* Over-render margin (Supp. B 317-319; R27): the frames handed to evis_step (height x
  * width of the configuration) were rendered with `margin` extra pixels on each side.  The warp uses all of them;
  * the margin is cropped off afterwards: the event model runs and events exist only for the inner

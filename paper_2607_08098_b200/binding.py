@@ -53,7 +53,7 @@ class evis_profile(C.Structure):
 # every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
-           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin"]
+           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel"]
 
 _lib = None
 
@@ -85,6 +85,7 @@ def load() -> C.CDLL:
     L.evis_set_thresholds.argtypes = [vp, vp, vp, C.c_int]
     L.evis_set_refractory.argtypes = [vp, C.c_float]
     L.evis_set_margin.argtypes = [vp, C.c_int]
+    L.evis_set_channel.argtypes = [vp, C.c_int]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
     for name in SYMBOLS:
@@ -166,6 +167,10 @@ class Evis:
         p_on, p_off = _dev_ptr(theta_on, (E, H, W), "theta_on"), _dev_ptr(theta_off, (E, H, W), "theta_off")
         torch.cuda.synchronize(self.device)                 # the library copies on its own stream
         _check(self._lib.evis_set_thresholds(self._ctx, p_on, p_off, 1), "evis_set_thresholds")
+
+    def set_channel(self, channel: int) -> None:
+        """evis_set_channel (colour events): 0 / 1 / 2 = log of R / G / B, -1 = Rec.709 luminance."""
+        _check(self._lib.evis_set_channel(self._ctx, int(channel)), "evis_set_channel")
 
     def set_margin(self, margin: int) -> None:
         """evis_set_margin: the frames carry `margin` over-rendered pixels per side, cropped after the warp."""

@@ -27,6 +27,7 @@ struct evis_ctx {
     float *l_ref, *l_prev;
     float *th_on, *th_off;            // Eq. 8 maps [E*H*W] (owned), in force when th_active
     bool th_active;
+    int channel; bool channel_set;    // colour events: log of one channel instead of the luminance
     float *t_last;                    // refractory state [E*H*W] (owned), in force when tau_r > 0
     float tau_r;
     SubstepTable *tab;                // device
@@ -408,7 +409,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     if (ctx->prof_on) { ctx->prof_acc.steps += 1; if (ctx->prof_spans.size() > 8192) prof_drain(ctx); }
     {
         Span sp(ctx, st, EVIS_STAGE_PREP, 1);
-        CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, B.L, B.mv, B.fwd, B.Z,
+        CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, ctx->channel_set ? ctx->channel : -1, B.L, B.mv, B.fwd, B.Z,
                        first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr,
                        ctx->path == EVIS_PATH_TILE ? ctx->cfg.max_motion_px : 0.0f, ctx->counters + C_MOTION, st));
     }
@@ -556,6 +557,14 @@ int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta
     ctx->th_on = on; ctx->th_off = off;
     ctx->th_active = true;
     ctx->launches += 2;
+    return EVIS_OK;
+}
+
+int evis_set_channel(evis_ctx *ctx, int channel)
+{
+    if (!ctx || channel < -1 || channel > 2) return EVIS_ERR_INVALID_ARG;
+    ctx->channel = channel;
+    ctx->channel_set = channel >= 0;
     return EVIS_OK;
 }
 

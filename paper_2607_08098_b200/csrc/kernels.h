@@ -49,8 +49,9 @@ struct DebugOut {  // all nullable; [S,E,H,W]
 };
 
 // a1 + a9 (prep.cu)
+// channel: -1 = Rec.709 luminance (Eq. 3), 0 / 1 / 2 = that channel alone (colour events)
 cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, const float *depth, long long n,
-                        float eps, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
+                        float eps, int channel, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
                         float *l_prev, float motion_bound /* 0 = unchecked */, unsigned long long *viol,
                         cudaStream_t st);
 

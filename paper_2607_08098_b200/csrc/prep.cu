@@ -14,10 +14,12 @@
 
 namespace evis {
 
-__device__ __forceinline__ float log_lum(float r, float g, float b, double eps)
+// channel < 0: Rec.709 luminance (Eq. 3); 0 / 1 / 2: that channel alone -- colour events (R28)
+__device__ __forceinline__ float log_lum(float r, float g, float b, double eps, int channel)
 {
     double I = __dadd_rn(__dadd_rn(__dmul_rn(0.2126, (double)r), __dmul_rn(0.7152, (double)g)),
                          __dmul_rn(0.0722, (double)b));
+    if (channel >= 0) I = (double)(channel == 0 ? r : (channel == 1 ? g : b));
     if (!(I > 0.0)) I = 0.0;
     return __double2float_rn(log(__dadd_rn(I, eps)));
 }
@@ -26,7 +28,7 @@ __device__ __forceinline__ float log_lum(float r, float g, float b, double eps)
 template <bool VEC>
 __global__ void __launch_bounds__(256)
 k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float *__restrict__ fwd_in,
-       const float *__restrict__ depth, long long n, float eps_f,
+       const float *__restrict__ depth, long long n, float eps_f, int channel,
        float *__restrict__ L, float2 *__restrict__ mv_out, float2 *__restrict__ fwd_out,
        float *__restrict__ Z, float *__restrict__ l_ref, float *__restrict__ l_prev, float bound,
        unsigned long long *__restrict__ viol)
@@ -40,10 +42,10 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
         const float4 *r4 = reinterpret_cast<const float4 *>(rad + 3 * p);
         const float4 a = __ldcs(r4), b = __ldcs(r4 + 1), c = __ldcs(r4 + 2);
         float4 l;
-        l.x = log_lum(a.x, a.y, a.z, eps);
-        l.y = log_lum(a.w, b.x, b.y, eps);
-        l.z = log_lum(b.z, b.w, c.x, eps);
-        l.w = log_lum(c.y, c.z, c.w, eps);
+        l.x = log_lum(a.x, a.y, a.z, eps, channel);
+        l.y = log_lum(a.w, b.x, b.y, eps, channel);
+        l.z = log_lum(b.z, b.w, c.x, eps, channel);
+        l.w = log_lum(c.y, c.z, c.w, eps, channel);
         *reinterpret_cast<float4 *>(L + p) = l;
         if (l_ref) {                                  // first keyframe: L_ref = L_prev = L   (R6)
             *reinterpret_cast<float4 *>(l_ref + p) = l;
@@ -68,7 +70,7 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
         *reinterpret_cast<float4 *>(Z + p) = __ldcs(reinterpret_cast<const float4 *>(depth + p));
     } else {
         if (t >= n) return;
-        const float l = log_lum(rad[3 * t], rad[3 * t + 1], rad[3 * t + 2], eps);
+        const float l = log_lum(rad[3 * t], rad[3 * t + 1], rad[3 * t + 2], eps, channel);
         L[t] = l;
         if (l_ref) { l_ref[t] = l; l_prev[t] = l; }
         mv_out[t] = make_float2(mv[2 * t], mv[2 * t + 1]);
@@ -85,17 +87,17 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
 static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, const float *depth, long long n,
-                        float eps, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
+                        float eps, int channel, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
                         float *l_prev, float bound, unsigned long long *viol, cudaStream_t st)
 {
     if (!(bound > 0.0f)) bound = __builtin_inff();      // no bound declared: nothing to check
     const bool vec = (n % 4 == 0) && aligned16(rad) && aligned16(mv) && aligned16(depth) && (!fwd || aligned16(fwd));
     if (vec) {
         const long long threads = n / 4;
-        k_prep<true><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, L, mv_out,
+        k_prep<true><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, channel, L, mv_out,
                                                                          fwd_out, Z, l_ref, l_prev, bound, viol);
     } else {
-        k_prep<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, L, mv_out,
+        k_prep<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, channel, L, mv_out,
                                                                     fwd_out, Z, l_ref, l_prev, bound, viol);
     }
     return cudaGetLastError();

@@ -129,7 +129,7 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
 def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Sequence[int]] = None,
                mode: int = 0, path: int = binding.PATH_GLOBAL, use_fwd: bool = True, debug: bool = True,
                capacity: int = 1 << 24, max_motion: Optional[float] = None, thresholds=None,
-               tau_r: float = 0.0, margin: int = 0) -> ParityReport:
+               tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None) -> ParityReport:
     """GPU runs the whole batch; the oracle runs ``envs`` (default: all).  Returns the report after
     asserting every bit-exact criterion; tolerances are asserted by the caller on the report."""
     sc = scenes.make_scene(spec)
@@ -144,12 +144,14 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
         th_np = (thresholds[0][sel].cpu().numpy(), thresholds[1][sel].cpu().numpy())
     if tau_r > 0.0:                                 # refractory period
         ev.set_refractory(tau_r)
+    if channel is not None:                         # colour events
+        ev.set_channel(channel)
     if margin:                                      # over-render margin: spec = the over-rendered frame
         ev.set_margin(margin)
     inner = (Ellipsis, slice(margin, H - margin), slice(margin, W - margin))
     ora = orc.Oracle(len(sel), H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
                      composite_mode=mode, debug=True, theta_on=None if th_np is None else th_np[0],
-                     theta_off=None if th_np is None else th_np[1], tau_r=tau_r, margin=margin)
+                     theta_off=None if th_np is None else th_np[1], tau_r=tau_r, margin=margin, channel=channel)
     rep = ParityReport()
     try:
         for k in range(n_keyframes):

@@ -313,6 +313,26 @@ def test_over_render_margin(margin, extra, monkeypatch):
     _assert_tolerances(rep)
 
 
+@pytest.mark.parametrize("path", PATHS)
+def test_colour_events(path):
+    """Colour events (R28): one context per channel, L = log(channel + eps); each matches the oracle
+    run on that channel, on both paths, and the three streams differ (the scenes are tinted)."""
+    spec = scenes.small(scenes.config(2), num_envs=2, height=120, width=160, num_keyframes=3)
+    n = []
+    for ch in (0, 1, 2):
+        rep = parity.run_parity(spec, 3, path=_path(path, spec), channel=ch)
+        _assert_tolerances(rep)
+        n.append(rep.events_oracle)
+    assert len(set(n)) == 3
+    ev = binding.Evis(1, 8, 8, 4, 0.2, 0.2, 1e-3, 1.0 / 60.0, event_capacity=1 << 10)
+    for bad in (-2, 3):
+        with pytest.raises(binding.EvisError) as ei:
+            ev.set_channel(bad)
+        assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+    ev.set_channel(-1)
+    ev.destroy()
+
+
 def test_margin_api_contract():
     """evis_set_margin: negative or too large margins are INVALID_ARG; margin 0 is the plain frame; coordinates
     of a margin run stay inside the cropped frame; the tile path refuses it."""
