@@ -22,7 +22,7 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 zero motion identity, P2 substep S reproduces
  * keyframe B, P3 integer translation, P4 8x8 gather-form brute force, P5 analytic two-rectangle
- * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8), P12 refractory period.  UNPINNED by paper or
+ * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8), P12 refractory period, P13 margin, P14 colour, P15 noise events.  UNPINNED by paper or
  * mathematics (fixed by DESIGN.md readings only): log base R1, epsilon R2, initial reference
  * level R6, nearest-pixel depth lookup R16, hole handling R20, the composite choice R19.
  */
@@ -161,6 +161,68 @@ void evo_composite(int H, int W, int i, int S, int mode,
     }
 }
 
+/* ---- Noise events (Eq. 9-10) [R29] --------------------------------------------------
+ * "In each synthesis step of duration dt, a pixel leaks with probability P_leak = r_l dt" (spurious ON event);
+ * shot noise: random-polarity events with P_shot = r_s dt (1 - Ibar), Ibar in [0,1] the normalized intensity;
+ * hot pixels: a fixed subset H fires with P_hot = r_h dt.  The draws come from a counter-based generator that
+ * the CUDA path implements too (same integers on both sides):
+ *   mix64 = the splitmix64 finalizer;  key(q) = mix64(mix64(mix64(seed ^ G (kf + 1)) + env) + q), q = y W + x;
+ *   h_s = mix64(key + 4 i + s) for substep i and stream s = 0, 1, 2;  a 24-bit field u gives uf = u 2^-24.
+ *   leak iff uf(h0 >> 40) < r_l dt;  shot iff uf((h0 >> 16) & 0xFFFFFF) < (r_s dt)(1 - Ibar), polarity h0 & 1;
+ *   hot (pixels of H only) iff uf(h1 >> 40) < r_h dt, polarity h0 & 2.
+ * Stamps: uniform in the substep, t = fma(uf, dt, (i - 1) dt), fields h2 >> 40 (leak), (h2 >> 16) & 0xFFFFFF
+ * (shot), (h1 >> 16) & 0xFFFFFF (hot).  Ibar = clamp((exp(L) - eps) / I_white, 0, 1) with L the frame's log
+ * value and exp32 below (binary32 with a fixed operation order, so that both sides decide alike).  Noise events
+ * follow the pixel's threshold crossings of the substep in the order leak, shot, hot; they leave L_ref alone,
+ * and they neither see nor feed the refractory period.                                                       */
+typedef struct {
+    uint64_t seed;
+    float r_leak, r_shot, r_hot;     /* rates in Hz, >= 0 */
+    float i_white;                   /* intensity that normalizes to 1 */
+    float eps;                       /* the log epsilon */
+    const uint8_t *hot;              /* [H*W] membership of H for this env, or NULL */
+} evo_noise;
+
+static uint64_t evo_mix64(uint64_t z)
+{
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ull;
+    z ^= z >> 27; z *= 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    return z;
+}
+
+uint64_t evo_noise_key(uint64_t seed, int kf, int env, int64_t q)
+{
+    uint64_t z = evo_mix64(seed ^ (0x9E3779B97F4A7C15ull * (uint64_t)(kf + 1)));
+    z = evo_mix64(z + (uint64_t)env);
+    return evo_mix64(z + (uint64_t)q);
+}
+
+uint64_t evo_noise_hash(uint64_t key, int i, int s) { return evo_mix64(key + 4ull * (uint64_t)i + (uint64_t)s); }
+
+/* exp in binary32, every operation written out: x = k ln2 + r, |r| <= ln2 / 2, Taylor to r^7 by Horner with fma,
+ * scaled by 2^k through the exponent field.  Relative error ~2e-7 on [-80, 80]; outside it saturates.          */
+float evo_exp32(float x)
+{
+    if (!(x > -80.0f)) return 0.0f;
+    if (x > 80.0f) x = 80.0f;
+    const float kf = rintf(x * 1.44269504f);
+    float r = fmaf(kf, -0.693145752f, x);          /* ln2 split in two binary32 parts */
+    r = fmaf(kf, -1.42860677e-06f, r);
+    float p = 1.98412698e-4f;                       /* 1/7! ... 1/2!, 1, 1 */
+    p = fmaf(p, r, 1.38888889e-3f);
+    p = fmaf(p, r, 8.33333333e-3f);
+    p = fmaf(p, r, 4.16666667e-2f);
+    p = fmaf(p, r, 1.66666667e-1f);
+    p = fmaf(p, r, 0.5f);
+    p = fmaf(p, r, 1.0f);
+    p = fmaf(p, r, 1.0f);
+    uint32_t bits; memcpy(&bits, &p, 4);
+    bits += (uint32_t)((int32_t)kf << 23);         /* p in [0.7, 1.5]: the exponent field cannot wrap for |k| <= 116 */
+    memcpy(&p, &bits, 4);
+    return p;
+}
+
 /* ---- Eq. 4 + reference update for one frame of one env ------------------------
  * dL = L - Lref ; n = floor(|dL| / C) ; p = sgn(dL) ; Lref <- Lref + p n C.
  * C = C+ for dL > 0, C- for dL < 0 [R4]; n capped at 255 [R7]; the k-th crossing of the frame is
@@ -176,6 +238,7 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
                         float c_pos, float c_neg,
                         const float *th_on, const float *th_off,   /* [H*W] or NULL (both): Eq. 8 maps */
                         float tau_r, float *t_last,                /* refractory period (<= 0: off) and its state */
+                        const evo_noise *noise,                    /* noise events (NULL: off) */
                         const float *Lhat,
                         float *Lref, float *Lprev,
                         evo_event *ev, int64_t cap, int64_t n_have,
@@ -236,6 +299,36 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
                 }
                 ++made;
             }
+            if (noise) {                                             /* Eq. 9-10 and hot pixels [R29] */
+                const float dtf = T / (float)S, t0 = (float)(i - 1) * dtf, U = 5.9604644775390625e-08f; /* 2^-24 */
+                const uint64_t key = evo_noise_key(noise->seed, kf, env, q);
+                const uint64_t h0 = evo_noise_hash(key, i, 0), h1 = evo_noise_hash(key, i, 1), h2 = evo_noise_hash(key, i, 2);
+                int np_[3], nk = 0; float nt[3]; int nkind[3];
+                if ((float)(h0 >> 40) * U < noise->r_leak * dtf) {
+                    np_[nk] = +1; nt[nk] = fmaf((float)(h2 >> 40) * U, dtf, t0); nkind[nk++] = 1001;
+                }
+                const float ps = noise->r_shot * dtf, us = (float)((h0 >> 16) & 0xFFFFFFu) * U;
+                if (us < ps) {
+                    float ibar = (evo_exp32(L) - noise->eps) / noise->i_white;
+                    if (!(ibar >= 0.0f)) ibar = 0.0f;
+                    if (ibar > 1.0f) ibar = 1.0f;
+                    if (us < ps * (1.0f - ibar)) {
+                        np_[nk] = (h0 & 1u) ? +1 : -1; nt[nk] = fmaf((float)((h2 >> 16) & 0xFFFFFFu) * U, dtf, t0); nkind[nk++] = 1002;
+                    }
+                }
+                if (noise->hot && noise->hot[q] && (float)(h1 >> 40) * U < noise->r_hot * dtf) {
+                    np_[nk] = (h0 & 2u) ? +1 : -1; nt[nk] = fmaf((float)((h1 >> 16) & 0xFFFFFFu) * U, dtf, t0); nkind[nk++] = 1003;
+                }
+                for (int a = 0; a < nk; ++a) {
+                    if (n_have + made < cap) {
+                        evo_event *o = &ev[n_have + made];
+                        o->env = env; o->x = x; o->y = y; o->p = np_[a]; o->substep = i; o->k = nkind[a];
+                        o->kf = kf; o->pad = 0;
+                        o->t_off = (double)nt[a];
+                    }
+                    ++made;
+                }
+            }
             if (n > 0) Lref[q] = fmaf((float)(p * n), C, Lref[q]);
             Lprev[q] = L;
         }
@@ -251,6 +344,7 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
 int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, int margin, float T, float c_pos, float c_neg,
                      const float *th_on, const float *th_off,              /* [H*W] or NULL: Eq. 8 maps of this env */
                      float tau_r, float *t_last,                           /* refractory period (<= 0: off), state [H*W] */
+                     const evo_noise *noise,                               /* noise events of this env (NULL: off) */
                      const float *LA, const float *fwdA, const float *ZA,
                      const float *LB, const float *mB, const float *ZB,
                      float *Lref, float *Lprev,
@@ -278,7 +372,7 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, int margin,
                 if (qx >= margin && qx < W - margin && qy >= margin && qy < H - margin) ++*holes;
             }
         }
-        made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, th_on, th_off, tau_r, t_last, Lhat, Lref, Lprev,
+        made += evo_event_frame(H, W, env, kf, i, S, T, c_pos, c_neg, th_on, th_off, tau_r, t_last, noise, Lhat, Lref, Lprev,
                                 ev, cap, n_have + made, dbg_dL ? dbg_dL + (int64_t)(i - 1) * P : 0);
     }
     /* the next interval starts T later: keep t_last relative to its start (binary32, -inf stays -inf) [R26] */

@@ -14,6 +14,12 @@ import numpy as np
 
 from . import build as _build
 
+class Noise(C.Structure):
+    """evo_noise (oracle/evis_oracle.c): parameters of the noise events, Eq. 9-10 and hot pixels [R29]."""
+    _fields_ = [("seed", C.c_uint64), ("r_leak", C.c_float), ("r_shot", C.c_float), ("r_hot", C.c_float),
+                ("i_white", C.c_float), ("eps", C.c_float), ("hot", C.c_void_p)]
+
+
 EVENT_DTYPE = np.dtype([("env", "<i4"), ("x", "<i4"), ("y", "<i4"), ("p", "<i4"), ("substep", "<i4"),
                         ("k", "<i4"), ("kf", "<i4"), ("pad", "<i4"), ("t_off", "<f8")])
 NONE = 0xFFFFFFFF
@@ -35,13 +41,19 @@ def lib():
         L.evo_splat.restype = None
         L.evo_composite.argtypes = [C.c_int] * 5 + [u64p, u64p, fp, fp, fp, fp, u8p, u32p]
         L.evo_composite.restype = None
-        L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [fp, fp, fp, C.c_void_p,
+        L.evo_event_frame.argtypes = [C.c_int] * 6 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [C.c_void_p] + [fp, fp, fp, C.c_void_p,
                                                                         C.c_int64, C.c_int64, fp]
         L.evo_event_frame.restype = C.c_int64
-        L.evo_interval.argtypes = ([C.c_int] * 7 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [fp] * 8 + [u64p, u64p, fp]
+        L.evo_interval.argtypes = ([C.c_int] * 7 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [C.c_void_p] + [fp] * 8 + [u64p, u64p, fp]
                                    + [C.c_void_p, C.c_int64, C.c_int64]
                                    + [u32p, u32p, u8p, u32p, fp, fp, C.POINTER(C.c_int64)])
         L.evo_interval.restype = C.c_int64
+        L.evo_exp32.argtypes = [C.c_float]
+        L.evo_exp32.restype = C.c_float
+        L.evo_noise_key.argtypes = [C.c_uint64, C.c_int, C.c_int, C.c_int64]
+        L.evo_noise_key.restype = C.c_uint64
+        L.evo_noise_hash.argtypes = [C.c_uint64, C.c_int, C.c_int]
+        L.evo_noise_hash.restype = C.c_uint64
         _lib = L
     return _lib
 
@@ -81,7 +93,8 @@ def splat(i: int, S: int, src_is_B: bool, disp: np.ndarray, Zsrc: np.ndarray, Zo
 
 def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float, T: float,
                  Lref0: Optional[np.ndarray] = None, theta_on: Optional[np.ndarray] = None,
-                 theta_off: Optional[np.ndarray] = None, tau_r: float = 0.0, t_last0: Optional[np.ndarray] = None):
+                 theta_off: Optional[np.ndarray] = None, tau_r: float = 0.0, t_last0: Optional[np.ndarray] = None,
+                 noise: Optional[dict] = None):
     """Event stage alone (Eq. 4): feed a sequence of S log frames [S,H,W] to one env.
     theta_on / theta_off [H,W]: per-pixel thresholds replacing c_pos / c_neg (Eq. 8).
     tau_r > 0: refractory period; t_last0 [H,W] = stamps of the last emitted events relative to
@@ -95,6 +108,7 @@ def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float,
     ton = None if theta_on is None else np.ascontiguousarray(theta_on, np.float32)
     toff = None if theta_off is None else np.ascontiguousarray(theta_off, np.float32)
     assert (ton is None) == (toff is None)
+    nz, _hot = _noise_struct(noise, 0)
     tl0 = np.full((H, W), -np.inf, np.float32) if t_last0 is None else np.ascontiguousarray(t_last0, np.float32)
     cap = 1 << 16
     while True:
@@ -105,10 +119,26 @@ def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float,
         for i in range(1, S + 1):
             n += lib().evo_event_frame(H, W, 0, 0, i, S, float(T), float(c_pos), float(c_neg),
                                        _f(ton) if ton is not None else None, _f(toff) if toff is not None else None,
-                                       float(tau_r), _f(tl), _f(frames[i - 1]), _f(lr), _f(lp), ev.ctypes.data, cap, n, None)
+                                       float(tau_r), _f(tl), C.addressof(nz) if nz is not None else None,
+                                       _f(frames[i - 1]), _f(lr), _f(lp), ev.ctypes.data, cap, n, None)
         if n <= cap:
             return (ev[:n], lr, tl) if tau_r > 0.0 else (ev[:n], lr)
         cap = int(n)
+
+
+def _noise_struct(noise: Optional[dict], env: int):
+    """noise = dict(seed, r_leak, r_shot, r_hot, i_white, eps, hot=None or uint8 [E,H,W] / [H,W]) -> (Noise, keepalive)."""
+    if noise is None:
+        return None, None
+    hot = noise.get("hot")
+    hp = None
+    if hot is not None:
+        hot = np.ascontiguousarray(hot, np.uint8)
+        hp = np.ascontiguousarray(hot[env] if hot.ndim == 3 else hot)
+    nz = Noise(int(noise["seed"]), float(noise.get("r_leak", 0.0)), float(noise.get("r_shot", 0.0)),
+               float(noise.get("r_hot", 0.0)), float(noise.get("i_white", 1.0)), float(noise.get("eps", 1e-3)),
+               hp.ctypes.data if hp is not None else None)
+    return nz, hp
 
 
 class Oracle:
@@ -117,7 +147,7 @@ class Oracle:
     def __init__(self, num_envs: int, height: int, width: int, substeps: int, c_pos: float, c_neg: float,
                  log_eps: float, keyframe_dt: float, composite_mode: int = 0, debug: bool = False,
                  theta_on: Optional[np.ndarray] = None, theta_off: Optional[np.ndarray] = None,
-                 tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None):
+                 tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None, noise: Optional[dict] = None):
         self.E, self.H, self.W, self.S = num_envs, height, width, substeps
         self.c_pos, self.c_neg, self.eps, self.T = c_pos, c_neg, log_eps, keyframe_dt
         self.mode = composite_mode
@@ -130,6 +160,7 @@ class Oracle:
         # over-render margin (Supp. B): height x width is the over-rendered frame; the warp runs on
         # all of it, then `margin` pixels are cropped off each side: events outside the crop are dropped and the
         # others are reported in the cropped frame's coordinates [R27]
+        self.noise = None if noise is None else dict(noise, eps=log_eps)   # Eq. 9-10 and hot pixels [R29]
         self.channel = channel                     # colour events: None = luminance, 0/1/2 = R/G/B
         self.margin = int(margin)
         assert 0 <= 2 * self.margin < min(height, width)
@@ -180,12 +211,13 @@ class Oracle:
             holes.value = 0
             n = 0
             for e in range(E):
+                nz, _hot = _noise_struct(self.noise, e)
                 d = self.dbg
                 n += lib().evo_interval(
                     H, W, S, self.mode, e, kf, self.margin, float(self.T), float(self.c_pos), float(self.c_neg),
                     _f(self.th_on[e]) if self.th_on is not None else None,
                     _f(self.th_off[e]) if self.th_off is not None else None,
-                    self.tau_r, _f(t_last[e]),
+                    self.tau_r, _f(t_last[e]), C.addressof(nz) if nz is not None else None,
                     _f(A["L"][e]), _f(A["fwd"][e]), _f(A["Z"][e]), _f(LB[e]), _f(mB[e]), _f(ZB[e]),
                     _f(Lref[e]), _f(Lprev[e]), _p(zA, C.c_uint64), _p(zB, C.c_uint64), _f(Lhat),
                     ev.ctypes.data, cap, n,

@@ -611,3 +611,86 @@ def test_p14b_colour_events_are_three_independent_runs():
         o.step(base, mv, z)
         n_ev.append(len(o.step(nxt, mv, z)))
     assert n_ev[0] == H * W * math.floor(math.log(3.0) / C) and n_ev[1] == n_ev[2] == 0
+
+
+# ---- P15: noise events (Eq. 9-10) [R29] --------------------------------------------------------
+def test_p15_generator_is_splitmix64_and_its_fields_are_uniform():
+    """The counter hash is the published splitmix64 output function: with key + 4 i + s equal to the golden-ratio
+    increment it must return the first output of splitmix64 seeded with 0 (known test vector).  Its 24-bit fields
+    are uniform and the three streams are uncorrelated."""
+    L = orc.lib()
+    G = 0x9E3779B97F4A7C15
+    assert L.evo_noise_hash((G - 4) & (2 ** 64 - 1), 1, 0) == 0xE220A8397B1DCDAF
+    assert L.evo_noise_hash((2 * G - 6) & (2 ** 64 - 1), 1, 2) == 0x6E789E6AA1B965F4
+    key = [L.evo_noise_key(12345, 3, 1, q) for q in range(4000)]
+    assert len(set(key)) == 4000
+    f = lambda h, sh: ((h >> sh) & 0xFFFFFF) / 2.0 ** 24
+    u = np.array([[f(L.evo_noise_hash(k, i, s), sh) for s in (0, 1, 2) for sh in (40, 16)] for k in key for i in (1, 2, 3)])
+    assert np.all(np.abs(u.mean(axis=0) - 0.5) < 4 * (1 / 12 / len(u)) ** 0.5)
+    hist = np.stack([np.histogram(u[:, c], bins=16, range=(0, 1))[0] for c in range(u.shape[1])])
+    chi2 = ((hist - len(u) / 16) ** 2 / (len(u) / 16)).sum(axis=1)
+    assert np.all(chi2 < 45.0)                                   # 15 dof: P(chi2 > 45) ~ 8e-5
+    cc = np.corrcoef(u.T)
+    assert np.all(np.abs(cc - np.eye(u.shape[1])) < 0.04)
+
+
+def test_p15b_exp32_is_exp():
+    xs = np.concatenate([np.linspace(-20, 20, 4001), [-79.9, 79.9, 0.0, -0.0, 1e-8]]).astype(np.float32)
+    for x in xs:
+        got, want = orc.lib().evo_exp32(float(x)), math.exp(float(x))
+        assert abs(got - want) <= 6e-7 * want, (x, got, want)
+    assert orc.lib().evo_exp32(-1000.0) == 0.0 and orc.lib().evo_exp32(float("nan")) == 0.0
+    assert orc.lib().evo_exp32(1000.0) == orc.lib().evo_exp32(80.0)
+
+
+def _noise_run(L_value, noise, S=64, H=40, W=50, T=1.0):
+    frames = np.full((S, H, W), L_value, np.float32)
+    ev, lr = orc.event_frames(frames, frames[0], 0.2, 0.2, T, noise=noise)
+    return ev, S * H * W, T / S
+
+
+def test_p15c_leak_rate_polarity_and_stamps():
+    """Static scene, leak only: every pixel-substep is a Bernoulli trial with P = r_l dt (Eq. 9); the events are ON,
+    their stamps uniform inside their substep; another seed gives another draw; zero rates give nothing."""
+    noise = dict(seed=7, r_leak=3.2, eps=1e-3)
+    ev, N, dt = _noise_run(0.0, noise)
+    P = 3.2 * dt
+    assert abs(len(ev) - N * P) < 4 * (N * P * (1 - P)) ** 0.5
+    assert np.all(ev["p"] == 1) and np.all(ev["k"] == 1001)
+    fr = ev["t_off"] / dt - (ev["substep"] - 1)
+    assert np.all((fr >= 0) & (fr < 1)) and abs(fr.mean() - 0.5) < 4 * (1 / 12 / len(ev)) ** 0.5
+    ev2, _, _ = _noise_run(0.0, dict(noise, seed=8))
+    assert len(ev2) != len(ev) or not np.array_equal(ev2["x"], ev["x"])
+    assert len(_noise_run(0.0, dict(seed=7, eps=1e-3))[0]) == 0
+
+
+def test_p15d_shot_rate_falls_with_intensity():
+    """Eq. 10: P_shot = r_s dt (1 - Ibar).  Black (I = 0): the full rate; I = I_white / 2: half of it; I >= I_white:
+    none.  Polarity is a fair coin."""
+    eps, iw = 1e-3, 2.0
+    for I, frac in ((0.0, 1.0), (1.0, 0.5), (2.0, 0.0), (50.0, 0.0)):
+        ev, N, dt = _noise_run(math.log(I + eps), dict(seed=11, r_shot=6.4, i_white=iw, eps=eps))
+        P = 6.4 * dt * frac
+        assert abs(len(ev) - N * P) <= 4 * (N * P * (1 - P)) ** 0.5 + (0 if frac else 0), (I, len(ev), N * P)
+        if frac:
+            assert np.all(ev["k"] == 1002) and abs((ev["p"] == 1).mean() - 0.5) < 4 * 0.5 / len(ev) ** 0.5
+
+
+def test_p15e_hot_pixels_and_signal_untouched():
+    """Hot pixels fire only inside H, at r_h dt; with all three sources on, the threshold crossings, their stamps
+    and L_ref are those of the noise-free run (noise events leave L_ref alone)."""
+    S, H, W = 64, 40, 50
+    hot = np.zeros((H, W), np.uint8)
+    hot[::5, ::7] = 1
+    ev, N, dt = _noise_run(0.0, dict(seed=3, r_hot=16.0, eps=1e-3, hot=hot), S, H, W)
+    n_hot = int(hot.sum()) * S
+    P = 16.0 * dt
+    assert np.all(hot[ev["y"], ev["x"]] == 1) and np.all(ev["k"] == 1003)
+    assert abs(len(ev) - n_hot * P) < 4 * (n_hot * P * (1 - P)) ** 0.5
+    r = _rng(16)
+    frames = np.cumsum(r.normal(0, 0.15, size=(S, H, W)), axis=0).astype(np.float32)
+    L0 = np.zeros((H, W), np.float32)
+    a, lra = orc.event_frames(frames, L0, 0.2, 0.3, 1.0)
+    b, lrb = orc.event_frames(frames, L0, 0.2, 0.3, 1.0, noise=dict(seed=3, r_leak=2.0, r_shot=2.0, r_hot=9.0, eps=1e-3, hot=hot))
+    sig = b[b["k"] < 1000]
+    assert np.array_equal(lra, lrb) and len(b) > len(a) and np.array_equal(sig, a)
