@@ -140,6 +140,24 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
  * stay in force), BAD_STATE (tile path), CUDA, OOM. */
 int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta_off, int src_is_device);
 
+/* Noise events (Eq. 9-10; R29).  In every substep (duration dt = T / S) every pixel
+ * draws, from a counter-based generator keyed (seed, interval, env, pixel, substep) -- so the stream does not depend
+ * on scheduling --: a leak event (ON) with probability r_leak dt (Eq. 9); a shot event of random polarity with
+ * probability r_shot dt (1 - Ibar), Ibar = clamp((exp(L) - eps) / i_white, 0, 1) the normalized intensity of the
+ * warped frame (Eq. 10); and, for the pixels of the hot set, an event of random polarity with probability r_hot dt.
+ * Their timestamps are uniform inside the substep; they follow the pixel's threshold crossings of that substep in
+ * the stream (leak, shot, hot), leave L_ref alone and neither see nor feed the refractory period.  Rates in Hz. */
+typedef struct {
+    uint64_t seed;
+    float    r_leak, r_shot, r_hot;   /* >= 0 */
+    float    i_white;                 /* > 0: the linear intensity that normalizes to 1 */
+} evis_noise;
+/* noise = NULL switches the noise events off.  hot_mask: [E,H,W] bytes, non-zero = the pixel belongs to the hot set
+ * (DEVICE pointer if mask_is_device != 0, else HOST; nullable = empty set); the library copies it.  Applies from the
+ * next evis_step on; synchronises.  Global path only.  Errors: INVALID_ARG (negative or non-finite rate, i_white
+ * <= 0), BAD_STATE (tile path), CUDA, OOM. */
+int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_mask, int mask_is_device);
+
 /* Colour events ("Replacing I with individual R, G, B channels and applying the event model to each
  * independently produces color events"; R28): channel = 0, 1 or 2 makes this context take
  * L = log(channel + eps) of the radiance's R, G or B instead of the Rec.709 luminance; -1 = luminance (default).

@@ -53,7 +53,7 @@ class evis_profile(C.Structure):
 # every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
-           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel"]
+           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise"]
 
 _lib = None
 
@@ -86,12 +86,18 @@ def load() -> C.CDLL:
     L.evis_set_refractory.argtypes = [vp, C.c_float]
     L.evis_set_margin.argtypes = [vp, C.c_int]
     L.evis_set_channel.argtypes = [vp, C.c_int]
+    L.evis_set_noise.argtypes = [vp, C.POINTER(evis_noise), vp, C.c_int]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
     for name in SYMBOLS:
         getattr(L, name)              # raises AttributeError if the library lacks a declared symbol
     _lib = L
     return L
+
+
+class evis_noise(C.Structure):
+    _fields_ = [("seed", C.c_uint64), ("r_leak", C.c_float), ("r_shot", C.c_float), ("r_hot", C.c_float),
+                ("i_white", C.c_float)]
 
 
 class EvisError(RuntimeError):
@@ -167,6 +173,22 @@ class Evis:
         p_on, p_off = _dev_ptr(theta_on, (E, H, W), "theta_on"), _dev_ptr(theta_off, (E, H, W), "theta_off")
         torch.cuda.synchronize(self.device)                 # the library copies on its own stream
         _check(self._lib.evis_set_thresholds(self._ctx, p_on, p_off, 1), "evis_set_thresholds")
+
+    def set_noise(self, seed: int = 0, r_leak: float = 0.0, r_shot: float = 0.0, r_hot: float = 0.0,
+                  i_white: float = 1.0, hot: Optional[torch.Tensor] = None, off: bool = False) -> None:
+        """evis_set_noise (Eq. 9-10 and hot pixels): rates in Hz; ``hot`` = uint8 CUDA tensor [E,H,W] or None;
+        ``off=True`` switches the noise events off."""
+        if off:
+            _check(self._lib.evis_set_noise(self._ctx, None, None, 1), "evis_set_noise")
+            return
+        cfg = evis_noise(int(seed), float(r_leak), float(r_shot), float(r_hot), float(i_white))
+        hp = None
+        if hot is not None:
+            if not (hot.is_cuda and hot.dtype == torch.uint8 and hot.is_contiguous() and tuple(hot.shape) == (self.E, self.H, self.W)):
+                raise ValueError("hot: need a contiguous uint8 CUDA tensor of shape (E, H, W)")
+            torch.cuda.synchronize(self.device)
+            hp = hot.data_ptr()
+        _check(self._lib.evis_set_noise(self._ctx, C.byref(cfg), hp, 1), "evis_set_noise")
 
     def set_channel(self, channel: int) -> None:
         """evis_set_channel (colour events): 0 / 1 / 2 = log of R / G / B, -1 = Rec.709 luminance."""

@@ -27,6 +27,8 @@ struct evis_ctx {
     float *l_ref, *l_prev;
     float *th_on, *th_off;            // Eq. 8 maps [E*H*W] (owned), in force when th_active
     bool th_active;
+    evis_noise noise; bool noise_on;  // noise events (Eq. 9-10), parameters as given
+    unsigned char *hot;               // hot-pixel set [E*H*W] (owned) or null
     int channel; bool channel_set;    // colour events: log of one channel instead of the luminance
     float *t_last;                    // refractory state [E*H*W] (owned), in force when tau_r > 0
     float tau_r;
@@ -154,6 +156,14 @@ struct Span {
     }
 };
 
+unsigned long long host_mix64(unsigned long long z)      // splitmix64 output function (R29)
+{
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ull;
+    z ^= z >> 27; z *= 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    return z;
+}
+
 size_t env_size_mb(const char *name, size_t dflt)
 {
     const char *v = getenv(name);
@@ -168,7 +178,7 @@ void free_all(evis_ctx *ctx)
         if (k == 0) cudaFree(ctx->kf[k].L);
         cudaFree(ctx->kf[k].mv); cudaFree(ctx->kf[k].fwd); cudaFree(ctx->kf[k].Z);
     }
-    cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last); cudaFree(ctx->tab); cudaFree(ctx->zmem);
+    cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last); cudaFree(ctx->hot); cudaFree(ctx->tab); cudaFree(ctx->zmem);
     cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
     cudaFree(ctx->st_rad); cudaFree(ctx->st_mv); cudaFree(ctx->st_fwd); cudaFree(ctx->st_depth);
@@ -426,7 +436,21 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     ctx->ep.kf = (uint32_t)(ctx->steps - 1);
     EventSink sink{ctx->arrival, ctx->arrival_cap, ctx->counters + C_ALLOC, ctx->counters + C_EVENTS, ctx->directory};
     const Thresholds th{ctx->th_active ? ctx->th_on : nullptr, ctx->th_active ? ctx->th_off : nullptr};
-    const Refractory rf{ctx->tau_r > 0.0f ? ctx->t_last : nullptr, ctx->tau_r, ctx->cfg.keyframe_dt};
+    // direct mode (the resolve kernel writes events) serves the refractory period and the noise events
+    Refractory rf{};
+    rf.t_last = (ctx->tau_r > 0.0f || ctx->noise_on) ? ctx->t_last : nullptr;
+    rf.tau_r = ctx->tau_r;
+    rf.T = ctx->cfg.keyframe_dt;
+    if (ctx->noise_on) {
+        // P = r dt, binary32 products of the rates and T / S (R29); the per-step part of the generator keys
+        volatile float pl = ctx->noise.r_leak * ctx->ep.dt, ps = ctx->noise.r_shot * ctx->ep.dt, ph = ctx->noise.r_hot * ctx->ep.dt;
+        rf.noise_on = 1;
+        rf.noise_key = host_mix64(ctx->noise.seed ^ (0x9E3779B97F4A7C15ull * ((unsigned long long)ctx->ep.kf + 1ull)));
+        rf.p_leak = pl; rf.p_shot = ps; rf.p_hot = ph;
+        rf.i_white = ctx->noise.i_white;
+        rf.eps = ctx->cfg.log_eps;
+        rf.hot = ctx->hot;
+    }
     {
         Span sp(ctx, st, EVIS_STAGE_CLEAR, 2);
         CU(cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), st));   // the per-step counters
@@ -552,11 +576,41 @@ int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta
     }
     cudaFree(bad);
     if (rc != EVIS_OK) { cudaFree(on); cudaFree(off); return rc; }
-    cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last);
+    cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last); cudaFree(ctx->hot);
     if (!ctx->th_on) ctx->device_bytes += 2 * P * sizeof(float);
     ctx->th_on = on; ctx->th_off = off;
     ctx->th_active = true;
     ctx->launches += 2;
+    return EVIS_OK;
+}
+
+int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_mask, int mask_is_device)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    if (!noise) { ctx->noise_on = false; return EVIS_OK; }
+    const float big = 3.0e38f;
+    if (!(noise->r_leak >= 0.0f && noise->r_leak < big) || !(noise->r_shot >= 0.0f && noise->r_shot < big) ||
+        !(noise->r_hot >= 0.0f && noise->r_hot < big) || !(noise->i_white > 0.0f && noise->i_white < big))
+        return EVIS_ERR_INVALID_ARG;
+    const size_t P = (size_t)ctx->g.E * ctx->g.HW;
+    if (hot_mask) {
+        if (!ctx->hot) CU(dalloc(ctx, &ctx->hot, P));
+        CU(cudaMemcpyAsync(ctx->hot, hot_mask, P, mask_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->own_stream));
+    } else if (ctx->hot) {
+        cudaFree(ctx->hot);
+        ctx->hot = nullptr;
+    }
+    if (!ctx->t_last) {                                   // the direct resolve variant carries t_last
+        CU(dalloc(ctx, &ctx->t_last, P));
+        CU(launch_fill(ctx->t_last, (long long)P, -INFINITY, ctx->own_stream));
+    }
+    CU(cudaStreamSynchronize(ctx->own_stream));
+    ctx->noise = *noise;
+    ctx->noise_on = true;
     return EVIS_OK;
 }
 

@@ -38,8 +38,14 @@ struct Thresholds {
 // With it on, the resolve kernel leaves EVENTS (not records) in the arrival buffer and order.cu copies them.
 struct Refractory {
     float *t_last;
-    float tau_r;    // seconds, > 0
+    float tau_r;    // seconds, >= 0 (0 with t_last set: direct mode for the noise events only)
     float T;        // keyframe period
+    // Noise events (Eq. 9-10, R29); they ride on the direct (event-writing) resolve variant
+    int noise_on;
+    unsigned long long noise_key;    // mix64(seed ^ G (kf + 1)): the per-step part of the pixel keys
+    float p_leak, p_shot, p_hot;     // r dt, binary32 products
+    float i_white, eps;
+    const unsigned char *hot;        // [E*H*W] membership of the hot set, or null
 };
 
 struct DebugOut {  // all nullable; [S,E,H,W]

@@ -333,6 +333,95 @@ def test_colour_events(path):
     ev.destroy()
 
 
+@pytest.mark.parametrize("tau_r,margin", [(0.0, 0), (0.002, 6)])
+def test_noise_events(tau_r, margin):
+    """Noise events (Eq. 9-10, R29): leak, shot and hot-pixel events drawn by the counter-based
+    generator must be the oracle's, event for event (pixel, substep, polarity, stamp), interleaved with the threshold
+    crossings; L_ref is that of the noise-free run.  Second case: with a refractory period and an over-render margin."""
+    from oracle import evis_oracle as orc
+    spec = scenes.small(scenes.config(4), num_envs=3, height=97 + 2 * margin, width=131 + 2 * margin, num_keyframes=4)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    gen = torch.Generator().manual_seed(5)
+    hot = (torch.rand((E, H, W), generator=gen) < 0.02).to(torch.uint8)
+    par = dict(seed=99, r_leak=20.0, r_shot=60.0, r_hot=400.0, i_white=1.5)
+    sc = scenes.make_scene(spec)
+    ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, path=binding.PATH_GLOBAL,
+                      event_capacity=1 << 24)
+    ev.set_noise(hot=hot.cuda(), **par)
+    if tau_r:
+        ev.set_refractory(tau_r)
+    if margin:
+        ev.set_margin(margin)
+    ora = orc.Oracle(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, tau_r=tau_r, margin=margin,
+                     noise=dict(par, hot=hot.numpy()))
+    ref = orc.Oracle(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, tau_r=tau_r, margin=margin)
+    n_noise = 0
+    for k in range(4):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        n = ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        h = {key: v.cpu().numpy() for key, v in kf.items()}
+        oe = ora.step(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"])
+        re_ = ref.step(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"])
+        ge = ev.read_events()
+        assert n == len(ge) == len(oe)
+        if k == 0:
+            continue
+        assert np.array_equal(oe[oe["k"] < 1000], re_)                 # the crossings are those of the noise-free run
+        n_noise += int((oe["k"] >= 1000).sum())
+        g = ge[np.lexsort((ge["t_off"], ge["x"], ge["y"], ge["substep"], ge["env"]))]
+        o = oe[np.lexsort((oe["t_off"], oe["x"], oe["y"], oe["substep"], oe["env"]))]
+        for f in ("env", "x", "y", "substep", "p"):
+            assert np.array_equal(g[f].astype(np.int64), o[f].astype(np.int64)), f
+        assert float(np.max(np.abs(g["t_off"].astype(np.float64) - o["t_off"]))) <= parity.TOL_T
+        lref, _ = ev.get_state()
+        inner = (Ellipsis, slice(margin, H - margin), slice(margin, W - margin))
+        assert np.array_equal(lref[inner], ora.Lref[inner])
+    ev.destroy()
+    # all three sources fired: expected counts from the rates (3 intervals)
+    assert n_noise > 0.5 * 3 * E * (H - 2 * margin) * (W - 2 * margin) * (20.0 + 400.0 * 0.02) * spec.keyframe_dt
+
+
+def test_noise_api_contract():
+    """evis_set_noise: bad rates are INVALID_ARG; switching it off restores the plain stream exactly; the tile path
+    refuses it."""
+    spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=3)
+    E, H, W = spec.num_envs, spec.height, spec.width
+    sc = scenes.make_scene(spec)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(3)]
+
+    def run(setup, path=binding.PATH_GLOBAL):
+        ev = binding.Evis(E, H, W, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                          max_motion_px=spec.max_motion_px(), path=path, event_capacity=1 << 22)
+        setup(ev)
+        out = []
+        for kf in kfs:
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+            out.append(ev.read_events().copy())
+        ev.destroy()
+        return np.concatenate(out)
+
+    base = run(lambda ev: None)
+
+    def bad(ev):
+        for kw in (dict(r_leak=-1.0), dict(r_shot=float("nan")), dict(r_hot=float("inf")), dict(i_white=0.0)):
+            with pytest.raises(binding.EvisError) as ei:
+                ev.set_noise(**kw)
+            assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+        ev.set_noise(seed=1, r_leak=50.0)
+        ev.set_noise(off=True)
+    assert np.array_equal(base, run(bad))
+    noisy = run(lambda ev: ev.set_noise(seed=1, r_leak=50.0))
+    assert len(noisy) > len(base)
+    assert np.array_equal(noisy, run(lambda ev: ev.set_noise(seed=1, r_leak=50.0)))      # deterministic
+    assert not np.array_equal(noisy, run(lambda ev: ev.set_noise(seed=2, r_leak=50.0)))
+
+    def tile(ev):
+        with pytest.raises(binding.EvisError) as ei:
+            ev.set_noise(seed=1, r_leak=1.0)
+        assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    run(tile, path=binding.PATH_TILE)
+
+
 def test_margin_api_contract():
     """evis_set_margin: negative or too large margins are INVALID_ARG; margin 0 is the plain frame; coordinates
     of a margin run stay inside the cropped frame; the tile path refuses it."""
