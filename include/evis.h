@@ -125,6 +125,13 @@ int evis_create(const evis_config *cfg, evis_ctx **out);
 int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd,
               const float *depth, void *cuda_stream, uint64_t *n_events);
 
+/* The ordered stream of a step is produced on a stream of the library's own, after the step's work on
+ * `cuda_stream`, so that it overlaps the next evis_step (the calls that return events or counters wait for it).
+ * evis_wait_events makes `cuda_stream` wait for the ordered stream of the last step -- needed only by a caller that
+ * consumes evis_events_device()'s buffer, or measures time, on its own stream without one of those calls.
+ * Errors: INVALID_ARG, CUDA. */
+int evis_wait_events(evis_ctx *ctx, void *cuda_stream);
+
 /* Same step with HOST buffers (pageable or pinned): copies them to device staging owned by the
  * context on the context's own stream, runs the step and synchronises.  n_events nullable. */
 int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd,

@@ -53,7 +53,7 @@ class evis_profile(C.Structure):
 # every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
-           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise"]
+           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events"]
 
 _lib = None
 
@@ -86,6 +86,7 @@ def load() -> C.CDLL:
     L.evis_set_refractory.argtypes = [vp, C.c_float]
     L.evis_set_margin.argtypes = [vp, C.c_int]
     L.evis_set_channel.argtypes = [vp, C.c_int]
+    L.evis_wait_events.argtypes = [vp, vp]
     L.evis_set_noise.argtypes = [vp, C.POINTER(evis_noise), vp, C.c_int]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
@@ -201,6 +202,11 @@ class Evis:
     def set_refractory(self, tau_r: float) -> None:
         """evis_set_refractory: refractory period in seconds, 0 = off; resets the per-pixel state."""
         _check(self._lib.evis_set_refractory(self._ctx, float(tau_r)), "evis_set_refractory")
+
+    def wait_events(self, stream: Optional[torch.cuda.Stream] = None) -> None:
+        """evis_wait_events: make ``stream`` (default: torch's current stream) wait for the last step's ordered stream."""
+        st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+        _check(self._lib.evis_wait_events(self._ctx, C.c_void_p(st)), "evis_wait_events")
 
     def step_host(self, rad, mv_bwd, depth, mv_fwd=None, allow=()) -> int:
         """evis_step_host: HOST buffers (numpy or CPU tensors); copies, runs and synchronises."""

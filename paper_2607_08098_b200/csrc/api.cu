@@ -52,8 +52,20 @@ struct evis_ctx {
     cudaEvent_t ev_fork, ev_join[MAX_REG];
 
     // event stream
-    uint4 *arrival, *ordered;
-    uint2 *directory;
+    // The order stage of step k runs on `ord_stream` while the chunk phase of step k + 1 runs on the caller's
+    // stream (it is bound by HBM, the chunk phase by instruction issue), so the buffers the two share are doubled:
+    // slot = step & 1 (slot 1 aliases slot 0 when EVIS_NO_OVERLAP=1).  `ordered`, `bsum` and the sticky counters
+    // are touched by the order stream only.
+    uint4 *arrival, *ordered;         // arrival = slot 0
+    uint2 *directory;                 // slot 0
+    uint4 *arrival_s[2];
+    uint2 *directory_s[2];
+    unsigned long long *counters_s[2];
+    cudaStream_t ord_stream;
+    cudaEvent_t ev_chunks[2], ev_order[2];
+    bool ord_pending[2];
+    bool overlap;
+    int last_slot;
     uint32_t dir_entries;
     unsigned long long *bsum;
     // device counters.  Reset every step: [0] events, [1] holes, [2] arrival slots handed out,
@@ -186,6 +198,14 @@ void free_all(evis_ctx *ctx)
     prof_drain(ctx);
     for (cudaEvent_t e : ctx->prof_free) cudaEventDestroy(e);
     ctx->prof_free.clear();
+    if (ctx->arrival_s[1] != ctx->arrival_s[0]) {
+        cudaFree(ctx->arrival_s[1]); cudaFree(ctx->directory_s[1]); cudaFree(ctx->counters_s[1]);
+    }
+    if (ctx->ord_stream) cudaStreamDestroy(ctx->ord_stream);
+    for (int k = 0; k < 2; ++k) {
+        if (ctx->ev_chunks[k]) cudaEventDestroy(ctx->ev_chunks[k]);
+        if (ctx->ev_order[k]) cudaEventDestroy(ctx->ev_order[k]);
+    }
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int r = 0; r < evis_ctx::MAX_REG; ++r) {
         if (ctx->reg_stream[r]) cudaStreamDestroy(ctx->reg_stream[r]);
@@ -322,6 +342,23 @@ int create_impl(evis_ctx *ctx)
     CU(cudaMemset(ctx->counters, 0, NCOUNTERS * sizeof(unsigned long long)));
     CU(cudaHostAlloc((void **)&ctx->h_counters, NCOUNTERS * sizeof(unsigned long long), cudaHostAllocDefault));
     memset(ctx->h_counters, 0, NCOUNTERS * sizeof(unsigned long long));
+    {
+        const char *no = getenv("EVIS_NO_OVERLAP");       // test hook: order stage serialised with the next step
+        ctx->overlap = !(no && no[0] == '1');
+        ctx->arrival_s[0] = ctx->arrival; ctx->directory_s[0] = ctx->directory; ctx->counters_s[0] = ctx->counters;
+        ctx->arrival_s[1] = ctx->arrival; ctx->directory_s[1] = ctx->directory; ctx->counters_s[1] = ctx->counters;
+        if (ctx->overlap) {
+            CU(dalloc(ctx, &ctx->arrival_s[1], (size_t)ctx->arrival_cap));
+            CU(dalloc(ctx, &ctx->directory_s[1], (size_t)ent));
+            CU(dalloc(ctx, &ctx->counters_s[1], NCOUNTERS));
+            CU(cudaMemset(ctx->counters_s[1], 0, NCOUNTERS * sizeof(unsigned long long)));
+        }
+        CU(cudaStreamCreateWithFlags(&ctx->ord_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < 2; ++k) {
+            CU(cudaEventCreateWithFlags(&ctx->ev_chunks[k], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&ctx->ev_order[k], cudaEventDisableTiming));
+        }
+    }
     if (c.debug_capture) {
         CU(dalloc(ctx, &ctx->dbg.win, P * g.S));
         CU(dalloc(ctx, &ctx->dbg.dir, P * g.S));
@@ -330,9 +367,18 @@ int create_impl(evis_ctx *ctx)
     return EVIS_OK;
 }
 
+// everything this context has enqueued: the caller's stream of the last step, then the order stream
+cudaError_t sync_all(evis_ctx *ctx)
+{
+    cudaError_t e = cudaSuccess;
+    if (ctx->last_stream || ctx->steps) e = cudaStreamSynchronize(ctx->last_stream);
+    if (e == cudaSuccess && ctx->ord_stream) e = cudaStreamSynchronize(ctx->ord_stream);
+    return e;
+}
+
 int fetch_counters(evis_ctx *ctx)
 {
-    if (ctx->last_stream || ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    CU(sync_all(ctx));
     ctx->last_events = ctx->h_counters[C_EVENTS];
     ctx->last_holes = ctx->h_counters[C_HOLES];
     ctx->last_motion = ctx->h_counters[C_MOTION] != 0;
@@ -434,7 +480,12 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     }
 
     ctx->ep.kf = (uint32_t)(ctx->steps - 1);
-    EventSink sink{ctx->arrival, ctx->arrival_cap, ctx->counters + C_ALLOC, ctx->counters + C_EVENTS, ctx->directory};
+    // slot of this step's arrival buffer, directory and per-step counters; the order stage that used it last
+    // (two steps ago with overlap, the last step without) must be done before it is cleared
+    const int sl = ctx->overlap ? (int)(ctx->steps & 1) : 0;
+    unsigned long long *cnt = ctx->counters_s[sl];
+    if (ctx->ord_pending[sl]) CU(cudaStreamWaitEvent(st, ctx->ev_order[sl], 0));
+    EventSink sink{ctx->arrival_s[sl], ctx->arrival_cap, cnt + C_ALLOC, cnt + C_EVENTS, ctx->directory_s[sl]};
     const Thresholds th{ctx->th_active ? ctx->th_on : nullptr, ctx->th_active ? ctx->th_off : nullptr};
     // direct mode (the resolve kernel writes events) serves the refractory period and the noise events
     Refractory rf{};
@@ -453,8 +504,8 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     }
     {
         Span sp(ctx, st, EVIS_STAGE_CLEAR, 2);
-        CU(cudaMemsetAsync(ctx->counters, 0, 4 * sizeof(unsigned long long), st));   // the per-step counters
-        CU(cudaMemsetAsync(ctx->directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
+        CU(cudaMemsetAsync(cnt, 0, 4 * sizeof(unsigned long long), st));   // the per-step counters
+        CU(cudaMemsetAsync(sink.directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
     }
 
     if (ctx->path == EVIS_PATH_GLOBAL) {
@@ -502,7 +553,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 {
                     Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 1, !multi);
                     CU(launch_global_resolve(g, zc, A, B, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, th, rf, sink,
-                                             ctx->counters + C_HOLES, ctx->dbg, cs));
+                                             cnt + C_HOLES, ctx->dbg, cs));
                 }
             }
         }
@@ -513,22 +564,32 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
             }
     } else {
         Span sp(ctx, st, EVIS_STAGE_TILE, 1);
-        CU(launch_tile(g, ctx->tile, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink, ctx->counters + C_HOLES,
-                       ctx->counters + C_ITEM, ctx->dbg, st));
+        CU(launch_tile(g, ctx->tile, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink, cnt + C_HOLES,
+                       cnt + C_ITEM, ctx->dbg, st));
     }
+    // a8, second half, on the order stream: it starts when this step's chunks are done and overlaps the next step
+    cudaStream_t os = ctx->ord_stream;
+    CU(cudaEventRecord(ctx->ev_chunks[sl], st));
+    CU(cudaStreamWaitEvent(os, ctx->ev_chunks[sl], 0));
     {
-        Span sp(ctx, st, EVIS_STAGE_ORDER, 3);
+        Span sp(ctx, os, EVIS_STAGE_ORDER, 3);
+        unsigned long long *sticky = ctx->counters_s[0];             // C_MOTION, C_TOTAL live in slot 0's array
         if (ctx->path == EVIS_PATH_GLOBAL && !rf.t_last) {
             const uint32_t tx = (g.W + G_TILE_W - 1) / G_TILE_W, ty = (g.H + G_TILE_H - 1) / G_TILE_H;
             CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
-                             ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, ctx->ep, th, (uint32_t)g.W,
-                             (uint32_t)g.HW, (uint32_t)g.margin, tx, tx * ty, (uint32_t)g.S, st));
+                             cnt + C_EVENTS, sticky + C_TOTAL, ctx->ep, th, (uint32_t)g.W,
+                             (uint32_t)g.HW, (uint32_t)g.margin, tx, tx * ty, (uint32_t)g.S, os));
         } else {
             CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
-                            ctx->counters + C_EVENTS, ctx->counters + C_TOTAL, st));
+                            cnt + C_EVENTS, sticky + C_TOTAL, os));
         }
+        CU(cudaMemcpyAsync(ctx->h_counters, cnt, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, os));
+        CU(cudaMemcpyAsync(ctx->h_counters + C_MOTION, sticky + C_MOTION, 2 * sizeof(unsigned long long),
+                           cudaMemcpyDeviceToHost, os));
     }
-    CU(cudaMemcpyAsync(ctx->h_counters, ctx->counters, NCOUNTERS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaEventRecord(ctx->ev_order[sl], os));
+    ctx->ord_pending[sl] = true;
+    ctx->last_slot = sl;
     ctx->steps += 1;
     ctx->cur ^= 1;
     ctx->have_events = true;
@@ -549,7 +610,7 @@ int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     // work already enqueued keeps the thresholds it was launched with
-    if (ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    if (ctx->steps) CU(sync_all(ctx));
     if (!theta_on) { ctx->th_active = false; return EVIS_OK; }
     const size_t P = (size_t)ctx->g.E * ctx->g.HW;
     float *on = nullptr, *off = nullptr;
@@ -584,13 +645,23 @@ int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta
     return EVIS_OK;
 }
 
+int evis_wait_events(evis_ctx *ctx, void *cuda_stream)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->steps > 1 && ctx->ord_pending[ctx->last_slot])
+        CU(cudaStreamWaitEvent((cudaStream_t)cuda_stream, ctx->ev_order[ctx->last_slot], 0));
+    return EVIS_OK;
+}
+
 int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_mask, int mask_is_device)
 {
     if (!ctx) return EVIS_ERR_INVALID_ARG;
     if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
-    if (ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    if (ctx->steps) CU(sync_all(ctx));
     if (!noise) { ctx->noise_on = false; return EVIS_OK; }
     const float big = 3.0e38f;
     if (!(noise->r_leak >= 0.0f && noise->r_leak < big) || !(noise->r_shot >= 0.0f && noise->r_shot < big) ||
@@ -629,7 +700,7 @@ int evis_set_margin(evis_ctx *ctx, int margin)
     if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
-    if (ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    if (ctx->steps) CU(sync_all(ctx));
     ctx->g.margin = margin;
     return EVIS_OK;
 }
@@ -640,7 +711,7 @@ int evis_set_refractory(evis_ctx *ctx, float tau_r)
     if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
-    if (ctx->steps) CU(cudaStreamSynchronize(ctx->last_stream));
+    if (ctx->steps) CU(sync_all(ctx));
     if (tau_r > 0.0f) {
         // (re)start with no event emitted yet: t_last = -inf at every pixel
         const size_t P = (size_t)ctx->g.E * ctx->g.HW;
@@ -753,7 +824,7 @@ int evis_get_state(evis_ctx *ctx, float *l_ref, float *l_prev)
     if (!ctx) return EVIS_ERR_INVALID_ARG;
     if (!ctx->steps) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
-    CU(cudaStreamSynchronize(ctx->last_stream));
+    CU(sync_all(ctx));
     const size_t bytes = (size_t)ctx->g.E * ctx->g.HW * sizeof(float);
     if (l_ref) CU(cudaMemcpy(l_ref, ctx->l_ref, bytes, cudaMemcpyDeviceToHost));
     if (l_prev) CU(cudaMemcpy(l_prev, ctx->l_prev, bytes, cudaMemcpyDeviceToHost));
@@ -765,7 +836,7 @@ int evis_set_state(evis_ctx *ctx, const float *l_ref, const float *l_prev)
     if (!ctx) return EVIS_ERR_INVALID_ARG;
     if (!ctx->steps) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
-    CU(cudaStreamSynchronize(ctx->last_stream));
+    CU(sync_all(ctx));
     const size_t bytes = (size_t)ctx->g.E * ctx->g.HW * sizeof(float);
     if (l_ref) CU(cudaMemcpy(ctx->l_ref, l_ref, bytes, cudaMemcpyHostToDevice));
     if (l_prev) CU(cudaMemcpy(ctx->l_prev, l_prev, bytes, cudaMemcpyHostToDevice));
@@ -777,7 +848,7 @@ int evis_debug_read(evis_ctx *ctx, uint32_t *win, uint8_t *dir, float *l_hat)
     if (!ctx) return EVIS_ERR_INVALID_ARG;
     if (!ctx->cfg.debug_capture || ctx->steps < 2) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
-    CU(cudaStreamSynchronize(ctx->last_stream));
+    CU(sync_all(ctx));
     const size_t n = (size_t)ctx->g.E * ctx->g.HW * ctx->g.S;
     if (win) CU(cudaMemcpy(win, ctx->dbg.win, n * sizeof(uint32_t), cudaMemcpyDeviceToHost));
     if (dir) CU(cudaMemcpy(dir, ctx->dbg.dir, n, cudaMemcpyDeviceToHost));

@@ -422,6 +422,38 @@ def test_noise_api_contract():
     run(tile, path=binding.PATH_TILE)
 
 
+@pytest.mark.parametrize("path", PATHS)
+def test_back_to_back_steps_overlap_the_order_stage(path, monkeypatch):
+    """The ordered stream of step k is produced on the library's order stream while step k + 1 already runs on the
+    caller's stream (doubled arrival buffers).  Six steps enqueued without any synchronisation must leave the same
+    last-step events, event total and carried state as the same steps synchronised one by one, and as a context
+    with the overlap switched off (EVIS_NO_OVERLAP=1)."""
+    spec = scenes.small(scenes.config(4), num_envs=6, height=130, width=173, num_keyframes=7)
+    sc = scenes.make_scene(spec)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(7)]
+    torch.cuda.synchronize()
+
+    def run(sync_each):
+        ev = binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps,
+                          spec.keyframe_dt, max_motion_px=spec.max_motion_px(), path=_path(path, spec), event_capacity=1 << 24)
+        for kf in kfs:
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=sync_each)
+        last = ev.read_events().copy()
+        info = ev.info()
+        state = ev.get_state()
+        ev.destroy()
+        return last, info.total_events, info.last_holes, state
+
+    a = run(False)
+    b = run(True)
+    monkeypatch.setenv("EVIS_NO_OVERLAP", "1")
+    c = run(False)
+    for other in (b, c):
+        assert len(a[0]) > 0 and np.array_equal(a[0], other[0])
+        assert a[1] == other[1] and a[2] == other[2]
+        assert np.array_equal(a[3][0], other[3][0]) and np.array_equal(a[3][1], other[3][1])
+
+
 def test_margin_api_contract():
     """evis_set_margin: negative or too large margins are INVALID_ARG; margin 0 is the plain frame; coordinates
     of a margin run stay inside the cropped frame; the tile path refuses it."""
