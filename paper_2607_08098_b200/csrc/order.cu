@@ -133,8 +133,9 @@ k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *
 // A block owns ORD_PER_BLOCK consecutive directory entries = one contiguous range of the ordered stream;
 // the directory holds each chunk's event count, so the block scan of those counts places every chunk.
 // Then the warps take chunks one at a time (shared counter): 32 records per pass -- one coalesced 16-byte
-// load per lane --, warp scan of the crossing counts n, and every lane writes the n events of its record
-// (a7: timestamp of the k-th crossing, R8: linear in log intensity between L_prev and L_hat).
+// load per lane --, warp scan of the crossing counts n, and the warp writes the pass's events 32 at a time, one per
+// lane, found by a search over the scan (a7: timestamp of the k-th crossing, R8: linear in log intensity between
+// L_prev and L_hat).
 __global__ void __launch_bounds__(ORD_NT)
 k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__restrict__ bsum,
          const uint4 *__restrict__ arrival, unsigned long long arrival_cap, uint4 *__restrict__ ordered,
@@ -197,33 +198,45 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
                 const uint32_t u = __shfl_up_sync(FULL, incl, dd);
                 if (lane >= dd) incl += u;
             }
-            unsigned long long o = first + (incl - nev);
-            first += __shfl_sync(FULL, incl, 31);
-            if (nev) {
-                const float l_ref = __uint_as_float(rec.x), l_prev = __uint_as_float(rec.y), l_hat = __uint_as_float(rec.z);
-                const bool up = __fsub_rn(l_hat, l_ref) > 0.0f;
-                const uint32_t pos = rec.w & 0xFFFFu;
-                const uint32_t xy = org + (pos % G_TILE_W) + ((pos / G_TILE_W) << 16);
-                float pc = up ? ep.c_pos : -ep.c_neg;                        // p C
-                if (th.on) {                                                 // Eq. 8: the pixel's own thresholds
-                    const size_t pix = (size_t)env * HW + (size_t)(xy >> 16) * W + (xy & 0xFFFFu);
-                    pc = up ? __ldg(th.on + pix) : -__ldg(th.off + pix);
-                }
-                const uint32_t xyc = xy - (margin | (margin << 16));         // coordinates in the cropped frame (R27)
-                const uint32_t w1 = env | ((up ? 0x01u : 0xFFu) << 16) | (sub << 24);
-                // fr_k = (L_ref + k p C - L_prev) / (L_hat - L_prev), clamped to [0, 1]; 1 when the denominator is 0.
-                // Timestamps decide nothing (compared within 1e-7 s; a substep is ~1e-3 s): reciprocal once per record.
-                const float den = __fsub_rn(l_hat, l_prev);
-                const bool flat = !(fabsf(den) > 1e-30f);
-                const float rden = flat ? 0.0f : __fdividef(1.0f, den);
-                float kf = 0.0f;
-                for (uint32_t k = 0; k < nev; ++k, ++o) {
-                    kf += 1.0f;
-                    float fr = __fmul_rn(__fsub_rn(__fmaf_rn(kf, pc, l_ref), l_prev), rden);
-                    fr = flat ? 1.0f : fminf(fmaxf(fr, 0.0f), 1.0f);
-                    if (o < cap) ordered[o] = make_uint4(xyc, w1, __float_as_uint(__fmaf_rn(fr, ep.dt, t0)), ep.kf);
-                }
+            const uint32_t excl = incl - nev, total_ev = __shfl_sync(FULL, incl, 31);
+            // per record, in its own lane: polarity and threshold, cropped position, reciprocal of the denominator
+            const float l_ref = __uint_as_float(rec.x), l_prev = __uint_as_float(rec.y), l_hat = __uint_as_float(rec.z);
+            const bool up = __fsub_rn(l_hat, l_ref) > 0.0f;
+            const uint32_t pos = rec.w & 0xFFFFu;
+            const uint32_t xy = org + (pos % G_TILE_W) + ((pos / G_TILE_W) << 16);
+            float pc = up ? ep.c_pos : -ep.c_neg;                        // p C
+            if (th.on && nev) {                                          // Eq. 8: the pixel's own thresholds
+                const size_t pix = (size_t)env * HW + (size_t)(xy >> 16) * W + (xy & 0xFFFFu);
+                pc = up ? __ldg(th.on + pix) : -__ldg(th.off + pix);
             }
+            const uint32_t xyc = xy - (margin | (margin << 16));         // coordinates in the cropped frame (R27)
+            const uint32_t w1 = env | ((up ? 0x01u : 0xFFu) << 16) | (sub << 24);
+            // fr_k = (L_ref + k p C - L_prev) / (L_hat - L_prev), clamped to [0, 1]; 1 when the denominator is 0.
+            // Timestamps decide nothing (compared within 1e-7 s; a substep is ~1e-3 s): reciprocal once per record;
+            // rden = NaN marks the flat case.
+            const float den = __fsub_rn(l_hat, l_prev);
+            const float rden = fabsf(den) > 1e-30f ? __fdividef(1.0f, den) : __int_as_float(0x7FC00000);
+            // the pass's events, 32 at a time, one per lane: event e belongs to the last lane s with excl[s] <= e
+            // (a 5-step search over the scan), is its crossing k = e - excl[s] + 1, and goes to first + e -- the
+            // stores of a warp are contiguous
+            for (uint32_t e0 = 0; e0 < total_ev; e0 += 32) {
+                const uint32_t e = e0 + lane;
+                int sl = 0;
+#pragma unroll
+                for (int dd = 16; dd >= 1; dd >>= 1) {
+                    const uint32_t tt = __shfl_sync(FULL, excl, sl + dd);
+                    if (tt <= e) sl += dd;
+                }
+                const float kf = (float)(e - __shfl_sync(FULL, excl, sl) + 1u);
+                const float o_ref = __shfl_sync(FULL, l_ref, sl), o_prev = __shfl_sync(FULL, l_prev, sl);
+                const float o_pc = __shfl_sync(FULL, pc, sl), o_rden = __shfl_sync(FULL, rden, sl);
+                const uint32_t o_xy = __shfl_sync(FULL, xyc, sl), o_w1 = __shfl_sync(FULL, w1, sl);
+                float fr = __fmul_rn(__fsub_rn(__fmaf_rn(kf, o_pc, o_ref), o_prev), o_rden);
+                fr = o_rden != o_rden ? 1.0f : fminf(fmaxf(fr, 0.0f), 1.0f);
+                const unsigned long long o = first + e;
+                if (e < total_ev && o < cap) ordered[o] = make_uint4(o_xy, o_w1, __float_as_uint(__fmaf_rn(fr, ep.dt, t0)), ep.kf);
+            }
+            first += total_ev;
         }
     }
 }
