@@ -12,6 +12,13 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 
 
+def pytest_sessionstart(session):
+    """The tests call the C-ABI library in-tree: (re)build it when it is missing or older than its sources (an
+    incremental nvcc build, a no-op when up to date).  A failing build fails the session loudly."""
+    from paper_2607_08098_b200 import build as cuda_build
+    cuda_build.build()
+
+
 def pytest_collection_modifyitems(config, items):
     try:
         import torch
