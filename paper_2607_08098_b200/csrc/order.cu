@@ -212,10 +212,13 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
             const uint32_t xyc = xy - (margin | (margin << 16));         // coordinates in the cropped frame (R27)
             const uint32_t w1 = env | ((up ? 0x01u : 0xFFu) << 16) | (sub << 24);
             // fr_k = (L_ref + k p C - L_prev) / (L_hat - L_prev), clamped to [0, 1]; 1 when the denominator is 0.
-            // Timestamps decide nothing (compared within 1e-7 s; a substep is ~1e-3 s): reciprocal once per record;
-            // rden = NaN marks the flat case.
+            // Timestamps decide nothing (compared within 1e-7 s; a substep is ~1e-3 s): reciprocal once per record.
+            // A zero denominator (fr = 1) is encoded as rden = +inf with L_prev = -inf: (lev + inf) * inf clamps to 1;
+            // a NaN denominator (non-finite L) gives fr = NaN -> 0, like the oracle's !(fr >= 0).
             const float den = __fsub_rn(l_hat, l_prev);
-            const float rden = fabsf(den) > 1e-30f ? __fdividef(1.0f, den) : __int_as_float(0x7FC00000);
+            const bool flat = den == 0.0f;
+            const float rden = flat ? __int_as_float(0x7F800000) : __fdividef(1.0f, den);
+            const float l_prev_e = flat ? __int_as_float(0xFF800000) : l_prev;
             // the pass's events, 32 at a time, one per lane: event e belongs to the last lane s with excl[s] <= e
             // (a 5-step search over the scan), is its crossing k = e - excl[s] + 1, and goes to first + e -- the
             // stores of a warp are contiguous
@@ -228,11 +231,11 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
                     if (tt <= e) sl += dd;
                 }
                 const float kf = (float)(e - __shfl_sync(FULL, excl, sl) + 1u);
-                const float o_ref = __shfl_sync(FULL, l_ref, sl), o_prev = __shfl_sync(FULL, l_prev, sl);
+                const float o_ref = __shfl_sync(FULL, l_ref, sl), o_prev = __shfl_sync(FULL, l_prev_e, sl);
                 const float o_pc = __shfl_sync(FULL, pc, sl), o_rden = __shfl_sync(FULL, rden, sl);
                 const uint32_t o_xy = __shfl_sync(FULL, xyc, sl), o_w1 = __shfl_sync(FULL, w1, sl);
                 float fr = __fmul_rn(__fsub_rn(__fmaf_rn(kf, o_pc, o_ref), o_prev), o_rden);
-                fr = o_rden != o_rden ? 1.0f : fminf(fmaxf(fr, 0.0f), 1.0f);
+                fr = fminf(fmaxf(fr, 0.0f), 1.0f);
                 const unsigned long long o = first + e;
                 if (e < total_ev && o < cap) ordered[o] = make_uint4(o_xy, o_w1, __float_as_uint(__fmaf_rn(fr, ep.dt, t0)), ep.kf);
             }

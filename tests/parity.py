@@ -90,7 +90,10 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
         win, d, lh = win[inner], d[inner], lh[inner]
         bad = (d != o_dir) | (win != o_idx)
         rep.winner_mismatch += int(bad.sum())
-        rep.max_dL = max(rep.max_dL, float(np.max(np.abs(lh.astype(np.float64) - o_lh))))
+        fin = np.isfinite(o_lh)                    # non-finite L (infinite radiance) must agree as such
+        assert np.array_equal(fin, np.isfinite(lh)) and np.array_equal(lh[~fin], o_lh[~fin], equal_nan=True)
+        if fin.any():
+            rep.max_dL = max(rep.max_dL, float(np.max(np.abs(lh[fin].astype(np.float64) - o_lh[fin]))))
         rep.holes += int((o_dir == 3).sum())
 
     # --- events: multiset per (env, substep, y, x, polarity) -----------------------------------
@@ -129,7 +132,7 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
 def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Sequence[int]] = None,
                mode: int = 0, path: int = binding.PATH_GLOBAL, use_fwd: bool = True, debug: bool = True,
                capacity: int = 1 << 24, max_motion: Optional[float] = None, thresholds=None,
-               tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None) -> ParityReport:
+               tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None, mutate=None) -> ParityReport:
     """GPU runs the whole batch; the oracle runs ``envs`` (default: all).  Returns the report after
     asserting every bit-exact criterion; tolerances are asserted by the caller on the report."""
     sc = scenes.make_scene(spec)
@@ -156,6 +159,8 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
     try:
         for k in range(n_keyframes):
             kf = scenes.render_keyframe(sc, k, device="cuda")
+            if mutate is not None:                  # degenerate-input cases: the test edits the keyframe in place
+                mutate(k, kf)
             fwd = kf["mv_fwd"] if use_fwd else None
             n = ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=fwd, sync=True)
             h = {key: v[sel].cpu().numpy() for key, v in kf.items()}

@@ -454,6 +454,34 @@ def test_back_to_back_steps_overlap_the_order_stage(path, monkeypatch):
         assert np.array_equal(a[3][0], other[3][0]) and np.array_equal(a[3][1], other[3][1])
 
 
+@pytest.mark.parametrize("use_fwd", [True, False])
+def test_degenerate_inputs(use_fwd):
+    """Inputs the readings R3, R17 and R18 cover: negative, NaN and infinite radiance (luminance clamps to 0, NaN -> 0);
+    depth that is 0, negative, +inf or NaN (the source is skipped); motion vectors that are NaN, infinite or huge
+    (the source lands nowhere).  Sprinkled over ~3 % of the pixels of every keyframe of a config-2 style scene, the
+    GPU must still match the oracle bit for bit: winners, holes, events, L_ref."""
+    spec = scenes.small(scenes.config(2), num_envs=2, height=101, width=135, num_keyframes=4)
+    gen = torch.Generator(device="cuda").manual_seed(77)
+
+    def mutate(k, kf):
+        E, H, W = kf["depth"].shape
+        pick = lambda frac: torch.rand((E, H, W), generator=gen, device="cuda") < frac
+        bad_r = torch.tensor([-3.0, float("nan"), float("inf"), 0.0], device="cuda")
+        m = pick(0.01)
+        kf["rad"][m] = bad_r[torch.randint(0, 4, (int(m.sum()), 3), generator=gen, device="cuda")]
+        bad_z = torch.tensor([0.0, -2.0, float("inf"), float("nan")], device="cuda")
+        m = pick(0.01)
+        kf["depth"][m] = bad_z[torch.randint(0, 4, (int(m.sum()),), generator=gen, device="cuda")]
+        bad_m = torch.tensor([float("nan"), float("inf"), -float("inf"), 1e9, -3e5], device="cuda")
+        for key in ("mv_bwd", "mv_fwd"):
+            m = pick(0.01)
+            kf[key][m] = bad_m[torch.randint(0, 5, (int(m.sum()), 2), generator=gen, device="cuda")]
+
+    rep = parity.run_parity(spec, 4, path=binding.PATH_GLOBAL, use_fwd=use_fwd, mutate=mutate)
+    _assert_tolerances(rep)
+    assert rep.holes > 0
+
+
 def test_margin_api_contract():
     """evis_set_margin: negative or too large margins are INVALID_ARG; margin 0 is the plain frame; coordinates
     of a margin run stay inside the cropped frame; the tile path refuses it."""
