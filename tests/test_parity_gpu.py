@@ -155,6 +155,22 @@ def test_blend_mode_global():
     _assert_tolerances(rep)
 
 
+def test_maximum_substeps_255():
+    """S = 255, the largest substep count the ABI admits (substep index in 8 bits), with fast motion."""
+    spec = scenes.SceneSpec("s255", 2, 48, 61, 3, 1.0 / 30.0, 255, 0.15, 0.2, num_rects=5, v_max=900.0, seed=9)
+    rep = parity.run_parity(spec, 3, path=binding.PATH_GLOBAL)
+    _assert_tolerances(rep)
+
+
+def test_frame_larger_than_2_pow_24_pixels():
+    """A 4100 x 4100 frame (1.68e7 pixels > 2^24): the source index no longer fits the tagged key's 24 bits, so
+    the library must take the untagged [dir | Zt | 32-bit index] keys on its own; winners from the far end of the
+    index range must survive.  One env, S = 2."""
+    spec = scenes.SceneSpec("big", 1, 4100, 4100, 2, 1.0 / 60.0, 2, 0.2, 0.2, num_rects=8, v_max=600.0, seed=21)
+    rep = parity.run_parity(spec, 2, path=binding.PATH_AUTO, capacity=1 << 26)
+    _assert_tolerances(rep)
+
+
 def test_large_s_166():
     spec = scenes.SceneSpec("s166", 2, 90, 120, 3, 1.0 / 60.0, 166, 0.2, 0.2, num_rects=6, v_max=300.0, seed=5)
     rep = parity.run_parity(spec, 3, path=binding.PATH_GLOBAL)
