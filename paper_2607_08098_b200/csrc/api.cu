@@ -93,7 +93,10 @@ struct evis_ctx {
 
 namespace {
 
-enum { C_EVENTS = 0, C_HOLES = 1, C_ALLOC = 2, C_ITEM = 3, C_MOTION = 4, C_TOTAL = 5, NCOUNTERS = 6 };
+// Device counters, one per 128-byte line: the arrival reservation (C_ALLOC) is on every resolve block's critical
+// path and must not queue behind the event / hole tallies in the same L2 sector.  [0, C_STEP_END) are reset
+// every step; C_MOTION and C_TOTAL are sticky.
+enum { C_EVENTS = 0, C_HOLES = 16, C_ALLOC = 32, C_ITEM = 48, C_STEP_END = 64, C_MOTION = 64, C_TOTAL = 80, NCOUNTERS = 96 };
 
 struct DeviceGuard {
     int prev;
@@ -504,7 +507,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     }
     {
         Span sp(ctx, st, EVIS_STAGE_CLEAR, 2);
-        CU(cudaMemsetAsync(cnt, 0, 4 * sizeof(unsigned long long), st));   // the per-step counters
+        CU(cudaMemsetAsync(cnt, 0, C_STEP_END * sizeof(unsigned long long), st));   // the per-step counters
         CU(cudaMemsetAsync(sink.directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
     }
 
@@ -583,8 +586,8 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
             CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
                             cnt + C_EVENTS, sticky + C_TOTAL, os));
         }
-        CU(cudaMemcpyAsync(ctx->h_counters, cnt, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, os));
-        CU(cudaMemcpyAsync(ctx->h_counters + C_MOTION, sticky + C_MOTION, 2 * sizeof(unsigned long long),
+        CU(cudaMemcpyAsync(ctx->h_counters, cnt, C_STEP_END * sizeof(unsigned long long), cudaMemcpyDeviceToHost, os));
+        CU(cudaMemcpyAsync(ctx->h_counters + C_MOTION, sticky + C_MOTION, (NCOUNTERS - C_MOTION) * sizeof(unsigned long long),
                            cudaMemcpyDeviceToHost, os));
     }
     CU(cudaEventRecord(ctx->ev_order[sl], os));
