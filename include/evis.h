@@ -210,6 +210,11 @@ int evis_profile_read(evis_ctx *ctx, evis_profile *out);
  * warped log frame L_prev, each [E,H,W] float32, to/from HOST memory.  Either may be NULL. */
 int evis_get_state(evis_ctx *ctx, float *l_ref, float *l_prev);
 int evis_set_state(evis_ctx *ctx, const float *l_ref, const float *l_prev);
+/* The third piece of carried state, when the refractory period (or the noise events) is on: t_last [E,H,W] float32,
+ * the timestamp of each pixel's last emitted event relative to the start of the NEXT interval (-inf: none yet; pixels
+ * cropped by the margin keep their initial value).  Exactly one of the HOST pointers is given: get copies it out, set
+ * copies it in.  Errors: INVALID_ARG, BAD_STATE (neither feature has been switched on), CUDA. */
+int evis_refractory_state(evis_ctx *ctx, float *get_t_last, const float *set_t_last);
 
 /* Test hook (needs debug_capture = 1): for the last step, per substep i-1 in [0,S), per pixel:
  *   win   [S,E,H,W] uint32: source linear index y*W+x of the composite winner, 0xFFFFFFFF = hole

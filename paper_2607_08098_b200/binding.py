@@ -53,7 +53,7 @@ class evis_profile(C.Structure):
 # every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
-           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events"]
+           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state"]
 
 _lib = None
 
@@ -87,6 +87,7 @@ def load() -> C.CDLL:
     L.evis_set_margin.argtypes = [vp, C.c_int]
     L.evis_set_channel.argtypes = [vp, C.c_int]
     L.evis_wait_events.argtypes = [vp, vp]
+    L.evis_refractory_state.argtypes = [vp, vp, vp]
     L.evis_set_noise.argtypes = [vp, C.POINTER(evis_noise), vp, C.c_int]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
@@ -267,6 +268,16 @@ class Evis:
         lref, lprev = np.empty(shp, np.float32), np.empty(shp, np.float32)
         _check(self._lib.evis_get_state(self._ctx, lref.ctypes.data, lprev.ctypes.data), "evis_get_state")
         return lref, lprev
+
+    def get_t_last(self) -> np.ndarray:
+        """evis_refractory_state (get): stamps of the last emitted events, relative to the next interval's start."""
+        out = np.empty((self.E, self.H, self.W), np.float32)
+        _check(self._lib.evis_refractory_state(self._ctx, out.ctypes.data, None), "evis_refractory_state")
+        return out
+
+    def set_t_last(self, t_last: np.ndarray) -> None:
+        _check(self._lib.evis_refractory_state(self._ctx, None, _host_ptr(t_last, (self.E, self.H, self.W), "t_last")),
+               "evis_refractory_state")
 
     def set_state(self, l_ref: Optional[np.ndarray], l_prev: Optional[np.ndarray]) -> None:
         shp = (self.E, self.H, self.W)

@@ -834,6 +834,18 @@ int evis_get_state(evis_ctx *ctx, float *l_ref, float *l_prev)
     return EVIS_OK;
 }
 
+int evis_refractory_state(evis_ctx *ctx, float *get_t_last, const float *set_t_last)
+{
+    if (!ctx || (get_t_last && set_t_last)) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->t_last) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    CU(sync_all(ctx));
+    const size_t bytes = (size_t)ctx->g.E * ctx->g.HW * sizeof(float);
+    if (get_t_last) CU(cudaMemcpy(get_t_last, ctx->t_last, bytes, cudaMemcpyDeviceToHost));
+    if (set_t_last) CU(cudaMemcpy(ctx->t_last, set_t_last, bytes, cudaMemcpyHostToDevice));
+    return EVIS_OK;
+}
+
 int evis_set_state(evis_ctx *ctx, const float *l_ref, const float *l_prev)
 {
     if (!ctx) return EVIS_ERR_INVALID_ARG;

@@ -177,6 +177,8 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
             if rep.ties == 0:
                 assert np.array_equal(lref[sel][inner], ora.Lref[inner]), "carried L_ref differs"
             assert np.allclose(lprev[sel][inner], ora.Lprev[inner], atol=TOL_L, rtol=0)
+            if tau_r > 0.0 and rep.ties == 0:       # the carried refractory state, bit for bit (R26)
+                assert np.array_equal(ev.get_t_last()[sel][inner], ora.t_last[inner]), "carried t_last differs"
             info = ev.info()
             if envs is None:
                 assert info.last_holes == ora.holes

@@ -545,6 +545,37 @@ def test_margin_api_contract():
     run(tile, path=binding.PATH_TILE)
 
 
+def test_checkpoint_resume_with_refractory_state():
+    """Checkpoint / resume: L_ref, L_prev (evis_get_state) and t_last (evis_refractory_state) taken after step 3 and
+    put into a fresh context -- together with keyframe 3 as its first keyframe -- reproduce steps 4 and 5 exactly."""
+    spec = scenes.small(scenes.config(4), num_envs=2, height=97, width=131, num_keyframes=6)
+    sc = scenes.make_scene(spec)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(6)]
+    mk = lambda: binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps,
+                              spec.keyframe_dt, path=binding.PATH_GLOBAL, event_capacity=1 << 24)
+    step = lambda ev, k: ev.step(kfs[k]["rad"], kfs[k]["mv_bwd"], kfs[k]["depth"], mv_fwd=kfs[k]["mv_fwd"], sync=True)
+    a = mk(); a.set_refractory(0.003)
+    for k in range(4):
+        step(a, k)
+    lref, lprev = a.get_state()
+    tl = a.get_t_last()
+    want = []
+    for k in (4, 5):
+        step(a, k); want.append(a.read_events().copy())
+    a.destroy()
+    b = mk(); b.set_refractory(0.003)
+    with pytest.raises(binding.EvisError):
+        mk().get_t_last()                                             # BAD_STATE: the feature is off
+    step(b, 3)
+    b.set_state(lref, lprev); b.set_t_last(tl)
+    for i, k in enumerate((4, 5)):
+        step(b, k)
+        got = b.read_events().copy()
+        got["kf"] = want[i]["kf"]                                     # interval numbering restarts in the new context
+        assert len(got) > 0 and np.array_equal(got, want[i])
+    b.destroy()
+
+
 def test_refractory_api_contract():
     """evis_set_refractory: negative or non-finite tau_r is INVALID_ARG; tau_r = 0 restores the plain stream; the
     tile path refuses it."""
