@@ -195,6 +195,14 @@ int evis_set_refractory(evis_ctx *ctx, float tau_r);
  * (= min(true count, capacity, max)).  Errors: INVALID_ARG, BAD_STATE, CUDA. */
 int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t max, uint64_t *n_out);
 
+/* The same copy to HOST memory (pinned, for a real overlap) in two halves, so that the next evis_step_host can upload
+ * its keyframe while the events of this step go down the other direction of the link: _begin waits for the step,
+ * stores the number of events that will be copied in *n_out, starts the copy on a stream of the library's own and
+ * returns; _end waits for it.  `host_dst` must stay untouched until _end; the next step's ordered stream is not
+ * produced before the copy has finished.  A second _begin ends the first.  Errors: INVALID_ARG, BAD_STATE, CUDA. */
+int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, uint64_t *n_out);
+int evis_read_events_end(evis_ctx *ctx);
+
 /* Device pointer to the ordered stream of the last step and its stored length (no copy);
  * valid until the next evis_step on the same context. */
 int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_stored);

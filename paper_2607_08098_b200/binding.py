@@ -53,7 +53,7 @@ class evis_profile(C.Structure):
 # every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
-           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state"]
+           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end"]
 
 _lib = None
 
@@ -87,6 +87,8 @@ def load() -> C.CDLL:
     L.evis_set_margin.argtypes = [vp, C.c_int]
     L.evis_set_channel.argtypes = [vp, C.c_int]
     L.evis_wait_events.argtypes = [vp, vp]
+    L.evis_read_events_begin.argtypes = [vp, vp, C.c_uint64, u64p]
+    L.evis_read_events_end.argtypes = [vp]
     L.evis_refractory_state.argtypes = [vp, vp, vp]
     L.evis_set_noise.argtypes = [vp, C.POINTER(evis_noise), vp, C.c_int]
     L.evis_last_cuda_error.argtypes = [vp]
@@ -239,6 +241,16 @@ class Evis:
         _check(self._lib.evis_read_events(self._ctx, host_buf.ctypes.data, 0, host_buf.shape[0], C.byref(got)),
                "evis_read_events")
         return int(got.value)
+
+    def read_events_begin(self, host_buf: np.ndarray) -> int:
+        """evis_read_events_begin: start copying the last step's events into a (pinned) host buffer; returns their number."""
+        got = C.c_uint64(0)
+        _check(self._lib.evis_read_events_begin(self._ctx, host_buf.ctypes.data, host_buf.shape[0], C.byref(got)),
+               "evis_read_events_begin")
+        return int(got.value)
+
+    def read_events_end(self) -> None:
+        _check(self._lib.evis_read_events_end(self._ctx), "evis_read_events_end")
 
     def events_device(self) -> Tuple[int, int]:
         """(device pointer, stored count) of the ordered stream of the last step; no copy."""

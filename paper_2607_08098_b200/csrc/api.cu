@@ -62,6 +62,9 @@ struct evis_ctx {
     uint2 *directory_s[2];
     unsigned long long *counters_s[2];
     cudaStream_t ord_stream;
+    cudaStream_t copy_stream;         // evis_read_events_begin: device -> host copy of the ordered stream
+    cudaEvent_t ev_copy;
+    bool copy_pending;
     cudaEvent_t ev_chunks[2], ev_order[2];
     bool ord_pending[2];
     bool overlap;
@@ -205,6 +208,8 @@ void free_all(evis_ctx *ctx)
         cudaFree(ctx->arrival_s[1]); cudaFree(ctx->directory_s[1]); cudaFree(ctx->counters_s[1]);
     }
     if (ctx->ord_stream) cudaStreamDestroy(ctx->ord_stream);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->ev_copy) cudaEventDestroy(ctx->ev_copy);
     for (int k = 0; k < 2; ++k) {
         if (ctx->ev_chunks[k]) cudaEventDestroy(ctx->ev_chunks[k]);
         if (ctx->ev_order[k]) cudaEventDestroy(ctx->ev_order[k]);
@@ -357,6 +362,8 @@ int create_impl(evis_ctx *ctx)
             CU(cudaMemset(ctx->counters_s[1], 0, NCOUNTERS * sizeof(unsigned long long)));
         }
         CU(cudaStreamCreateWithFlags(&ctx->ord_stream, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ctx->ev_copy, cudaEventDisableTiming));
         for (int k = 0; k < 2; ++k) {
             CU(cudaEventCreateWithFlags(&ctx->ev_chunks[k], cudaEventDisableTiming));
             CU(cudaEventCreateWithFlags(&ctx->ev_order[k], cudaEventDisableTiming));
@@ -574,6 +581,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     cudaStream_t os = ctx->ord_stream;
     CU(cudaEventRecord(ctx->ev_chunks[sl], st));
     CU(cudaStreamWaitEvent(os, ctx->ev_chunks[sl], 0));
+    if (ctx->copy_pending) CU(cudaStreamWaitEvent(os, ctx->ev_copy, 0));   // `ordered` is still being copied out
     {
         Span sp(ctx, os, EVIS_STAGE_ORDER, 3);
         unsigned long long *sticky = ctx->counters_s[0];             // C_MOTION, C_TOTAL live in slot 0's array
@@ -766,6 +774,37 @@ int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t
     if (n) CU(cudaMemcpy(dst, ctx->ordered, n * sizeof(evis_event),
                          dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
     if (n_out) *n_out = n;
+    return EVIS_OK;
+}
+
+int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, uint64_t *n_out)
+{
+    if (!ctx || (!host_dst && max > 0)) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->have_events) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    const int rc = fetch_counters(ctx);
+    if (rc != EVIS_OK) return rc;
+    if (ctx->copy_pending) CU(cudaStreamSynchronize(ctx->copy_stream));
+    uint64_t n = ctx->last_events;
+    if (n > ctx->cfg.event_capacity) n = ctx->cfg.event_capacity;
+    if (n > max) n = max;
+    if (n) {
+        CU(cudaMemcpyAsync(host_dst, ctx->ordered, n * sizeof(evis_event), cudaMemcpyDeviceToHost, ctx->copy_stream));
+        CU(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
+        ctx->copy_pending = true;
+    }
+    if (n_out) *n_out = n;
+    return EVIS_OK;
+}
+
+int evis_read_events_end(evis_ctx *ctx)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->copy_pending) CU(cudaStreamSynchronize(ctx->copy_stream));
+    ctx->copy_pending = false;
     return EVIS_OK;
 }
 

@@ -576,6 +576,34 @@ def test_checkpoint_resume_with_refractory_state():
     b.destroy()
 
 
+def test_split_host_read_matches_the_plain_one():
+    """evis_read_events_begin / _end (copy overlapping the next upload) return the same events as evis_read_events,
+    step after step, while the next evis_step_host is already running."""
+    spec = scenes.small(scenes.config(4), num_envs=4, height=130, width=173, num_keyframes=5)
+    sc = scenes.make_scene(spec)
+    kfs = [{k: v.numpy() for k, v in scenes.render_keyframe(sc, i).items()} for i in range(5)]
+    mk = lambda: binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps,
+                              spec.keyframe_dt, path=binding.PATH_GLOBAL, event_capacity=1 << 24)
+    a, b = mk(), mk()
+    bufs = [torch.empty((1 << 24, 16), dtype=torch.uint8).pin_memory().numpy().view(binding.EVENT_DTYPE).reshape(-1)
+            for _ in range(2)]
+    plain, split, pending = [], [], None
+    for i, f in enumerate(kfs):
+        a.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
+        plain.append(a.read_events().copy())
+        b.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])      # runs while the previous copy may be in flight
+        if pending is not None:
+            b.read_events_end()
+            split.append(bufs[pending[0]][:pending[1]].copy())
+        pending = (i & 1, b.read_events_begin(bufs[i & 1]))
+    b.read_events_end()
+    split.append(bufs[pending[0]][:pending[1]].copy())
+    a.destroy(); b.destroy()
+    assert len(plain) == len(split) == 5 and sum(len(x) for x in plain) > 0
+    for x, y in zip(plain, split):
+        assert np.array_equal(x, y)
+
+
 def test_refractory_api_contract():
     """evis_set_refractory: negative or non-finite tau_r is INVALID_ARG; tau_r = 0 restores the plain stream; the
     tile path refuses it."""
