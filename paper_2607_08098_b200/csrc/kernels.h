@@ -81,7 +81,10 @@ constexpr int TMAP_BYTES = 128;    // sizeof(CUtensorMap)
 // of one resolve tile).  Returns false when the driver entry point is unavailable.
 bool make_z_tensor_maps(const Geom &g, unsigned long long *zd, unsigned long long *zc, size_t planes, void *tmap_d,
                         void *tmap_c);
-constexpr int G_TILE_W = 32, G_TILE_H = 16;    // ordering tile of the global path
+#ifndef EVIS_TILE_H
+#define EVIS_TILE_H 16
+#endif
+constexpr int G_TILE_W = 32, G_TILE_H = EVIS_TILE_H;    // ordering tile of the global path
 // The global path leaves RECORDS in the arrival buffer, one uint4 per firing pixel-substep:
 //   x, y, z = bits of L_ref (before the update), L_prev, L_hat;  w = raster position in the tile | n << 16
 // and directory entries (record offset, records | events << DIR_EV_SHIFT); order.cu expands them.
