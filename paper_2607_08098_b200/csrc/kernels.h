@@ -97,6 +97,16 @@ cudaError_t launch_global_resolve(const Geom &g, const ZChunk &zc, const Keyfram
                                   const SubstepTable &tab, float *l_ref, float *l_prev,
                                   const EventParams &ep, const Thresholds &th, const Refractory &rf,
                                   const EventSink &sink, unsigned long long *holes, const DebugOut &dbg, cudaStream_t st);
+// its four instantiation units (resolve_m*.cu): composite mode 0 / 1, without / with the debug capture
+#define EVIS_DECL_RESOLVE(name)                                                                                     \
+    cudaError_t name(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B, const SubstepTable &tab,  \
+                     float *l_ref, float *l_prev, const EventParams &ep, const Thresholds &th, const Refractory &rf, \
+                     const EventSink &sink, unsigned long long *holes, const DebugOut &dbg, cudaStream_t st)
+EVIS_DECL_RESOLVE(launch_resolve_m0);
+EVIS_DECL_RESOLVE(launch_resolve_m0d);
+EVIS_DECL_RESOLVE(launch_resolve_m1);
+EVIS_DECL_RESOLVE(launch_resolve_m1d);
+#undef EVIS_DECL_RESOLVE
 // fill n floats with v (prep.cu)
 cudaError_t launch_fill(float *p, long long n, float v, cudaStream_t st);
 
