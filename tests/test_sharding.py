@@ -42,7 +42,7 @@ def test_two_gloo_ranks_reduce_max_time_and_sum_counters():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
         port = s.getsockname()[1]
-    mgr = mp.Manager()
+    mgr = mp.get_context("spawn").Manager()        # not fork(): the test process is multi-threaded
     out = mgr.dict()
     mp.spawn(_worker, args=(2, port, out), nprocs=2, join=True)
     assert out[0][:2] == out[1][:2]
