@@ -33,7 +33,7 @@ ALGO_BYTES_PER_PIXEL = 52          # per pixel per keyframe interval, DESIGN.md 
 ALGO_BYTES_PER_EVENT = 16
 FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 ISSUE_PEAK = 148 * 4 * 32 * 1.965e9   # thread-instructions/s: SMs x schedulers x lanes x clocks.max.sm
-INSTR_PER_PXSS = 191.0                # issued thread-instruction slots per pixel-substep (ncu, profiles/r03_README.md)
+INSTR_PER_PXSS = 189.0                # issued thread-instruction slots per pixel-substep (ncu, profiles/r03_README.md)
 
 
 def ncu_traffic(workload: str, stage: str):
@@ -297,7 +297,7 @@ def run_ours(args, spec) -> None:
                 "launch_ms": stage_ms[dom] / dom_launches, "launches_per_step": dom_launches,
                 "stage_ms_per_step": stage_ms, "stage_launches_per_step": {k: v / K for k, v in prof["launches"].items()},
                 "whole_step_frac": algo_bytes_step / (ms / K * 1e-3) / 1e9 / peak,
-                # the binding roof: issued thread-instruction slots, ~191 per pixel-substep
+                # the binding roof: issued thread-instruction slots, ~189 per pixel-substep
                 "issue_roof": {"bound": "alu", "unit": "thread-instr/s", "peak": ISSUE_PEAK,
                                "instr_per_pixel_substep": INSTR_PER_PXSS,
                                "achieved": INSTR_PER_PXSS * pxss_step / (ms / K * 1e-3),
