@@ -186,7 +186,10 @@ def workload_config(spec, path: str) -> dict:
     return {"workload": spec.name, "envs": spec.num_envs, "height": spec.height, "width": spec.width,
             "substeps": spec.substeps, "keyframe_hz": round(1.0 / spec.keyframe_dt, 3),
             "c_pos": spec.c_pos, "c_neg": spec.c_neg, "log_eps": spec.log_eps, "path": path,
-            "l2": "inputs larger than L2 (one keyframe >= 126 MB), no flush" }
+            "l2": ("inputs larger than L2 (one keyframe = %d MB >= 126 MB, a new one every step), no flush" if
+                   spec.num_envs * spec.height * spec.width * 32 >= 126 << 20 else
+                   "one keyframe = %d MB < L2 (126 MB), a new one every step, no flush: a parity-size config, not the "
+                   "bench workload") % (spec.num_envs * spec.height * spec.width * 32 >> 20)}
 
 
 # ------------------------------------------------------------------------------------------------
