@@ -263,41 +263,40 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
                 float r = floorf(fabsf(d) / C);
                 n = r >= 255.0f ? 255 : (int)r;
             }
-            for (int k = 1; k <= n && tau_r > 0.0f; ++k) {
-                /* Refractory period [R26]: the crossing is stamped in binary32 (the stamp now
-                 * decides an integer: emitted or not) with the operation order below, and it is emitted iff
-                 * t - t_last >= tau_r, t_last = stamp of the pixel's last EMITTED event, kept relative to the
-                 * start of the current interval.  L_ref follows every crossing, emitted or not (Eq. 4).       */
-                const float dtf = T / (float)S;
+            for (int k = 1; k <= n; ++k) {
+                /* the k-th crossing of this frame: level_k = Lref + p k C, placed at the fraction fr of the frame
+                 * where the line from Lprev to L reaches it [R8]; fr = 1 when the frame did not move.            */
                 const float lev = fmaf((float)(p * k), C, Lref[q]);
-                const float num = lev - Lprev[q], den = L - Lprev[q];
-                float fr = 1.0f;
-                if (den != 0.0f) fr = num / den;
-                if (!(fr >= 0.0f)) fr = 0.0f;
-                if (fr > 1.0f) fr = 1.0f;
-                const float t = fmaf(fr, dtf, (float)(i - 1) * dtf);
-                if (!(t - t_last[q] >= tau_r)) continue;              /* suppressed */
-                t_last[q] = t;
-                if (n_have + made < cap) {
-                    evo_event *o = &ev[n_have + made];
-                    o->env = env; o->x = x; o->y = y; o->p = p; o->substep = i; o->k = k;
-                    o->kf = kf; o->pad = 0;
-                    o->t_off = (double)t;
+                double t;
+                if (tau_r > 0.0f) {
+                    /* Refractory period [R26]: the stamp now decides an integer (emitted or not), so
+                     * it is taken in binary32 with this operation order; the crossing is emitted iff
+                     * t - t_last >= tau_r, t_last = stamp of the pixel's last EMITTED event, kept relative to the
+                     * start of the current interval.  L_ref follows every crossing, emitted or not (Eq. 4).      */
+                    const float dtf = T / (float)S;
+                    const float num = lev - Lprev[q], den = L - Lprev[q];
+                    float fr = 1.0f;
+                    if (den != 0.0f) fr = num / den;
+                    if (!(fr >= 0.0f)) fr = 0.0f;
+                    if (fr > 1.0f) fr = 1.0f;
+                    const float tf = fmaf(fr, dtf, (float)(i - 1) * dtf);
+                    if (!(tf - t_last[q] >= tau_r)) continue;         /* suppressed */
+                    t_last[q] = tf;
+                    t = (double)tf;
+                } else {
+                    /* the stamp decides nothing: binary64 */
+                    const double den = (double)L - (double)Lprev[q];
+                    double fr = 1.0;
+                    if (den != 0.0) fr = ((double)lev - (double)Lprev[q]) / den;
+                    if (!(fr >= 0.0)) fr = 0.0;
+                    if (fr > 1.0) fr = 1.0;
+                    t = ((double)(i - 1) + fr) * dt;
                 }
-                ++made;
-            }
-            for (int k = 1; k <= n && !(tau_r > 0.0f); ++k) {
-                const float lev = fmaf((float)(p * k), C, Lref[q]);
-                const double den = (double)L - (double)Lprev[q];
-                double fr = 1.0;
-                if (den != 0.0) fr = ((double)lev - (double)Lprev[q]) / den;
-                if (!(fr >= 0.0)) fr = 0.0;
-                if (fr > 1.0) fr = 1.0;
                 if (n_have + made < cap) {
                     evo_event *o = &ev[n_have + made];
                     o->env = env; o->x = x; o->y = y; o->p = p; o->substep = i; o->k = k;
                     o->kf = kf; o->pad = 0;
-                    o->t_off = ((double)(i - 1) + fr) * dt;
+                    o->t_off = t;
                 }
                 ++made;
             }
