@@ -22,7 +22,8 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 zero motion identity, P2 substep S reproduces
  * keyframe B, P3 integer translation, P4 8x8 gather-form brute force, P5 analytic two-rectangle
- * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8), P12 refractory period, P13 margin, P14 colour, P15 noise events.  UNPINNED by paper or
+ * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8), P12 refractory period, P13 margin, P14 colour, P15 noise events,
+ * P16 composite mode 1 (every case of the rule by hand; linear time ramp along a translation).  UNPINNED by paper or
  * mathematics (fixed by DESIGN.md readings only): log base R1, epsilon R2, initial reference
  * level R6, nearest-pixel depth lookup R16, hole handling R20, the composite choice R19, and among the
  * non-idealities the choices of R26 (L_ref follows suppressed crossings) and R29 (Ibar's normalisation, stamps,

@@ -91,6 +91,21 @@ def splat(i: int, S: int, src_is_B: bool, disp: np.ndarray, Zsrc: np.ndarray, Zo
     return z
 
 
+def composite(i: int, S: int, mode: int, zA: np.ndarray, zB: np.ndarray, LA: np.ndarray, LB: np.ndarray,
+              Lprev: np.ndarray):
+    """The composite rule (R19) for one env and one substep from the two z-buffers [H,W] uint64 of
+    ``splat`` and the log frames [H,W].  Returns (Lhat float32, dir uint8: 0 B / 1 A / 2 blend / 3 hole, idx uint32)."""
+    H, W = zA.shape
+    Lhat = np.empty((H, W), np.float32)
+    d = np.empty((H, W), np.uint8)
+    idx = np.empty((H, W), np.uint32)
+    lib().evo_composite(H, W, i, S, int(mode), _p(np.ascontiguousarray(zA, np.uint64), C.c_uint64),
+                        _p(np.ascontiguousarray(zB, np.uint64), C.c_uint64),
+                        _f(np.ascontiguousarray(LA, np.float32)), _f(np.ascontiguousarray(LB, np.float32)),
+                        _f(np.ascontiguousarray(Lprev, np.float32)), _f(Lhat), _p(d, C.c_uint8), _p(idx, C.c_uint32))
+    return Lhat, d, idx
+
+
 def event_frames(frames: np.ndarray, L0: np.ndarray, c_pos: float, c_neg: float, T: float,
                  Lref0: Optional[np.ndarray] = None, theta_on: Optional[np.ndarray] = None,
                  theta_off: Optional[np.ndarray] = None, tau_r: float = 0.0, t_last0: Optional[np.ndarray] = None,

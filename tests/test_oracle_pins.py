@@ -177,6 +177,87 @@ def test_p3b_composite_through_the_full_interval():
 
 
 # ------------------------------------------------------------------------------------------------
+# P16: composite mode 1 (R19): nearest of the two winners; the time-weighted blend where both hit the same surface
+# ------------------------------------------------------------------------------------------------
+def _key(z, idx):
+    return (np.uint64(np.float32(z).view(np.uint32)) << np.uint64(32)) | np.uint64(idx)
+
+
+def test_p16_blend_mode_by_hand():
+    """Hand-made z-buffers of a 1 x 8 row, dyadic log values, S = 4 (f = i/4 exact): every case of the rule.
+    Expected values are written out from R19, not computed by the rule's code:
+      both hit, |Z_A - Z_B| <= 0.01 min  ->  (1 - f) L_A* + f L_B*      (swapped weights fail: L_A* != L_B*)
+      both hit, depths apart             ->  the nearer one, from either side
+      one hit -> it;  none -> the previous value.
+    The 1 % boundary is inclusive: Z = 100 and 101 differ by exactly 0.01f * 100 = 1 in binary32."""
+    S = 4
+    assert np.float32(0.01) * np.float32(100.0) == np.float32(1.0)      # the boundary case is exact
+    LA = np.array([[-2.0, 1.5, 0.25, 3.0, -1.0, 0.5, 2.0, -3.0]], np.float32)
+    LB = np.array([[4.0, -0.5, 1.0, -2.0, 0.75, -1.5, 1.0, 2.5]], np.float32)
+    Lprev = np.full((1, 8), 7.0, np.float32)
+    E_ = EMPTY
+    #             same depth   1% apart(incl)  just over 1%        A nearer       B nearer      only A   only B   none
+    zA = np.array([[_key(2.0, 1), _key(100.0, 0), _key(100.0, 3), _key(1.0, 5), _key(8.0, 2), _key(3.0, 7), E_, E_]], np.uint64)
+    zB = np.array([[_key(2.0, 6), _key(101.0, 4), _key(np.nextafter(np.float32(101.0), np.float32(200.0)), 4),
+                    _key(4.0, 0), _key(2.0, 7), E_, _key(5.0, 3), E_]], np.uint64)
+    for i in range(1, S + 1):
+        f = i / S
+        lh, d, idx = orc.composite(i, S, 1, zA, zB, LA, LB, Lprev)
+        want = [(1 - f) * 1.5 + f * 1.0,          # LA[1], LB[6]
+                (1 - f) * -2.0 + f * 0.75,        # LA[0], LB[4]   (boundary: still the same surface)
+                3.0,                              # A at 100 is nearer than B at 101.00001: LA[3]
+                0.5,                              # LA[5]
+                2.5,                              # LB[7]
+                -3.0,                             # LA[7]
+                -2.0,                             # LB[3]
+                7.0]                              # hold
+        assert lh[0].tolist() == want, (i, lh[0].tolist())
+        assert d[0].tolist() == [2, 2, 1, 1, 0, 1, 0, 3]
+        assert idx[0].tolist() == [6, 4, 3, 5, 7, 7, 3, orc.NONE]
+    # mode 0 on the same buffers: B wherever it hit, else A (PAPER.md:129)
+    lh, d, _ = orc.composite(2, S, 0, zA, zB, LA, LB, Lprev)
+    assert lh[0].tolist() == [1.0, 0.75, 0.75, 4.0, 2.5, -3.0, -2.0, 7.0]
+    assert d[0].tolist() == [0, 0, 0, 0, 0, 1, 0, 3]
+
+
+@pytest.mark.parametrize("d", [(1, 0), (-2, 1)])
+def test_p16b_blend_is_a_linear_ramp_in_time_along_a_translation(d):
+    """A plane translating by an integer d per substep whose brightness rises by delta between the keyframes:
+    where both keyframes see the surface, mode 1 gives L_A(surface) + f delta -- the time-weighted blend of
+    north_star, exact for dyadic values; the strip only B (only A) sees takes that keyframe's value; the rest
+    holds.  The z-buffers come from evo_splat, pinned by P3 on this very scene.
+    (P2 does not carry over to mode 1: at i = S direction A lands with Z = Z_B of its far end, so a nearer A
+    surface may legitimately replace keyframe B's own pixel.)"""
+    H, W, S = 20, 24, 4
+    dx, dy = d
+    r = _rng(16)
+    big = (r.integers(-24, 25, size=(H + 64, W + 64)) / 8.0).astype(np.float32)     # dyadic texture
+    ys, xs = np.mgrid[0:H, 0:W]
+    tex = lambda px, py: big[ys - py + 32, xs - px + 32]
+    delta = np.float32(0.75)
+    LA, LB = tex(0, 0), tex(S * dx, S * dy) + delta
+    mv = np.empty((H, W, 2), np.float32)
+    mv[..., 0], mv[..., 1] = -S * dx, -S * dy
+    Z = np.full((H, W), 3.0, np.float32)
+    prev = LA.copy()
+    for i in range(1, S + 1):
+        f = i / S
+        zA = orc.splat(i, S, False, -mv, Z, Z)
+        zB = orc.splat(i, S, True, mv, Z, Z)
+        lh, dirs, _ = orc.composite(i, S, 1, zA, zB, LA, LB, prev)
+        sbx, sby = xs + (S - i) * dx, ys + (S - i) * dy
+        sax, say = xs - i * dx, ys - i * dy
+        inB = (sbx >= 0) & (sbx < W) & (sby >= 0) & (sby < H)
+        inA = (sax >= 0) & (sax < W) & (say >= 0) & (say < H)
+        surf = tex(i * dx, i * dy)                                      # the plane at time f, brightness of A
+        want = np.where(inA & inB, surf + np.float32(f) * delta,
+                        np.where(inB, surf + delta, np.where(inA, surf, prev)))
+        assert np.array_equal(lh, want.astype(np.float32)), i
+        assert np.array_equal(dirs, np.where(inA & inB, 2, np.where(inB, 0, np.where(inA, 1, 3))))
+        prev = lh
+
+
+# ------------------------------------------------------------------------------------------------
 # P4: 8x8 brute force, gather form, straight from the definition of S(q) (Eq. 6)
 # ------------------------------------------------------------------------------------------------
 def _brute_winner(H, W, i, S, src_is_B, disp, Zsrc, Zoth):
