@@ -57,12 +57,14 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based, 1..4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--path", default="auto", choices=["auto", "global", "tile"])
     ap.add_argument("--envs", type=int, default=0, help="override the number of envs (0 = the config's)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=6)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--profile-range", action="store_true",
+                    help="bracket the timed region with cudaProfilerStart / Stop (for `ncu --replay-mode app-range`: "
+                         "counters of the whole step in its real multi-stream schedule); implies no e2e / cpu legs")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json config 5: one JSON line per (envs x resolution x S) point, device-resident")
     return ap.parse_args()
@@ -219,7 +221,7 @@ def run_ours(args, spec) -> None:
     sc = scenes.make_scene(spec)
     n_kf = Wm + K + 1
     kfs = [scenes.render_keyframe(sc, k, device=dev) for k in range(n_kf)]
-    path = {"auto": binding.PATH_AUTO, "global": binding.PATH_GLOBAL, "tile": binding.PATH_TILE}[args.path]
+    path = binding.PATH_AUTO
     cap = int(min(0x7FFFFFFF, max(1 << 22, 10 * E * H * W)))          # events stored per step
     mk = lambda: binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
                               max_motion_px=spec.max_motion_px(), path=path, device=local, event_capacity=cap)
@@ -246,21 +248,25 @@ def run_ours(args, spec) -> None:
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     t0 = time.time()
+    if args.profile_range:
+        torch.cuda.profiler.start()
     e0.record(stream)
     for k in range(Wm + 1, Wm + 1 + K):
         step(k)
     ev.wait_events(stream)                              # the last step's ordered stream is part of the timed region
     e1.record(stream)
     barrier()
+    if args.profile_range:
+        torch.cuda.profiler.stop()
     t1 = time.time()
     ms = e0.elapsed_time(e1)
     clocks = clk.stop(t0, t1)
     i1 = ev.info()
-    if i1.last_overflow:
+    if i1.overflow_steps != i0.overflow_steps:          # sticky: any step of the timed region, not only the last
         raise SystemExit("bench.py: event capacity overflow in the timed region")
     events = i1.total_events - i0.total_events
     launches = i1.kernel_launches - i0.kernel_launches
-    path_used = {binding.PATH_GLOBAL: "global", binding.PATH_TILE: "tile"}[i1.path]
+    path_used = "global"
 
     # ---- per-stage device time of the same steps (second pass over the same keyframes, CUDA events
     #      recorded by the library on the launching stream) -> dominant kernel for the roofline -------
@@ -314,7 +320,7 @@ def run_ours(args, spec) -> None:
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
 
     # ---- e2e: HOST buffers through evis_step_host + evis_read_events -------------------------------------
-    if not args.no_e2e:
+    if not args.no_e2e and not args.profile_range:
         Ke = max(1, min(args.e2e_steps, K))
         hk = []
         for k in range(Wm + 1 + Ke):
@@ -351,7 +357,7 @@ def run_ours(args, spec) -> None:
                       "api": "evis_step_host (pinned host keyframes) + evis_read_events_begin / _end (pinned host stream, "
                              "overlapping the next upload)"}
 
-    if rank == 0 and not args.no_cpu:
+    if rank == 0 and not args.no_cpu and not args.profile_range:
         out["cpu_baseline"] = cpu_baseline(scenes.small(spec, seed=spec.seed - 1000 * rank), args.cpu_seconds)
     if rank == 0:
         print(json.dumps(out))
@@ -396,7 +402,7 @@ def run_sweep(args) -> None:
         torch.cuda.synchronize(dev)
         ms = e0.elapsed_time(e1)
         i1 = ev.info()
-        if i1.last_overflow:
+        if i1.overflow_steps != i0.overflow_steps:
             raise SystemExit("bench.py: event capacity overflow in the sweep")
         events = i1.total_events - i0.total_events
         ev.destroy()

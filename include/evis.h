@@ -33,13 +33,18 @@ typedef enum {
     EVIS_ERR_INVALID_ARG  = -1,   /* NULL pointer, non-positive size, threshold <= 0, ... */
     EVIS_ERR_CUDA         = -2,   /* a CUDA call failed; evis_last_cuda_error() has the code */
     EVIS_ERR_OOM          = -3,   /* device allocation failed */
-    EVIS_ERR_OVERFLOW     = -4,   /* more events than event_capacity: the count returned is the
-                                     true count, the stored stream is an incomplete prefix */
-    EVIS_ERR_MOTION_BOUND = -5,   /* a motion vector exceeded max_motion_px on the tile path */
+    EVIS_ERR_OVERFLOW     = -4,   /* more events than event_capacity: the count returned is the true count; the
+                                     stored stream is the first event_capacity events of the deterministic order,
+                                     or EMPTY when the intermediate records did not fit either (evis_info
+                                     last_overflow = 2): a read call then reports 0 events */
+    EVIS_ERR_MOTION_BOUND = -5,   /* a motion vector exceeded the max_motion_px the caller declared (the results
+                                     are exact all the same: the z-buffers take any motion) */
     EVIS_ERR_BAD_STATE    = -6    /* call order violated (e.g. read before any step) */
 } evis_status;
 
-enum { EVIS_PATH_AUTO = 0, EVIS_PATH_GLOBAL = 1, EVIS_PATH_TILE = 2 };
+/* One path: z-buffers in global memory (L2-resident chunks), any motion.  The per-tile shared-memory path of
+ * round 1 (value 2) was measured 3-4x slower on every workload and retired: 2 is INVALID_ARG. */
+enum { EVIS_PATH_AUTO = 0, EVIS_PATH_GLOBAL = 1 };
 enum { EVIS_COMPOSITE_B_PRIMARY = 0, EVIS_COMPOSITE_BLEND = 1 };
 
 typedef struct {
@@ -48,8 +53,8 @@ typedef struct {
     float    c_pos, c_neg;              /* contrast thresholds C+, C- (> 0)  (Eq. 4, R4)         */
     float    log_eps;                   /* eps of L = log(I + eps) (> 0)     (R2)   */
     float    keyframe_dt;               /* T = 1/f_k in seconds (> 0)                            */
-    float    max_motion_px;             /* bound on |mv| (infinity norm) the caller guarantees;
-                                           0 = unknown -> global z-buffer path                   */
+    float    max_motion_px;             /* bound on |mv| (infinity norm) the caller declares; a violation
+                                           is reported (EVIS_ERR_MOTION_BOUND); 0 = none declared   */
     int32_t  composite_mode;            /* EVIS_COMPOSITE_*  (R19)                 */
     int32_t  path;                      /* EVIS_PATH_*                                           */
     int32_t  device;                    /* CUDA device ordinal                                   */
@@ -71,17 +76,19 @@ typedef struct {
 } evis_event;
 
 typedef struct {
-    int32_t  path;              /* EVIS_PATH_GLOBAL or EVIS_PATH_TILE actually used              */
+    int32_t  path;              /* EVIS_PATH_GLOBAL                                              */
     int32_t  tile_w, tile_h;    /* ordering tile of the event stream                             */
-    int32_t  halo;              /* tile path: halo in pixels                                     */
+    int32_t  halo;              /* reserved (0)                                                  */
     uint64_t steps;             /* evis_step calls so far                                        */
     uint64_t last_events;       /* true event count of the last step                             */
     uint64_t last_holes;        /* pixel-substeps of the last step reached by neither keyframe   */
     uint64_t kernel_launches;   /* kernels + memsets this library launched since creation        */
-    int32_t  last_overflow;     /* 1 if the last step overflowed event_capacity                  */
-    int32_t  last_motion_violation; /* 1 if a motion vector exceeded the tile-path bound         */
+    int32_t  last_overflow;     /* last step: 0 all events stored; 1 more than event_capacity (a valid prefix
+                                   is stored); 2 the intermediate records overflowed too (nothing valid stored) */
+    int32_t  last_motion_violation; /* 1 if a motion vector exceeded the declared max_motion_px   */
     uint64_t device_bytes;      /* device memory owned by the context                            */
     uint64_t total_events;      /* true event count summed over every step so far                */
+    uint64_t overflow_steps;    /* steps so far whose events did not all fit (sticky)            */
 } evis_info;
 
 /* Per-stage device time, measured with CUDA events on the stream evis_step was given (test and
@@ -91,7 +98,7 @@ enum { EVIS_STAGE_PREP = 0,     /* a1 + a9: log-luminance, keyframe take-over   
        EVIS_STAGE_SPLAT = 2,    /* global path: a2-a4                                             */
        EVIS_STAGE_RESOLVE = 3,  /* global path: a5-a8 (resolve, event model, compaction)          */
        EVIS_STAGE_ORDER = 4,    /* a8: deterministic ordering                                     */
-       EVIS_STAGE_TILE = 5,     /* tile path: a2-a8 fused                                         */
+       EVIS_STAGE_RESERVED5 = 5,
        EVIS_STAGE_WARP = 6,     /* global path with concurrent z-buffer regions: a2-a8 of all chunks, from the
                                    fork of the internal streams to their join (kernels overlap, so splat and
                                    resolve are not timed apart)                                   */
@@ -142,9 +149,9 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
  * caller samples them, e.g. max(N(C, sigma^2), theta_min), once per pixel).  DEVICE pointers if src_is_device != 0,
  * else HOST.  The library copies the maps (the caller may free its buffers when the call returns; the call
  * synchronises) and uses them from the next evis_step on: Eq. 4 at pixel u runs with theta_on(u) for dL > 0 and
- * theta_off(u) for dL < 0.  Both NULL = back to the scalar thresholds.  Global path only.
+ * theta_off(u) for dL < 0.  Both NULL = back to the scalar thresholds.  
  * Errors: INVALID_ARG (exactly one pointer NULL; a value that is not finite and > 0 -- the previous thresholds
- * stay in force), BAD_STATE (tile path), CUDA, OOM. */
+ * stay in force), CUDA, OOM. */
 int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta_off, int src_is_device);
 
 /* Noise events (Eq. 9-10; R29).  In every substep (duration dt = T / S) every pixel
@@ -161,23 +168,29 @@ typedef struct {
 } evis_noise;
 /* noise = NULL switches the noise events off.  hot_mask: [E,H,W] bytes, non-zero = the pixel belongs to the hot set
  * (DEVICE pointer if mask_is_device != 0, else HOST; nullable = empty set); the library copies it.  Applies from the
- * next evis_step on; synchronises.  Global path only.  Errors: INVALID_ARG (negative or non-finite rate, i_white
- * <= 0), BAD_STATE (tile path), CUDA, OOM. */
+ * next evis_step on; synchronises.  Errors: INVALID_ARG (negative or non-finite rate, i_white
+ * <= 0), CUDA, OOM. */
 int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_mask, int mask_is_device);
+
+/* The index `kf` the NEXT closed interval gets (it is stored in every event and keys the noise generator, R29);
+ * it starts at 0 and advances by one per interval.  A context resumed from a checkpoint (evis_set_state,
+ * evis_refractory_state, keyframe A fed again as its first step) sets it to the interval it continues with, so that
+ * events carry the original indices and a noise run draws the same noise events.  Errors: INVALID_ARG. */
+int evis_set_interval_index(evis_ctx *ctx, uint32_t next_kf);
 
 /* Colour events ("Replacing I with individual R, G, B channels and applying the event model to each
  * independently produces color events"; R28): channel = 0, 1 or 2 makes this context take
  * L = log(channel + eps) of the radiance's R, G or B instead of the Rec.709 luminance; -1 = luminance (default).
  * A colour sensor is three contexts fed the same keyframes, one per channel.  Applies to the keyframes given to
- * later evis_step calls: set it before the first one.  Both paths.  Errors: INVALID_ARG. */
+ * later evis_step calls: set it before the first one.  Errors: INVALID_ARG. */
 int evis_set_channel(evis_ctx *ctx, int channel);
 
 /* Over-render margin (Supp. B 317-319; R27): the frames handed to evis_step (height x
  * width of the configuration) were rendered with `margin` extra pixels on each side.  The warp uses all of them;
  * the margin is cropped off afterwards: the event model runs and events exist only for the inner
  * (height - 2 margin) x (width - 2 margin) pixels, x and y of an event are relative to that cropped frame, holes are
- * counted inside it.  0 = no margin (default).  Applies from the next evis_step on; synchronises.  Global path only.
- * Errors: INVALID_ARG (negative, or 2 margin >= min(height, width)), BAD_STATE (tile path), CUDA. */
+ * counted inside it.  0 = no margin (default).  Applies from the next evis_step on; synchronises.  
+ * Errors: INVALID_ARG (negative, or 2 margin >= min(height, width)), CUDA. */
 int evis_set_margin(evis_ctx *ctx, int margin);
 
 /* Refractory period (R26): with tau_r > 0 (seconds) a threshold crossing of a pixel is
@@ -185,14 +198,16 @@ int evis_set_margin(evis_ctx *ctx, int margin);
  * EMITTED event (none before the call: every pixel starts free); suppressed crossings still move L_ref (Eq. 4 is
  * unchanged).  The timestamps then decide which events exist, so they are computed in IEEE binary32 with a fixed
  * operation order.  The state t_last is carried across steps.  tau_r = 0 switches the period off.  Calling it
- * again with tau_r > 0 resets t_last.  Applies from the next evis_step on; synchronises.  Global path only.
- * Errors: INVALID_ARG (negative or non-finite tau_r), BAD_STATE (tile path), CUDA, OOM. */
+ * again with tau_r > 0 resets t_last.  Applies from the next evis_step on; synchronises.  
+ * Errors: INVALID_ARG (negative or non-finite tau_r), CUDA, OOM. */
 int evis_set_refractory(evis_ctx *ctx, float tau_r);
 
 /* Copy the events of the last step, in the deterministic order
  * (env, substep, tile row, tile column, y, x, crossing k), to `dst` (room for `max` events;
  * device pointer if dst_is_device != 0, else host).  Synchronises.  *n_out = events copied
- * (= min(true count, capacity, max)).  Errors: INVALID_ARG, BAD_STATE, CUDA. */
+ * (= min(stored, max); stored = min(true count, capacity), see EVIS_ERR_OVERFLOW).
+ * Errors: INVALID_ARG, BAD_STATE, CUDA; OVERFLOW when the last step overflowed (the valid prefix, if any, has been
+ * copied all the same).  The same holds for evis_read_events_begin and evis_events_device. */
 int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t max, uint64_t *n_out);
 
 /* The same copy to HOST memory (pinned, for a real overlap) in two halves, so that the next evis_step_host can upload

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libevis.so")
 EVIS_OK = 0
 EVIS_ERR_INVALID_ARG, EVIS_ERR_CUDA, EVIS_ERR_OOM = -1, -2, -3
 EVIS_ERR_OVERFLOW, EVIS_ERR_MOTION_BOUND, EVIS_ERR_BAD_STATE = -4, -5, -6
-PATH_AUTO, PATH_GLOBAL, PATH_TILE = 0, 1, 2
+PATH_AUTO, PATH_GLOBAL = 0, 1
 COMPOSITE_B_PRIMARY, COMPOSITE_BLEND = 0, 1
 
 EVENT_DTYPE = np.dtype([("x", "<u2"), ("y", "<u2"), ("env", "<u2"), ("p", "i1"), ("substep", "u1"),
@@ -39,11 +39,12 @@ class evis_info(C.Structure):
     _fields_ = [("path", C.c_int32), ("tile_w", C.c_int32), ("tile_h", C.c_int32), ("halo", C.c_int32),
                 ("steps", C.c_uint64), ("last_events", C.c_uint64), ("last_holes", C.c_uint64),
                 ("kernel_launches", C.c_uint64), ("last_overflow", C.c_int32),
-                ("last_motion_violation", C.c_int32), ("device_bytes", C.c_uint64), ("total_events", C.c_uint64)]
+                ("last_motion_violation", C.c_int32), ("device_bytes", C.c_uint64), ("total_events", C.c_uint64),
+                ("overflow_steps", C.c_uint64)]
 
 
 NUM_STAGES = 8
-STAGE_NAMES = ["prep", "clear", "splat", "resolve", "order", "tile", "splat+resolve", "s7"]
+STAGE_NAMES = ["prep", "clear", "splat", "resolve", "order", "s5", "splat+resolve", "s7"]
 
 
 class evis_profile(C.Structure):
@@ -53,7 +54,8 @@ class evis_profile(C.Structure):
 # every symbol include/evis.h declares (tests/test_abi.py checks the list against the header)
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
-           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end"]
+           "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end",
+           "evis_set_interval_index"]
 
 _lib = None
 
@@ -86,6 +88,7 @@ def load() -> C.CDLL:
     L.evis_set_refractory.argtypes = [vp, C.c_float]
     L.evis_set_margin.argtypes = [vp, C.c_int]
     L.evis_set_channel.argtypes = [vp, C.c_int]
+    L.evis_set_interval_index.argtypes = [vp, C.c_uint32]
     L.evis_wait_events.argtypes = [vp, vp]
     L.evis_read_events_begin.argtypes = [vp, vp, C.c_uint64, u64p]
     L.evis_read_events_end.argtypes = [vp]
@@ -198,6 +201,10 @@ class Evis:
         """evis_set_channel (colour events): 0 / 1 / 2 = log of R / G / B, -1 = Rec.709 luminance."""
         _check(self._lib.evis_set_channel(self._ctx, int(channel)), "evis_set_channel")
 
+    def set_interval_index(self, next_kf: int) -> None:
+        """evis_set_interval_index: the index the next closed interval gets (checkpoint / resume)."""
+        _check(self._lib.evis_set_interval_index(self._ctx, int(next_kf)), "evis_set_interval_index")
+
     def set_margin(self, margin: int) -> None:
         """evis_set_margin: the frames carry `margin` over-rendered pixels per side, cropped after the warp."""
         _check(self._lib.evis_set_margin(self._ctx, int(margin)), "evis_set_margin")
@@ -223,8 +230,9 @@ class Evis:
         return int(n.value)
 
     # -- evis_read_events --------------------------------------------------------------------------
-    def read_events(self, max_events: Optional[int] = None) -> np.ndarray:
-        """Events of the last step in the library's deterministic order (host structured array)."""
+    def read_events(self, max_events: Optional[int] = None, allow=()) -> np.ndarray:
+        """Events of the last step in the library's deterministic order (host structured array).  After a step that
+        overflowed the call raises EVIS_ERR_OVERFLOW unless ``allow`` lists it; the valid prefix is returned then."""
         info = self.info()
         n = min(info.last_events, self.cfg.event_capacity)
         if max_events is not None:
@@ -232,7 +240,7 @@ class Evis:
         out = np.empty(n, dtype=EVENT_DTYPE)
         got = C.c_uint64(0)
         _check(self._lib.evis_read_events(self._ctx, out.ctypes.data if n else None, 0, n, C.byref(got)),
-               "evis_read_events")
+               "evis_read_events", allow)
         return out[:got.value]
 
     def read_events_into(self, host_buf: np.ndarray) -> int:

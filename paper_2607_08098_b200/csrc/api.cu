@@ -11,13 +11,11 @@
 using namespace evis;
 
 static_assert(sizeof(evis_event) == 16, "evis_event is a 16-byte record");
-static_assert(sizeof(evis_config) == 64 && sizeof(evis_info) == 72, "ABI struct layout (binding.py mirrors it)");
+static_assert(sizeof(evis_config) == 64 && sizeof(evis_info) == 80, "ABI struct layout (binding.py mirrors it)");
 
 struct evis_ctx {
     evis_config cfg;
     Geom g;
-    int path;                         // EVIS_PATH_GLOBAL / EVIS_PATH_TILE in use
-    TilePlan tile;
     cudaStream_t own_stream;          // evis_step_host, state/debug copies
     cudaStream_t last_stream;
     int last_cuda;
@@ -72,7 +70,7 @@ struct evis_ctx {
     uint32_t dir_entries;
     unsigned long long *bsum;
     // device counters.  Reset every step: [0] events, [1] holes, [2] arrival slots handed out,
-    // [3] tile work counter.  Sticky: [4] motion-bound violations, [5] events over all steps.
+    // [3] unused.  Sticky: [4] motion-bound violations, [5] events over all steps.
     unsigned long long *counters;
     unsigned long long *h_counters;   // pinned host mirror
     unsigned long long arrival_cap;   // slots of the arrival buffer (capacity + slab slack)
@@ -82,6 +80,7 @@ struct evis_ctx {
     float *st_rad, *st_mv, *st_fwd, *st_depth;
 
     uint64_t steps, launches, device_bytes;
+    uint32_t kf_next;                 // index the next closed interval gets (evis_set_interval_index)
     uint64_t last_events, last_holes;
     int last_overflow, last_motion;
     bool have_events;
@@ -98,8 +97,8 @@ namespace {
 
 // Device counters, one per 128-byte line: the arrival reservation (C_ALLOC) is on every resolve block's critical
 // path and must not queue behind the event / hole tallies in the same L2 sector.  [0, C_STEP_END) are reset
-// every step; C_MOTION and C_TOTAL are sticky.
-enum { C_EVENTS = 0, C_HOLES = 16, C_ALLOC = 32, C_ITEM = 48, C_STEP_END = 64, C_MOTION = 64, C_TOTAL = 80, NCOUNTERS = 96 };
+// every step; C_MOTION, C_TOTAL and C_OVERFLOW (steps whose events did not all fit) are sticky.
+enum { C_EVENTS = 0, C_HOLES = 16, C_ALLOC = 32, C_ITEM = 48, C_STEP_END = 64, C_MOTION = 64, C_TOTAL = 80, C_OVERFLOW = 96, NCOUNTERS = 112 };
 
 struct DeviceGuard {
     int prev;
@@ -257,18 +256,9 @@ int create_impl(evis_ctx *ctx)
     volatile float dt = c.keyframe_dt / (float)g.S;
     ctx->ep.c_pos = c.c_pos; ctx->ep.c_neg = c.c_neg; ctx->ep.dt = dt; ctx->ep.kf = 0;
 
-    // path selection
     ctx->nset = g.mode == 0 ? 1 : 2;
-    ctx->path = EVIS_PATH_GLOBAL;
-    memset(&ctx->tile, 0, sizeof ctx->tile);
-    // AUTO = the global z-buffer path: it is the faster one on every measured workload;
-    // the fused shared-memory tile path runs on request, for bounded motion
-    if (c.path == EVIS_PATH_TILE && c.max_motion_px > 0.0f && plan_tile(g, c.max_motion_px, &ctx->tile))
-        ctx->path = EVIS_PATH_TILE;
-    if (c.path == EVIS_PATH_TILE && ctx->path != EVIS_PATH_TILE) return EVIS_ERR_INVALID_ARG;
-
     uint32_t tiles_x, tiles_y;
-    if (ctx->path == EVIS_PATH_GLOBAL) {
+    {
         // chunk = envs x substeps whose z-buffers fit one region's budget.  Defaults (measured on B200, DESIGN.md
         // Sec. 6): 4 regions on 4 streams; 24 MiB regions when one env's S substeps fit (the live keys stay in the
         // L2 and small grids overlap across streams), else 512 MiB / regions (substep chunks re-read the sources and carry
@@ -328,21 +318,14 @@ int create_impl(evis_ctx *ctx)
         }
         tiles_x = (g.W + G_TILE_W - 1) / G_TILE_W;
         tiles_y = (g.H + G_TILE_H - 1) / G_TILE_H;
-    } else {
-        tiles_x = ctx->tile.tiles_x;
-        tiles_y = ctx->tile.tiles_y;
     }
     const unsigned long long ent = (unsigned long long)g.E * g.S * tiles_x * tiles_y;
     if (ent >= 0xFFFFFFFFull) return EVIS_ERR_INVALID_ARG;
     ctx->dir_entries = (uint32_t)ent;
     CU(dalloc(ctx, &ctx->directory, (size_t)ent));
     CU(dalloc(ctx, &ctx->bsum, (size_t)(ent / ORDER_ENTRIES_PER_BLOCK + 2)));
-    if (ctx->path == EVIS_PATH_TILE) CU(tile_setup(g, ctx->tile, c.device));
-    // arrival buffer: the global path packs chunks densely; the tile path hands out slabs, so each
-    // persistent CTA may leave one slab partly used and lose < one chunk at every slab change
+    // arrival buffer: the chunks of records (or events, in direct mode) are packed densely
     ctx->arrival_cap = c.event_capacity;
-    if (ctx->path == EVIS_PATH_TILE)
-        ctx->arrival_cap += c.event_capacity / 8 + (unsigned long long)(ctx->tile.ctas + 1) * ctx->tile.slab;
     if (ctx->arrival_cap > 0xFFFFFFF0ull) ctx->arrival_cap = 0xFFFFFFF0ull;
     CU(dalloc(ctx, &ctx->arrival, (size_t)ctx->arrival_cap));
     CU(dalloc(ctx, &ctx->ordered, (size_t)c.event_capacity));
@@ -392,8 +375,18 @@ int fetch_counters(evis_ctx *ctx)
     ctx->last_events = ctx->h_counters[C_EVENTS];
     ctx->last_holes = ctx->h_counters[C_HOLES];
     ctx->last_motion = ctx->h_counters[C_MOTION] != 0;
-    ctx->last_overflow = ctx->last_events > ctx->cfg.event_capacity || ctx->h_counters[C_ALLOC] > ctx->arrival_cap;
+    // 2: records were dropped in arrival order, the stored stream has gaps and is unusable; 1: a valid prefix is stored
+    ctx->last_overflow = ctx->h_counters[C_ALLOC] > ctx->arrival_cap ? 2 : (ctx->last_events > ctx->cfg.event_capacity ? 1 : 0);
     return EVIS_OK;
+}
+
+// Events of the last step that the ordered stream validly holds (after fetch_counters): all of them; the first
+// event_capacity when there were more (a true prefix of the deterministic order); none when the ARRIVAL buffer
+// overflowed -- records were then dropped in scheduling order and the ordered stream has gaps.
+uint64_t stored_events(const evis_ctx *ctx)
+{
+    if (ctx->last_overflow == 2) return 0;
+    return ctx->last_events < ctx->cfg.event_capacity ? ctx->last_events : ctx->cfg.event_capacity;
 }
 
 }  // namespace
@@ -429,7 +422,7 @@ int evis_create(const evis_config *cfg, evis_ctx **out)
     if (!(cfg->max_motion_px >= 0.0f)) return EVIS_ERR_INVALID_ARG;
     if (cfg->composite_mode != EVIS_COMPOSITE_B_PRIMARY && cfg->composite_mode != EVIS_COMPOSITE_BLEND)
         return EVIS_ERR_INVALID_ARG;
-    if (cfg->path < EVIS_PATH_AUTO || cfg->path > EVIS_PATH_TILE) return EVIS_ERR_INVALID_ARG;
+    if (cfg->path != EVIS_PATH_AUTO && cfg->path != EVIS_PATH_GLOBAL) return EVIS_ERR_INVALID_ARG;
     if (cfg->event_capacity == 0 || cfg->event_capacity > 0x7FFFFFFFull) return EVIS_ERR_INVALID_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return EVIS_ERR_CUDA; }
@@ -477,7 +470,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         Span sp(ctx, st, EVIS_STAGE_PREP, 1);
         CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, ctx->channel_set ? ctx->channel : -1, B.L, B.mv, B.fwd, B.Z,
                        first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr,
-                       ctx->path == EVIS_PATH_TILE ? ctx->cfg.max_motion_px : 0.0f, ctx->counters + C_MOTION, st));
+                       ctx->cfg.max_motion_px, ctx->counters + C_MOTION, st));
     }
     ctx->last_stream = st;
     if (first) {
@@ -489,7 +482,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         return EVIS_OK;
     }
 
-    ctx->ep.kf = (uint32_t)(ctx->steps - 1);
+    ctx->ep.kf = ctx->kf_next;
     // slot of this step's arrival buffer, directory and per-step counters; the order stage that used it last
     // (two steps ago with overlap, the last step without) must be done before it is cleared
     const int sl = ctx->overlap ? (int)(ctx->steps & 1) : 0;
@@ -518,7 +511,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         CU(cudaMemsetAsync(sink.directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
     }
 
-    if (ctx->path == EVIS_PATH_GLOBAL) {
+    {
         // nreg > 1: the env chunks are dealt round-robin to the regions' streams, which fork from `st` here and
         // join it after the loop; the substep chunks of one env chunk stay on one stream (L_ref / L_prev carry)
         const bool multi = ctx->nreg > 1;
@@ -572,10 +565,6 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                 CU(cudaEventRecord(ctx->ev_join[r], ctx->reg_stream[r]));
                 CU(cudaStreamWaitEvent(st, ctx->ev_join[r], 0));
             }
-    } else {
-        Span sp(ctx, st, EVIS_STAGE_TILE, 1);
-        CU(launch_tile(g, ctx->tile, A, B, ctx->tab, ctx->l_ref, ctx->l_prev, ctx->ep, sink, cnt + C_HOLES,
-                       cnt + C_ITEM, ctx->dbg, st));
     }
     // a8, second half, on the order stream: it starts when this step's chunks are done and overlaps the next step
     cudaStream_t os = ctx->ord_stream;
@@ -585,14 +574,14 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     {
         Span sp(ctx, os, EVIS_STAGE_ORDER, 3);
         unsigned long long *sticky = ctx->counters_s[0];             // C_MOTION, C_TOTAL live in slot 0's array
-        if (ctx->path == EVIS_PATH_GLOBAL && !rf.t_last) {
+        if (!rf.t_last) {
             const uint32_t tx = (g.W + G_TILE_W - 1) / G_TILE_W, ty = (g.H + G_TILE_H - 1) / G_TILE_H;
             CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
-                             cnt + C_EVENTS, sticky + C_TOTAL, ctx->ep, th, (uint32_t)g.W,
+                             cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, ctx->ep, th, (uint32_t)g.W,
                              (uint32_t)g.HW, (uint32_t)g.margin, tx, tx * ty, (uint32_t)g.S, os));
         } else {
             CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
-                            cnt + C_EVENTS, sticky + C_TOTAL, os));
+                            cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, os));
         }
         CU(cudaMemcpyAsync(ctx->h_counters, cnt, C_STEP_END * sizeof(unsigned long long), cudaMemcpyDeviceToHost, os));
         CU(cudaMemcpyAsync(ctx->h_counters + C_MOTION, sticky + C_MOTION, (NCOUNTERS - C_MOTION) * sizeof(unsigned long long),
@@ -602,6 +591,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     ctx->ord_pending[sl] = true;
     ctx->last_slot = sl;
     ctx->steps += 1;
+    ctx->kf_next += 1;
     ctx->cur ^= 1;
     ctx->have_events = true;
     if (n_events) {
@@ -617,7 +607,6 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
 int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta_off, int src_is_device)
 {
     if (!ctx || ((theta_on == nullptr) != (theta_off == nullptr))) return EVIS_ERR_INVALID_ARG;
-    if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     // work already enqueued keeps the thresholds it was launched with
@@ -648,8 +637,9 @@ int evis_set_thresholds(evis_ctx *ctx, const float *theta_on, const float *theta
     }
     cudaFree(bad);
     if (rc != EVIS_OK) { cudaFree(on); cudaFree(off); return rc; }
-    cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last); cudaFree(ctx->hot);
+    // the new maps replace the old ones; nothing else the context owns is touched
     if (!ctx->th_on) ctx->device_bytes += 2 * P * sizeof(float);
+    cudaFree(ctx->th_on); cudaFree(ctx->th_off);
     ctx->th_on = on; ctx->th_off = off;
     ctx->th_active = true;
     ctx->launches += 2;
@@ -669,7 +659,6 @@ int evis_wait_events(evis_ctx *ctx, void *cuda_stream)
 int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_mask, int mask_is_device)
 {
     if (!ctx) return EVIS_ERR_INVALID_ARG;
-    if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     if (ctx->steps) CU(sync_all(ctx));
@@ -685,6 +674,7 @@ int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_ma
     } else if (ctx->hot) {
         cudaFree(ctx->hot);
         ctx->hot = nullptr;
+        ctx->device_bytes -= P;
     }
     if (!ctx->t_last) {                                   // the direct resolve variant carries t_last
         CU(dalloc(ctx, &ctx->t_last, P));
@@ -693,6 +683,13 @@ int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_ma
     CU(cudaStreamSynchronize(ctx->own_stream));
     ctx->noise = *noise;
     ctx->noise_on = true;
+    return EVIS_OK;
+}
+
+int evis_set_interval_index(evis_ctx *ctx, uint32_t next_kf)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    ctx->kf_next = next_kf;
     return EVIS_OK;
 }
 
@@ -708,7 +705,6 @@ int evis_set_margin(evis_ctx *ctx, int margin)
 {
     if (!ctx) return EVIS_ERR_INVALID_ARG;
     if (margin < 0 || 2 * (long long)margin >= (ctx->g.H < ctx->g.W ? ctx->g.H : ctx->g.W)) return EVIS_ERR_INVALID_ARG;
-    if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     if (ctx->steps) CU(sync_all(ctx));
@@ -719,7 +715,6 @@ int evis_set_margin(evis_ctx *ctx, int margin)
 int evis_set_refractory(evis_ctx *ctx, float tau_r)
 {
     if (!ctx || !(tau_r >= 0.0f) || !(tau_r < 3.0e38f)) return EVIS_ERR_INVALID_ARG;
-    if (ctx->path != EVIS_PATH_GLOBAL) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     if (ctx->steps) CU(sync_all(ctx));
@@ -768,13 +763,12 @@ int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t
     if (!guard.ok) return EVIS_ERR_CUDA;
     const int rc = fetch_counters(ctx);
     if (rc != EVIS_OK) return rc;
-    uint64_t n = ctx->last_events;
-    if (n > ctx->cfg.event_capacity) n = ctx->cfg.event_capacity;
+    uint64_t n = stored_events(ctx);
     if (n > max) n = max;
     if (n) CU(cudaMemcpy(dst, ctx->ordered, n * sizeof(evis_event),
                          dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
     if (n_out) *n_out = n;
-    return EVIS_OK;
+    return ctx->last_overflow ? EVIS_ERR_OVERFLOW : EVIS_OK;
 }
 
 int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, uint64_t *n_out)
@@ -786,8 +780,7 @@ int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, ui
     const int rc = fetch_counters(ctx);
     if (rc != EVIS_OK) return rc;
     if (ctx->copy_pending) CU(cudaStreamSynchronize(ctx->copy_stream));
-    uint64_t n = ctx->last_events;
-    if (n > ctx->cfg.event_capacity) n = ctx->cfg.event_capacity;
+    uint64_t n = stored_events(ctx);
     if (n > max) n = max;
     if (n) {
         CU(cudaMemcpyAsync(host_dst, ctx->ordered, n * sizeof(evis_event), cudaMemcpyDeviceToHost, ctx->copy_stream));
@@ -795,7 +788,7 @@ int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, ui
         ctx->copy_pending = true;
     }
     if (n_out) *n_out = n;
-    return EVIS_OK;
+    return ctx->last_overflow ? EVIS_ERR_OVERFLOW : EVIS_OK;
 }
 
 int evis_read_events_end(evis_ctx *ctx)
@@ -816,8 +809,8 @@ int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_st
     const int rc = fetch_counters(ctx);
     if (rc != EVIS_OK) return rc;
     *dev_ptr = reinterpret_cast<const evis_event *>(ctx->ordered);
-    *n_stored = ctx->last_events < ctx->cfg.event_capacity ? ctx->last_events : ctx->cfg.event_capacity;
-    return EVIS_OK;
+    *n_stored = stored_events(ctx);
+    return ctx->last_overflow ? EVIS_ERR_OVERFLOW : EVIS_OK;
 }
 
 int evis_get_info(evis_ctx *ctx, evis_info *info)
@@ -826,10 +819,9 @@ int evis_get_info(evis_ctx *ctx, evis_info *info)
     DeviceGuard guard(ctx->cfg.device);
     if (ctx->steps) { const int rc = fetch_counters(ctx); if (rc != EVIS_OK) return rc; }
     memset(info, 0, sizeof *info);
-    info->path = ctx->path;
-    info->tile_w = ctx->path == EVIS_PATH_TILE ? ctx->tile.tw : G_TILE_W;
-    info->tile_h = ctx->path == EVIS_PATH_TILE ? ctx->tile.th : G_TILE_H;
-    info->halo = ctx->path == EVIS_PATH_TILE ? ctx->tile.halo : 0;
+    info->path = EVIS_PATH_GLOBAL;
+    info->tile_w = G_TILE_W;
+    info->tile_h = G_TILE_H;
     info->steps = ctx->steps;
     info->last_events = ctx->last_events;
     info->last_holes = ctx->last_holes;
@@ -838,6 +830,7 @@ int evis_get_info(evis_ctx *ctx, evis_info *info)
     info->last_motion_violation = ctx->last_motion;
     info->device_bytes = ctx->device_bytes;
     info->total_events = ctx->h_counters[C_TOTAL];
+    info->overflow_steps = ctx->h_counters[C_OVERFLOW];
     return EVIS_OK;
 }
 

@@ -110,38 +110,19 @@ EVIS_DECL_RESOLVE(launch_resolve_m1d);
 // fill n floats with v (prep.cu)
 cudaError_t launch_fill(float *p, long long n, float v, cudaStream_t st);
 
-// ---- tile path (tile_path.cu): bounded motion, z-buffers in shared memory --------------------------
-struct TilePlan {
-    int tw, th;            // target tile (also the ordering tile)
-    int halo;              // source halo in pixels, >= ceil(max_motion_px) + 1
-    int tiles_x, tiles_y;
-    int threads;           // CTA size
-    int cand_cap;          // candidate sources kept in shared memory per tile
-    int smem_bytes;
-    int force_direct;      // test hook (EVIS_TILE_FORCE_DIRECT=1): never keep candidates resident
-    int ctas;              // persistent grid: SMs x resident CTAs per SM (set by tile_setup)
-    int slab;              // events per arrival slab a CTA reserves with one global atomic
-};
-bool plan_tile(const Geom &g, float max_motion_px, TilePlan *plan);     // false: motion too large for a tile
-cudaError_t tile_setup(const Geom &g, TilePlan &plan, int device);      // function attributes, persistent grid size
-// next_item: device work counter, zero before the launch (the persistent CTAs draw (env, tile) items from it)
-cudaError_t launch_tile(const Geom &g, const TilePlan &plan, const Keyframe &A, const Keyframe &B,
-                        const SubstepTable *tab_dev, float *l_ref, float *l_prev, const EventParams &ep,
-                        const EventSink &sink, unsigned long long *holes, unsigned long long *next_item,
-                        const DebugOut &dbg, cudaStream_t st);
-
 // ---- a8 ordering (order.cu) ----------------------------------------------------------------------
 // directory entry d = (arrival offset, count); ordered stream = chunks concatenated in d order, cut at
-// `capacity` events.  *step_events = events of this step is added to *total_events (running total).
+// `capacity` events.  *step_events = events of this step is added to *total_events (running total);
+// *overflow_steps counts the steps whose events did not all fit (sticky).
 constexpr int ORDER_ENTRIES_PER_BLOCK = 512;     // directory entries scanned and copied by one block
 cudaError_t launch_order(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out /*[n]*/,
                          uint4 *ordered, unsigned long long capacity, const unsigned long long *step_events,
-                         unsigned long long *total_events, cudaStream_t st);
+                         unsigned long long *total_events, unsigned long long *overflow_steps, cudaStream_t st);
 // The same for the global path's records: chunks are expanded to events (a7: timestamps) on the way.
 // tiles_x, tiles = tiles per row / per frame of the G_TILE_W x G_TILE_H tiling; S = substeps.
 cudaError_t launch_expand(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out, uint4 *ordered,
                           unsigned long long capacity, const unsigned long long *step_events,
-                          unsigned long long *total_events, const EventParams &ep, const Thresholds &th, uint32_t W,
+                          unsigned long long *total_events, unsigned long long *overflow_steps, const EventParams &ep, const Thresholds &th, uint32_t W,
                           uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st);
 // number of values among theta[0..n) that are not (finite and > 0), added to *bad (prep.cu)
 cudaError_t launch_check_positive(const float *theta, long long n, unsigned long long *bad, cudaStream_t st);

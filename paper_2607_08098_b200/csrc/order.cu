@@ -43,7 +43,7 @@ __device__ __forceinline__ unsigned long long block_scan_excl(unsigned long long
     return r;
 }
 
-// shift: 0 = the entry's .y is an event count (tile path), DIR_EV_SHIFT = records | events << shift (global path)
+// shift: 0 = the entry's .y is an event count (direct mode: the chunk holds events), DIR_EV_SHIFT = records | events << shift
 __global__ void __launch_bounds__(ORD_NT)
 k_dir_blocksum(const uint2 *__restrict__ dir, uint32_t n, unsigned long long *__restrict__ bsum, int shift)
 {
@@ -61,9 +61,13 @@ k_dir_blocksum(const uint2 *__restrict__ dir, uint32_t n, unsigned long long *__
 // single block: exclusive scan of the per-block sums in place
 __global__ void __launch_bounds__(1024)
 k_dir_scan_bsum(unsigned long long *__restrict__ bsum, uint32_t nb, const unsigned long long *__restrict__ step_events,
-                unsigned long long *__restrict__ total_events)
+                unsigned long long *__restrict__ total_events, const unsigned long long *__restrict__ alloc,
+                unsigned long long arrival_cap, unsigned long long capacity, unsigned long long *__restrict__ overflow_steps)
 {
-    if (threadIdx.x == 0) *total_events += *step_events;
+    if (threadIdx.x == 0) {
+        *total_events += *step_events;
+        if (*step_events > capacity || *alloc > arrival_cap) *overflow_steps += 1ull;      // sticky: evis_info.overflow_steps
+    }
     __shared__ unsigned long long s_w[33];
     const uint32_t per = (nb + blockDim.x - 1) / blockDim.x;
     const uint32_t lo = threadIdx.x * per, hi = min(lo + per, nb);
@@ -246,12 +250,12 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
 
 cudaError_t launch_expand(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
                           unsigned long long capacity, const unsigned long long *step_events,
-                          unsigned long long *total_events, const EventParams &ep, const Thresholds &th, uint32_t W,
+                          unsigned long long *total_events, unsigned long long *overflow_steps, const EventParams &ep, const Thresholds &th, uint32_t W,
                           uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st)
 {
     const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
     k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, DIR_EV_SHIFT);
-    k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events);
+    k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events, sink.alloc, sink.arrival_cap, capacity, overflow_steps);
     k_expand<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, sink.arrival_cap, ordered, capacity, ep, th,
                                     W, HW, margin, tiles_x, tiles, S);
     return cudaGetLastError();
@@ -259,11 +263,11 @@ cudaError_t launch_expand(const EventSink &sink, uint32_t n, unsigned long long 
 
 cudaError_t launch_order(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
                          unsigned long long capacity, const unsigned long long *step_events,
-                         unsigned long long *total_events, cudaStream_t st)
+                         unsigned long long *total_events, unsigned long long *overflow_steps, cudaStream_t st)
 {
     const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
     k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, 0);
-    k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events);
+    k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events, sink.alloc, sink.arrival_cap, capacity, overflow_steps);
     k_dir_copy<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, sink.arrival_cap, ordered, capacity);
     return cudaGetLastError();
 }

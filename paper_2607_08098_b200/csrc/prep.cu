@@ -33,7 +33,7 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
        float *__restrict__ Z, float *__restrict__ l_ref, float *__restrict__ l_prev, float bound,
        unsigned long long *__restrict__ viol)
 {
-    bool over = false;       // a motion vector beyond the bound the tile path was planned for
+    bool over = false;       // a motion vector beyond the bound the caller declared (max_motion_px)
     const double eps = (double)eps_f;
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (VEC) {

@@ -132,7 +132,8 @@ def compare_step(gpu_ev: np.ndarray, ora_ev: np.ndarray, ora: orc.Oracle, E: int
 def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Sequence[int]] = None,
                mode: int = 0, path: int = binding.PATH_GLOBAL, use_fwd: bool = True, debug: bool = True,
                capacity: int = 1 << 24, max_motion: Optional[float] = None, thresholds=None,
-               tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None, mutate=None) -> ParityReport:
+               tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None, mutate=None,
+               render_device: str = "cuda") -> ParityReport:
     """GPU runs the whole batch; the oracle runs ``envs`` (default: all).  Returns the report after
     asserting every bit-exact criterion; tolerances are asserted by the caller on the report."""
     sc = scenes.make_scene(spec)
@@ -158,7 +159,9 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
     rep = ParityReport()
     try:
         for k in range(n_keyframes):
-            kf = scenes.render_keyframe(sc, k, device="cuda")
+            kf = scenes.render_keyframe(sc, k, device=render_device)
+            if render_device != "cuda":             # rendered on the host (the generator is device-independent), copied over
+                kf = {key: v.cuda() for key, v in kf.items()}
             if mutate is not None:                  # degenerate-input cases: the test edits the keyframe in place
                 mutate(k, kf)
             fwd = kf["mv_fwd"] if use_fwd else None

@@ -34,7 +34,7 @@ def test_every_declared_symbol_is_exported(lib):
 def test_struct_layouts_match_the_header():
     assert C.sizeof(binding.evis_config) == 64
     assert binding.EVENT_DTYPE.itemsize == 16
-    assert C.sizeof(binding.evis_info) == 72
+    assert C.sizeof(binding.evis_info) == 80
 
 
 def test_argument_validation_needs_no_gpu(lib):

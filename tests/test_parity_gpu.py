@@ -11,18 +11,11 @@ from tests import parity
 
 pytestmark = pytest.mark.gpu
 
-PATHS = ["global", "tile"]
-TILE_MAX_MOTION = 23.0       # plan_tile() in tile_path.cu refuses larger motion bounds
+PATHS = ["global"]           # the per-tile shared-memory path of round 1 was retired
 
 
 def _path(name, spec):
-    """EVIS_PATH_AUTO resolves to the global path (the faster one on every BASELINE config); the tile path
-    is requested explicitly and exists only for bounded motion."""
-    if name == "global":
-        return binding.PATH_GLOBAL
-    if spec.max_motion_px() > TILE_MAX_MOTION:
-        pytest.skip("motion bound too large for the tile path")
-    return binding.PATH_TILE
+    return binding.PATH_GLOBAL
 
 
 def _assert_tolerances(rep):
@@ -102,31 +95,13 @@ def test_noise_stress(path, v_max, S):
     assert rep.holes > 0
 
 
-def test_tile_path_is_taken_and_direct_mode_matches(monkeypatch):
-    """PATH_TILE is honoured for bounded motion; with EVIS_TILE_FORCE_DIRECT=1 the tile kernel never keeps
-    candidates resident (the fallback for pools that overflow) and must give the same result."""
-    spec = scenes.small(scenes.config(4), num_envs=3, height=130, width=173, num_keyframes=3)
-    ev = binding.Evis(3, 130, 173, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
-                      max_motion_px=spec.max_motion_px(), path=binding.PATH_TILE)
-    info = ev.info()
-    assert info.path == binding.PATH_TILE and info.halo == int(np.ceil(spec.max_motion_px())) + 1
-    ev.destroy()
-    rep = parity.run_parity(spec, 3, path=binding.PATH_TILE)
-    _assert_tolerances(rep)
-    monkeypatch.setenv("EVIS_TILE_FORCE_DIRECT", "1")
-    rep = parity.run_parity(spec, 3, path=binding.PATH_TILE)
-    _assert_tolerances(rep)
-    nz = scenes.SceneSpec("noise", 1, 75, 131, 3, 1.0 / 60.0, 5, 0.3, 0.2, kind="noise", num_rects=0, v_max=600.0, seed=3)
-    rep = parity.run_parity(nz, 3, path=binding.PATH_TILE)
-    _assert_tolerances(rep)
-
-
-def test_tile_path_reports_motion_bound_violation():
-    """A motion vector beyond max_motion_px on the tile path is reported (EVIS_ERR_MOTION_BOUND)."""
+def test_declared_motion_bound_violation_is_reported():
+    """A motion vector beyond the max_motion_px the caller declared is reported (EVIS_ERR_MOTION_BOUND); the retired
+    tile path (path = 2) is INVALID_ARG."""
     spec = scenes.small(scenes.config(1), height=64, width=96, num_keyframes=2)
     sc = scenes.make_scene(spec)
     ev = binding.Evis(1, 64, 96, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
-                      max_motion_px=0.5, path=binding.PATH_TILE)
+                      max_motion_px=0.5, path=binding.PATH_GLOBAL)
     k0 = scenes.render_keyframe(sc, 0, device="cuda")
     assert float(k0["mv_bwd"].abs().max()) > 0.5
     ev.step(k0["rad"], k0["mv_bwd"], k0["depth"], sync=True)
@@ -136,11 +111,14 @@ def test_tile_path_reports_motion_bound_violation():
     assert ei.value.status == binding.EVIS_ERR_MOTION_BOUND
     assert ev.info().last_motion_violation == 1
     ev.destroy()
+    with pytest.raises(binding.EvisError) as ei:
+        binding.Evis(1, 64, 96, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, max_motion_px=8.0, path=2)
+    assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
 
 
-@pytest.mark.parametrize("path", [binding.PATH_TILE, binding.PATH_GLOBAL])
+@pytest.mark.parametrize("path", [binding.PATH_GLOBAL])
 def test_static_scene_shortcuts(path):
-    """Zero motion everywhere: the tile path's static-tile shortcut and the global splat's static-source
+    """Zero motion everywhere: the splat's static-source
     loop; a pure brightness change lands in substep 1 (R19 note) and matches the oracle."""
     spec = scenes.SceneSpec("static", 2, 70, 100, 3, 1.0 / 60.0, 8, 0.02, 0.025, num_rects=5, v_max=0.0,
                             ramp_max=30.0, seed=21)
@@ -245,8 +223,7 @@ def test_threshold_maps_eq8():
 
 def test_threshold_maps_api_contract():
     """evis_set_thresholds: one NULL map or a non-positive value is INVALID_ARG and leaves the thresholds in
-    force; constant maps equal the scalar thresholds event for event; (NULL, NULL) restores the scalars; the tile
-    path refuses the maps."""
+    force; constant maps equal the scalar thresholds event for event; (NULL, NULL) restores the scalars."""
     spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=3)
     E, H, W = spec.num_envs, spec.height, spec.width
     sc = scenes.make_scene(spec)
@@ -288,13 +265,6 @@ def test_threshold_maps_api_contract():
         ev.set_thresholds(None, None)
     assert np.array_equal(base, run(set_and_clear))
     assert len(run(lambda ev: ev.set_thresholds(on * 3.0, off * 3.0))) < len(base)
-
-    ev = binding.Evis(E, H, W, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
-                      max_motion_px=spec.max_motion_px(), path=binding.PATH_TILE, event_capacity=1 << 22)
-    with pytest.raises(binding.EvisError) as ei:
-        ev.set_thresholds(on, off)
-    assert ei.value.status == binding.EVIS_ERR_BAD_STATE
-    ev.destroy()
 
 
 @pytest.mark.parametrize("tau_r,with_maps", [(0.0005, False), (0.003, False), (0.02, True)])
@@ -397,9 +367,76 @@ def test_noise_events(tau_r, margin):
     assert n_noise > 0.5 * 3 * E * (H - 2 * margin) * (W - 2 * margin) * (20.0 + 400.0 * 0.02) * spec.keyframe_dt
 
 
+@pytest.mark.parametrize("order", ["refractory_then_thresholds", "noise_then_thresholds", "thresholds_noise_thresholds_off",
+                                   "everything_twice"])
+def test_setters_in_any_order(order):
+    """The feature setters own separate device state: whatever the call order, the run must be the oracle's with the
+    features that are in force (round 1 freed t_last and the hot set inside evis_set_thresholds), and the context's
+    device_bytes must count every buffer once."""
+    from oracle import evis_oracle as orc
+    spec = scenes.small(scenes.config(4), num_envs=2, height=97, width=131, num_keyframes=4)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    P = E * H * W
+    th = scenes.threshold_maps(spec, sigma=0.04, theta_min=0.02, device="cuda")
+    th_np = (th[0].cpu().numpy(), th[1].cpu().numpy())
+    gen = torch.Generator().manual_seed(6)
+    hot = (torch.rand((E, H, W), generator=gen) < 0.03).to(torch.uint8)
+    par = dict(seed=7, r_leak=30.0, r_shot=50.0, r_hot=300.0, i_white=1.5)
+    tau = 0.002
+    ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, event_capacity=1 << 24)
+    b0 = ev.info().device_bytes
+    okw = {}
+    if order == "refractory_then_thresholds":
+        ev.set_refractory(tau)
+        ev.set_thresholds(*th)
+        okw = dict(theta_on=th_np[0], theta_off=th_np[1], tau_r=tau)
+        extra = 4 * P + 8 * P
+    elif order == "noise_then_thresholds":
+        ev.set_noise(hot=hot.cuda(), **par)
+        ev.set_thresholds(*th)
+        okw = dict(theta_on=th_np[0], theta_off=th_np[1], noise=dict(par, hot=hot.numpy()))
+        extra = P + 4 * P + 8 * P
+    elif order == "thresholds_noise_thresholds_off":
+        ev.set_thresholds(*th)
+        ev.set_noise(hot=hot.cuda(), **par)
+        ev.set_thresholds(None, None)
+        okw = dict(noise=dict(par, hot=hot.numpy()))
+        extra = 8 * P + P + 4 * P
+    else:
+        ev.set_noise(hot=hot.cuda(), **par)
+        ev.set_noise(**par)                       # drops the hot set
+        ev.set_refractory(tau)
+        ev.set_thresholds(th[0] * 2.0, th[1] * 2.0)
+        ev.set_thresholds(*th)                    # replaces the maps
+        ev.set_refractory(tau)                    # resets t_last, keeps the buffer
+        okw = dict(theta_on=th_np[0], theta_off=th_np[1], tau_r=tau, noise=dict(par))
+        extra = 4 * P + 8 * P
+    assert ev.info().device_bytes == b0 + extra
+    ora = orc.Oracle(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, **okw)
+    sc = scenes.make_scene(spec)
+    total = 0
+    for k in range(4):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        n = ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        h = {key: v.cpu().numpy() for key, v in kf.items()}
+        oe = ora.step(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"])
+        ge = ev.read_events()
+        assert n == len(ge) == len(oe)
+        total += n
+        g = ge[np.lexsort((ge["t_off"], ge["x"], ge["y"], ge["substep"], ge["env"]))]
+        o = oe[np.lexsort((oe["t_off"], oe["x"], oe["y"], oe["substep"], oe["env"]))]
+        for f in ("env", "x", "y", "substep", "p"):
+            assert np.array_equal(g[f].astype(np.int64), o[f].astype(np.int64)), f
+        if n:
+            assert float(np.max(np.abs(g["t_off"].astype(np.float64) - o["t_off"]))) <= parity.TOL_T
+        if k:
+            assert np.array_equal(ev.get_state()[0], ora.Lref)
+    assert total > 0
+    ev.destroy()
+
+
 def test_noise_api_contract():
-    """evis_set_noise: bad rates are INVALID_ARG; switching it off restores the plain stream exactly; the tile path
-    refuses it."""
+    """evis_set_noise: bad rates are INVALID_ARG; switching it off restores the plain stream exactly."""
     spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=3)
     E, H, W = spec.num_envs, spec.height, spec.width
     sc = scenes.make_scene(spec)
@@ -431,11 +468,6 @@ def test_noise_api_contract():
     assert np.array_equal(noisy, run(lambda ev: ev.set_noise(seed=1, r_leak=50.0)))      # deterministic
     assert not np.array_equal(noisy, run(lambda ev: ev.set_noise(seed=2, r_leak=50.0)))
 
-    def tile(ev):
-        with pytest.raises(binding.EvisError) as ei:
-            ev.set_noise(seed=1, r_leak=1.0)
-        assert ei.value.status == binding.EVIS_ERR_BAD_STATE
-    run(tile, path=binding.PATH_TILE)
 
 
 @pytest.mark.parametrize("path", PATHS)
@@ -500,7 +532,7 @@ def test_degenerate_inputs(use_fwd):
 
 def test_margin_api_contract():
     """evis_set_margin: negative or too large margins are INVALID_ARG; margin 0 is the plain frame; coordinates
-    of a margin run stay inside the cropped frame; the tile path refuses it."""
+    of a margin run stay inside the cropped frame."""
     spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=3)
     E, H, W = spec.num_envs, spec.height, spec.width
     sc = scenes.make_scene(spec)
@@ -538,11 +570,6 @@ def test_margin_api_contract():
     key = lambda a: np.sort(a, order=["kf", "env", "substep", "y", "x", "t_off"])
     assert np.array_equal(key(ref), key(crop))
 
-    def tile(ev):
-        with pytest.raises(binding.EvisError) as ei:
-            ev.set_margin(4)
-        assert ei.value.status == binding.EVIS_ERR_BAD_STATE
-    run(tile, path=binding.PATH_TILE)
 
 
 def test_checkpoint_resume_with_refractory_state():
@@ -568,10 +595,45 @@ def test_checkpoint_resume_with_refractory_state():
         mk().get_t_last()                                             # BAD_STATE: the feature is off
     step(b, 3)
     b.set_state(lref, lprev); b.set_t_last(tl)
+    b.set_interval_index(3)
     for i, k in enumerate((4, 5)):
         step(b, k)
         got = b.read_events().copy()
-        got["kf"] = want[i]["kf"]                                     # interval numbering restarts in the new context
+        assert len(got) > 0 and np.array_equal(got, want[i])
+    b.destroy()
+
+
+def test_checkpoint_resume_of_a_noise_run():
+    """The noise generator is keyed by the interval index (R29): a resumed context told the index it continues with
+    (evis_set_interval_index) draws the same noise events and stamps the same kf as the uninterrupted run."""
+    spec = scenes.small(scenes.config(4), num_envs=2, height=97, width=131, num_keyframes=6)
+    sc = scenes.make_scene(spec)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(6)]
+    par = dict(seed=5, r_leak=40.0, r_shot=80.0, i_white=1.5)
+
+    def mk():
+        ev = binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps,
+                          spec.keyframe_dt, event_capacity=1 << 24)
+        ev.set_noise(**par)
+        ev.set_refractory(0.002)
+        return ev
+    step = lambda ev, k: ev.step(kfs[k]["rad"], kfs[k]["mv_bwd"], kfs[k]["depth"], mv_fwd=kfs[k]["mv_fwd"], sync=True)
+    a = mk()
+    for k in range(4):
+        step(a, k)
+    lref, lprev = a.get_state()
+    tl = a.get_t_last()
+    want = []
+    for k in (4, 5):
+        step(a, k); want.append(a.read_events().copy())
+    a.destroy()
+    b = mk()
+    step(b, 3)                                                        # keyframe A of the interval it continues with
+    b.set_state(lref, lprev); b.set_t_last(tl)
+    b.set_interval_index(3)                                           # keyframes 3 -> 4 close interval 3
+    for i, k in enumerate((4, 5)):
+        step(b, k)
+        got = b.read_events().copy()
         assert len(got) > 0 and np.array_equal(got, want[i])
     b.destroy()
 
@@ -605,8 +667,7 @@ def test_split_host_read_matches_the_plain_one():
 
 
 def test_refractory_api_contract():
-    """evis_set_refractory: negative or non-finite tau_r is INVALID_ARG; tau_r = 0 restores the plain stream; the
-    tile path refuses it."""
+    """evis_set_refractory: negative or non-finite tau_r is INVALID_ARG; tau_r = 0 restores the plain stream."""
     spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=3)
     E, H, W = spec.num_envs, spec.height, spec.width
     sc = scenes.make_scene(spec)
@@ -639,11 +700,6 @@ def test_refractory_api_contract():
     sup = run(lambda ev: ev.set_refractory(0.004))
     assert 0 < len(sup) < len(base)
 
-    def tile(ev):
-        with pytest.raises(binding.EvisError) as ei:
-            ev.set_refractory(0.01)
-        assert ei.value.status == binding.EVIS_ERR_BAD_STATE
-    run(tile, path=binding.PATH_TILE)
 
 
 def _run_stream(spec, n_kf, path, seed_offset=0):
@@ -728,8 +784,32 @@ def test_event_capacity_overflow_is_reported():
         ev.step(k1["rad"], k1["mv_bwd"], k1["depth"], sync=True)
     assert ei.value.status == binding.EVIS_ERR_OVERFLOW
     info = ev.info()
-    assert info.last_overflow == 1 and info.last_events > 100
-    assert len(ev.read_events()) == 100
+    # 100 slots hold neither the events nor the intermediate records: nothing valid is stored, and the read says so
+    assert info.last_overflow == 2 and info.last_events > 100 and info.overflow_steps == 1
+    with pytest.raises(binding.EvisError) as ei:
+        ev.read_events()
+    assert ei.value.status == binding.EVIS_ERR_OVERFLOW
+    assert len(ev.read_events(allow=(binding.EVIS_ERR_OVERFLOW,))) == 0
+    ev.destroy()
+    # capacity for the records but not for all events: the stored stream is the true prefix of the deterministic order
+    full = binding.Evis(2, 120, 160, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                        event_capacity=1 << 22)
+    full.step(k0["rad"], k0["mv_bwd"], k0["depth"], sync=True)
+    n_all = full.step(k1["rad"], k1["mv_bwd"], k1["depth"], sync=True)
+    want = full.read_events().copy()
+    full.destroy()
+    cap = n_all - 1000
+    ev = binding.Evis(2, 120, 160, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                      event_capacity=cap)
+    ev.step(k0["rad"], k0["mv_bwd"], k0["depth"], sync=True)
+    n = ev.step(k1["rad"], k1["mv_bwd"], k1["depth"], sync=True, allow=(binding.EVIS_ERR_OVERFLOW,))
+    info = ev.info()
+    if info.last_overflow == 1:                        # (records <= events, so this is the case unless no pixel fires twice)
+        got = ev.read_events(allow=(binding.EVIS_ERR_OVERFLOW,))
+        assert n == n_all and len(got) == cap and np.array_equal(got, want[:cap])
+    else:
+        assert info.last_overflow == 2
+    assert info.overflow_steps == 1
     ev.destroy()
 
 
