@@ -190,7 +190,8 @@ int evis_set_channel(evis_ctx *ctx, int channel);
  * the margin is cropped off afterwards: the event model runs and events exist only for the inner
  * (height - 2 margin) x (width - 2 margin) pixels, x and y of an event are relative to that cropped frame, holes are
  * counted inside it.  0 = no margin (default).  Applies from the next evis_step on; synchronises.  
- * Errors: INVALID_ARG (negative, or 2 margin >= min(height, width)), CUDA. */
+ * Errors: INVALID_ARG (negative, or 2 margin >= min(height, width)), BAD_STATE (a voxel grid is on: its shape is
+ * the cropped frame's, so the margin comes first), CUDA. */
 int evis_set_margin(evis_ctx *ctx, int margin);
 
 /* Refractory period (R26): with tau_r > 0 (seconds) a threshold crossing of a pixel is
@@ -201,6 +202,38 @@ int evis_set_margin(evis_ctx *ctx, int margin);
  * again with tau_r > 0 resets t_last.  Applies from the next evis_step on; synchronises.  
  * Errors: INVALID_ARG (negative or non-finite tau_r), CUDA, OOM. */
 int evis_set_refractory(evis_ctx *ctx, float tau_r);
+
+/* Voxel grid / accumulation image ("a per-polarity event voxel grid discretized into 128 temporal bins
+ * with linear interpolation applied along the time axis. Each bin is normalized by dividing by its maximum event
+ * count"; R30).  The library accumulates, on the device and in the same pass that lays
+ * out the event stream, V [E, 2, bins, H', W'] (H' x W' = the frame after the margin crop; channel 0 = ON, 1 = OFF) over
+ * a WINDOW of `window_steps` consecutive keyframe intervals: with t the time of an event from the start of the window
+ * and D = window_steps * T, tau = (bins - 1) t / D, and the event adds max(0, 1 - |tau - b|) to bin b of its pixel and
+ * polarity channel -- the two bins that bracket tau share one unit; bins = 1 is the plain per-polarity event count.
+ * The sums are kept in 32.32 fixed point with integer atomics, so they do not depend on scheduling.  The first
+ * window starts with the next evis_step that closes an interval; when a window is full the next step clears the grid
+ * and starts a new one (read it before).  keep_events = 0: the ordered event stream is not stored at all (the read
+ * calls for events then return BAD_STATE) -- no 16-byte event ever leaves the GPU.  cfg = NULL switches the grid off.
+ * Synchronises.  Errors: INVALID_ARG (bins < 1, window_steps < 1), CUDA, OOM. */
+typedef struct {
+    int32_t bins;            /* B >= 1 temporal bins per window                                  */
+    int32_t window_steps;    /* N >= 1 keyframe intervals per window                             */
+    int32_t keep_events;     /* 1: the ordered event stream is produced as well                  */
+    int32_t reserved;
+} evis_voxel_config;
+int evis_set_voxels(evis_ctx *ctx, const evis_voxel_config *cfg);
+
+/* Copy the grid as float32 [E, 2, bins, H', W'] to `dst` (device pointer if dst_is_device != 0, else host).
+ * normalize != 0: every (env, channel, bin) plane is divided by its own maximum when that is > 0.
+ * restart != 0: the next step starts a new window (clears the grid) even if this one is not full.
+ * *n_intervals (nullable) = keyframe intervals accumulated in the window so far.  Synchronises.
+ * Errors: INVALID_ARG, BAD_STATE (grid off), CUDA. */
+int evis_read_voxels(evis_ctx *ctx, float *dst, int dst_is_device, int normalize, int restart, uint32_t *n_intervals);
+/* The same to HOST memory (pinned, for a real overlap) in two halves, like evis_read_events_begin / _end: _begin
+ * enqueues the conversion and the copy behind the last step and returns without waiting; _end waits for the copy.
+ * The next step's accumulation waits for the copy too. */
+int evis_read_voxels_begin(evis_ctx *ctx, float *host_dst, int normalize, int restart);
+int evis_read_voxels_end(evis_ctx *ctx);
 
 /* Copy the events of the last step, in the deterministic order
  * (env, substep, tile row, tile column, y, x, crossing k), to `dst` (room for `max` events;

@@ -55,7 +55,7 @@ class evis_profile(C.Structure):
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
            "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end",
-           "evis_set_interval_index"]
+           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end"]
 
 _lib = None
 
@@ -94,12 +94,20 @@ def load() -> C.CDLL:
     L.evis_read_events_end.argtypes = [vp]
     L.evis_refractory_state.argtypes = [vp, vp, vp]
     L.evis_set_noise.argtypes = [vp, C.POINTER(evis_noise), vp, C.c_int]
+    L.evis_set_voxels.argtypes = [vp, C.POINTER(evis_voxel_config)]
+    L.evis_read_voxels.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_uint32)]
+    L.evis_read_voxels_begin.argtypes = [vp, vp, C.c_int, C.c_int]
+    L.evis_read_voxels_end.argtypes = [vp]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
     for name in SYMBOLS:
         getattr(L, name)              # raises AttributeError if the library lacks a declared symbol
     _lib = L
     return L
+
+
+class evis_voxel_config(C.Structure):
+    _fields_ = [("bins", C.c_int32), ("window_steps", C.c_int32), ("keep_events", C.c_int32), ("reserved", C.c_int32)]
 
 
 class evis_noise(C.Structure):
@@ -197,6 +205,37 @@ class Evis:
             hp = hot.data_ptr()
         _check(self._lib.evis_set_noise(self._ctx, C.byref(cfg), hp, 1), "evis_set_noise")
 
+    def set_voxels(self, bins: Optional[int], window_steps: int = 1, keep_events: bool = True) -> None:
+        """evis_set_voxels: per-polarity voxel grid [E, 2, bins, H', W'] over windows of `window_steps` intervals
+        (PAPER.md:331); bins = None switches it off."""
+        if bins is None:
+            _check(self._lib.evis_set_voxels(self._ctx, None), "evis_set_voxels")
+            self._vox = None
+            return
+        cfg = evis_voxel_config(int(bins), int(window_steps), int(bool(keep_events)), 0)
+        _check(self._lib.evis_set_voxels(self._ctx, C.byref(cfg)), "evis_set_voxels")
+        self._vox = int(bins)
+
+    def voxel_shape(self) -> Tuple[int, int, int, int, int]:
+        m = getattr(self, "_margin", 0)
+        return (self.E, 2, self._vox, self.H - 2 * m, self.W - 2 * m)
+
+    def read_voxels(self, normalize: bool = False, restart: bool = False) -> Tuple[np.ndarray, int]:
+        """evis_read_voxels to a new host array; returns (grid float32, intervals accumulated in the window)."""
+        out = np.empty(self.voxel_shape(), np.float32)
+        n = C.c_uint32(0)
+        _check(self._lib.evis_read_voxels(self._ctx, out.ctypes.data, 0, int(normalize), int(restart), C.byref(n)),
+               "evis_read_voxels")
+        return out, int(n.value)
+
+    def read_voxels_begin(self, host_buf: np.ndarray, normalize: bool = False, restart: bool = False) -> None:
+        assert host_buf.dtype == np.float32 and host_buf.flags.c_contiguous and host_buf.size == int(np.prod(self.voxel_shape()))
+        _check(self._lib.evis_read_voxels_begin(self._ctx, host_buf.ctypes.data, int(normalize), int(restart)),
+               "evis_read_voxels_begin")
+
+    def read_voxels_end(self) -> None:
+        _check(self._lib.evis_read_voxels_end(self._ctx), "evis_read_voxels_end")
+
     def set_channel(self, channel: int) -> None:
         """evis_set_channel (colour events): 0 / 1 / 2 = log of R / G / B, -1 = Rec.709 luminance."""
         _check(self._lib.evis_set_channel(self._ctx, int(channel)), "evis_set_channel")
@@ -208,6 +247,7 @@ class Evis:
     def set_margin(self, margin: int) -> None:
         """evis_set_margin: the frames carry `margin` over-rendered pixels per side, cropped after the warp."""
         _check(self._lib.evis_set_margin(self._ctx, int(margin)), "evis_set_margin")
+        self._margin = int(margin)
 
     def set_refractory(self, tau_r: float) -> None:
         """evis_set_refractory: refractory period in seconds, 0 = off; resets the per-pixel state."""

@@ -76,6 +76,14 @@ struct evis_ctx {
     unsigned long long arrival_cap;   // slots of the arrival buffer (capacity + slab slack)
     DebugOut dbg;
 
+    // voxel grid (evis_set_voxels): V in 32.32 fixed point, its float32 image for the read calls
+    bool vox_on, vox_restart;
+    evis_voxel_config vox;
+    unsigned long long *vox_v;
+    float *vox_out;
+    uint32_t vox_j;                   // intervals accumulated in the current window
+    size_t vox_cells;                 // E * 2 * bins * H' * W'
+
     // host-buffer entry point staging
     float *st_rad, *st_mv, *st_fwd, *st_depth;
 
@@ -198,6 +206,7 @@ void free_all(evis_ctx *ctx)
     cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last); cudaFree(ctx->hot); cudaFree(ctx->tab); cudaFree(ctx->zmem);
     cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
+    cudaFree(ctx->vox_v); cudaFree(ctx->vox_out);
     cudaFree(ctx->st_rad); cudaFree(ctx->st_mv); cudaFree(ctx->st_fwd); cudaFree(ctx->st_depth);
     if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
     prof_drain(ctx);
@@ -571,6 +580,23 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     CU(cudaEventRecord(ctx->ev_chunks[sl], st));
     CU(cudaStreamWaitEvent(os, ctx->ev_chunks[sl], 0));
     if (ctx->copy_pending) CU(cudaStreamWaitEvent(os, ctx->ev_copy, 0));   // `ordered` is still being copied out
+    VoxelSink vs{};
+    vs.store_events = 1;
+    if (ctx->vox_on) {
+        if (ctx->vox_restart || ctx->vox_j >= (uint32_t)ctx->vox.window_steps) {     // a new window starts with this interval
+            CU(cudaMemsetAsync(ctx->vox_v, 0, ctx->vox_cells * sizeof(unsigned long long), os));
+            ctx->vox_j = 0;
+            ctx->vox_restart = false;
+        }
+        volatile float tb = (float)ctx->vox_j * ctx->cfg.keyframe_dt;
+        volatile float sc = (float)(ctx->vox.bins - 1) / ((float)ctx->vox.window_steps * ctx->cfg.keyframe_dt);
+        vs.v = ctx->vox_v;
+        vs.bins = (uint32_t)ctx->vox.bins;
+        vs.hc = (uint32_t)(g.H - 2 * g.margin); vs.wc = (uint32_t)(g.W - 2 * g.margin);
+        vs.t_base = tb; vs.scale = sc;
+        vs.store_events = ctx->vox.keep_events != 0;
+        ctx->vox_j += 1;
+    }
     {
         Span sp(ctx, os, EVIS_STAGE_ORDER, 3);
         unsigned long long *sticky = ctx->counters_s[0];             // C_MOTION, C_TOTAL live in slot 0's array
@@ -578,10 +604,10 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
             const uint32_t tx = (g.W + G_TILE_W - 1) / G_TILE_W, ty = (g.H + G_TILE_H - 1) / G_TILE_H;
             CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
                              cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, ctx->ep, th, (uint32_t)g.W,
-                             (uint32_t)g.HW, (uint32_t)g.margin, tx, tx * ty, (uint32_t)g.S, os));
+                             (uint32_t)g.HW, (uint32_t)g.margin, tx, tx * ty, (uint32_t)g.S, vs, os));
         } else {
             CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
-                            cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, os));
+                            cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, vs, os));
         }
         CU(cudaMemcpyAsync(ctx->h_counters, cnt, C_STEP_END * sizeof(unsigned long long), cudaMemcpyDeviceToHost, os));
         CU(cudaMemcpyAsync(ctx->h_counters + C_MOTION, sticky + C_MOTION, (NCOUNTERS - C_MOTION) * sizeof(unsigned long long),
@@ -686,6 +712,84 @@ int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_ma
     return EVIS_OK;
 }
 
+int evis_set_voxels(evis_ctx *ctx, const evis_voxel_config *cfg)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    if (cfg && (cfg->bins < 1 || cfg->bins > 65535 || cfg->window_steps < 1)) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->steps) CU(sync_all(ctx));
+    if (ctx->copy_pending) { CU(cudaStreamSynchronize(ctx->copy_stream)); ctx->copy_pending = false; }
+    if (ctx->vox_v) {
+        ctx->device_bytes -= ctx->vox_cells * (sizeof(unsigned long long) + sizeof(float));
+        cudaFree(ctx->vox_v); cudaFree(ctx->vox_out);
+        ctx->vox_v = nullptr; ctx->vox_out = nullptr;
+    }
+    ctx->vox_on = false;
+    if (!cfg) return EVIS_OK;
+    const Geom &g = ctx->g;
+    ctx->vox_cells = (size_t)g.E * 2u * (size_t)cfg->bins * (size_t)(g.H - 2 * g.margin) * (size_t)(g.W - 2 * g.margin);
+    CU(dalloc(ctx, &ctx->vox_v, ctx->vox_cells));
+    CU(dalloc(ctx, &ctx->vox_out, ctx->vox_cells));
+    CU(cudaMemset(ctx->vox_v, 0, ctx->vox_cells * sizeof(unsigned long long)));
+    ctx->vox = *cfg;
+    ctx->vox_j = 0;
+    ctx->vox_restart = false;
+    ctx->vox_on = true;
+    return EVIS_OK;
+}
+
+// enqueue V -> float32 behind the last step's order stage (and behind a copy of the previous image still running)
+static int voxel_finish(evis_ctx *ctx, int normalize)
+{
+    const Geom &g = ctx->g;
+    const uint32_t plane = (uint32_t)(g.H - 2 * g.margin) * (uint32_t)(g.W - 2 * g.margin);
+    if (ctx->copy_pending) CU(cudaStreamWaitEvent(ctx->ord_stream, ctx->ev_copy, 0));
+    if (ctx->last_stream || ctx->steps) {                     // a step's order stage follows its chunk phase on ord_stream already;
+        CU(cudaEventRecord(ctx->ev_chunks[0], ctx->last_stream));     // this covers a context that has only seen its first keyframe
+        CU(cudaStreamWaitEvent(ctx->ord_stream, ctx->ev_chunks[0], 0));
+    }
+    CU(launch_voxel_finish(ctx->vox_v, ctx->vox_out, (uint32_t)(ctx->vox_cells / plane), plane, normalize, ctx->ord_stream));
+    ctx->launches += 1;
+    return EVIS_OK;
+}
+
+int evis_read_voxels(evis_ctx *ctx, float *dst, int dst_is_device, int normalize, int restart, uint32_t *n_intervals)
+{
+    if (!ctx || !dst) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->vox_on) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->copy_pending) { CU(cudaStreamSynchronize(ctx->copy_stream)); ctx->copy_pending = false; }
+    const int rc = voxel_finish(ctx, normalize);
+    if (rc != EVIS_OK) return rc;
+    CU(cudaStreamSynchronize(ctx->ord_stream));
+    CU(cudaMemcpy(dst, ctx->vox_out, ctx->vox_cells * sizeof(float), dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    if (n_intervals) *n_intervals = ctx->vox_j;
+    if (restart) ctx->vox_restart = true;
+    return EVIS_OK;
+}
+
+int evis_read_voxels_begin(evis_ctx *ctx, float *host_dst, int normalize, int restart)
+{
+    if (!ctx || !host_dst) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->vox_on) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->copy_pending) { CU(cudaStreamSynchronize(ctx->copy_stream)); ctx->copy_pending = false; }
+    const int rc = voxel_finish(ctx, normalize);
+    if (rc != EVIS_OK) return rc;
+    CU(cudaEventRecord(ctx->ev_copy, ctx->ord_stream));
+    CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_copy, 0));
+    CU(cudaMemcpyAsync(host_dst, ctx->vox_out, ctx->vox_cells * sizeof(float), cudaMemcpyDeviceToHost, ctx->copy_stream));
+    CU(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
+    ctx->copy_pending = true;
+    if (restart) ctx->vox_restart = true;
+    return EVIS_OK;
+}
+
+int evis_read_voxels_end(evis_ctx *ctx) { return evis_read_events_end(ctx); }
+
 int evis_set_interval_index(evis_ctx *ctx, uint32_t next_kf)
 {
     if (!ctx) return EVIS_ERR_INVALID_ARG;
@@ -705,6 +809,7 @@ int evis_set_margin(evis_ctx *ctx, int margin)
 {
     if (!ctx) return EVIS_ERR_INVALID_ARG;
     if (margin < 0 || 2 * (long long)margin >= (ctx->g.H < ctx->g.W ? ctx->g.H : ctx->g.W)) return EVIS_ERR_INVALID_ARG;
+    if (ctx->vox_on) return EVIS_ERR_BAD_STATE;       // the voxel grid has the cropped frame's shape: set the margin first
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     if (ctx->steps) CU(sync_all(ctx));
@@ -758,7 +863,7 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
 int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t max, uint64_t *n_out)
 {
     if (!ctx || (!dst && max > 0)) return EVIS_ERR_INVALID_ARG;
-    if (!ctx->have_events) return EVIS_ERR_BAD_STATE;
+    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events)) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     const int rc = fetch_counters(ctx);
@@ -774,7 +879,7 @@ int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t
 int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, uint64_t *n_out)
 {
     if (!ctx || (!host_dst && max > 0)) return EVIS_ERR_INVALID_ARG;
-    if (!ctx->have_events) return EVIS_ERR_BAD_STATE;
+    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events)) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     const int rc = fetch_counters(ctx);
@@ -804,7 +909,7 @@ int evis_read_events_end(evis_ctx *ctx)
 int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_stored)
 {
     if (!ctx || !dev_ptr || !n_stored) return EVIS_ERR_INVALID_ARG;
-    if (!ctx->have_events) return EVIS_ERR_BAD_STATE;
+    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events)) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     const int rc = fetch_counters(ctx);
     if (rc != EVIS_OK) return rc;

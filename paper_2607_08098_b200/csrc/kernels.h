@@ -110,6 +110,21 @@ EVIS_DECL_RESOLVE(launch_resolve_m1d);
 // fill n floats with v (prep.cu)
 cudaError_t launch_fill(float *p, long long n, float v, cudaStream_t st);
 
+// ---- voxel grid / accumulation image (reading R30) ------------------------------------------
+// V [E][2][bins][hc][wc] in 32.32 fixed point (integer atomics: the sum does not depend on the order of the adds).
+// An event of polarity channel c (ON 0, OFF 1) at window time t adds 1 - w to bin b0 = floor(tau) and w to b0 + 1,
+// tau = min((t_base + t_off) * scale, bins - 1), w = tau - b0: linear interpolation along the time axis.
+struct VoxelSink {
+    unsigned long long *v;      // null = off
+    uint32_t bins, hc, wc;
+    float t_base;               // start of this interval relative to the start of the window (j * T)
+    float scale;                // (bins - 1) / (window_steps * T)
+    int store_events;           // 0: the ordered stream is not written (voxels only)
+};
+// V -> float32 (out, same shape); normalize: every (env, channel, bin) plane divided by its maximum
+cudaError_t launch_voxel_finish(const unsigned long long *v, float *out, uint32_t planes, uint32_t cells, int normalize,
+                                cudaStream_t st);
+
 // ---- a8 ordering (order.cu) ----------------------------------------------------------------------
 // directory entry d = (arrival offset, count); ordered stream = chunks concatenated in d order, cut at
 // `capacity` events.  *step_events = events of this step is added to *total_events (running total);
@@ -117,13 +132,13 @@ cudaError_t launch_fill(float *p, long long n, float v, cudaStream_t st);
 constexpr int ORDER_ENTRIES_PER_BLOCK = 512;     // directory entries scanned and copied by one block
 cudaError_t launch_order(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out /*[n]*/,
                          uint4 *ordered, unsigned long long capacity, const unsigned long long *step_events,
-                         unsigned long long *total_events, unsigned long long *overflow_steps, cudaStream_t st);
+                         unsigned long long *total_events, unsigned long long *overflow_steps, const VoxelSink &vox, cudaStream_t st);
 // The same for the global path's records: chunks are expanded to events (a7: timestamps) on the way.
 // tiles_x, tiles = tiles per row / per frame of the G_TILE_W x G_TILE_H tiling; S = substeps.
 cudaError_t launch_expand(const EventSink &sink, uint32_t num_entries, unsigned long long *scan_out, uint4 *ordered,
                           unsigned long long capacity, const unsigned long long *step_events,
                           unsigned long long *total_events, unsigned long long *overflow_steps, const EventParams &ep, const Thresholds &th, uint32_t W,
-                          uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st);
+                          uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, const VoxelSink &vox, cudaStream_t st);
 // number of values among theta[0..n) that are not (finite and > 0), added to *bad (prep.cu)
 cudaError_t launch_check_positive(const float *theta, long long n, unsigned long long *bad, cudaStream_t st);
 

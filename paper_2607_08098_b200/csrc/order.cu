@@ -43,6 +43,20 @@ __device__ __forceinline__ unsigned long long block_scan_excl(unsigned long long
     return r;
 }
 
+// One event into the voxel grid (kernels.h): xy = cropped pixel, w1 = env | polarity << 16 | substep << 24.
+__device__ __forceinline__ void voxel_add(const VoxelSink &vox, uint32_t xy, uint32_t w1, float t_off)
+{
+    const float tau = fminf(__fmul_rn(__fadd_rn(vox.t_base, t_off), vox.scale), (float)(vox.bins - 1u));
+    const float b0f = floorf(tau);
+    const uint32_t b0 = (uint32_t)b0f;
+    const unsigned long long q = __float2ull_rd(__fmul_rn(__fsub_rn(tau, b0f), 4294967296.0f));      // w in 32.32, exact
+    const uint32_t ch = ((w1 >> 16) & 0xFFu) == 0x01u ? 0u : 1u;
+    const size_t plane = (size_t)vox.hc * vox.wc;
+    const size_t cell = (((size_t)(w1 & 0xFFFFu) * 2u + ch) * vox.bins + b0) * plane + (size_t)(xy >> 16) * vox.wc + (xy & 0xFFFFu);
+    atomicAdd(vox.v + cell, 0x100000000ull - q);
+    if (q && b0 + 1u < vox.bins) atomicAdd(vox.v + cell + plane, q);
+}
+
 // shift: 0 = the entry's .y is an event count (direct mode: the chunk holds events), DIR_EV_SHIFT = records | events << shift
 __global__ void __launch_bounds__(ORD_NT)
 k_dir_blocksum(const uint2 *__restrict__ dir, uint32_t n, unsigned long long *__restrict__ bsum, int shift)
@@ -84,7 +98,7 @@ k_dir_scan_bsum(unsigned long long *__restrict__ bsum, uint32_t nb, const unsign
 __global__ void __launch_bounds__(ORD_NT)
 k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__restrict__ bsum,
            const uint4 *__restrict__ arrival, unsigned long long arrival_cap, uint4 *__restrict__ ordered,
-           unsigned long long cap)
+           unsigned long long cap, const VoxelSink vox)
 {
     __shared__ unsigned long long s_w[33];
     __shared__ uint32_t s_rel[ORD_PER_BLOCK + 1];     // first output position of chunk e, relative to the block
@@ -129,7 +143,10 @@ k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *
         }
 #pragma unroll
         for (int u = 0; u < U; ++u)
-            if (ok[u]) ordered[out0 + o0 + u * ORD_NT] = val[u];
+            if (ok[u]) {
+                if (vox.store_events) ordered[out0 + o0 + u * ORD_NT] = val[u];
+                if (vox.v) voxel_add(vox, val[u].x, val[u].y, __uint_as_float(val[u].z));
+            }
     }
 }
 
@@ -144,7 +161,7 @@ __global__ void __launch_bounds__(ORD_NT)
 k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__restrict__ bsum,
          const uint4 *__restrict__ arrival, unsigned long long arrival_cap, uint4 *__restrict__ ordered,
          unsigned long long cap, const EventParams ep, const Thresholds th, uint32_t W, uint32_t HW, uint32_t margin,
-         uint32_t tiles_x, uint32_t tiles, uint32_t S)
+         uint32_t tiles_x, uint32_t tiles, uint32_t S, const VoxelSink vox)
 {
     constexpr unsigned FULL = 0xFFFFFFFFu;
     __shared__ unsigned long long s_w[33];
@@ -241,7 +258,11 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
                 float fr = __fmul_rn(__fsub_rn(__fmaf_rn(kf, o_pc, o_ref), o_prev), o_rden);
                 fr = fminf(fmaxf(fr, 0.0f), 1.0f);
                 const unsigned long long o = first + e;
-                if (e < total_ev && o < cap) ordered[o] = make_uint4(o_xy, o_w1, __float_as_uint(__fmaf_rn(fr, ep.dt, t0)), ep.kf);
+                if (e < total_ev && o < cap) {
+                    const float t_off = __fmaf_rn(fr, ep.dt, t0);
+                    if (vox.store_events) ordered[o] = make_uint4(o_xy, o_w1, __float_as_uint(t_off), ep.kf);
+                    if (vox.v) voxel_add(vox, o_xy, o_w1, t_off);
+                }
             }
             first += total_ev;
         }
@@ -251,24 +272,53 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
 cudaError_t launch_expand(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
                           unsigned long long capacity, const unsigned long long *step_events,
                           unsigned long long *total_events, unsigned long long *overflow_steps, const EventParams &ep, const Thresholds &th, uint32_t W,
-                          uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, cudaStream_t st)
+                          uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, const VoxelSink &vox, cudaStream_t st)
 {
     const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
     k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, DIR_EV_SHIFT);
     k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events, sink.alloc, sink.arrival_cap, capacity, overflow_steps);
     k_expand<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, sink.arrival_cap, ordered, capacity, ep, th,
-                                    W, HW, margin, tiles_x, tiles, S);
+                                    W, HW, margin, tiles_x, tiles, S, vox);
     return cudaGetLastError();
 }
 
 cudaError_t launch_order(const EventSink &sink, uint32_t n, unsigned long long *bsum, uint4 *ordered,
                          unsigned long long capacity, const unsigned long long *step_events,
-                         unsigned long long *total_events, unsigned long long *overflow_steps, cudaStream_t st)
+                         unsigned long long *total_events, unsigned long long *overflow_steps, const VoxelSink &vox, cudaStream_t st)
 {
     const uint32_t nb = (n + ORD_PER_BLOCK - 1) / ORD_PER_BLOCK;
     k_dir_blocksum<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, 0);
     k_dir_scan_bsum<<<1, 1024, 0, st>>>(bsum, nb, step_events, total_events, sink.alloc, sink.arrival_cap, capacity, overflow_steps);
-    k_dir_copy<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, sink.arrival_cap, ordered, capacity);
+    k_dir_copy<<<nb, ORD_NT, 0, st>>>(sink.directory, n, bsum, sink.arrival, sink.arrival_cap, ordered, capacity, vox);
+    return cudaGetLastError();
+}
+
+// V (32.32 fixed point) -> float32; one block per (env, channel, bin) plane; normalize: divided by the plane's maximum
+__global__ void __launch_bounds__(256)
+k_voxel_finish(const unsigned long long *__restrict__ v, float *__restrict__ out, uint32_t cells, int normalize)
+{
+    __shared__ unsigned long long s_m[8];
+    const unsigned long long *pv = v + (size_t)blockIdx.x * cells;
+    float *po = out + (size_t)blockIdx.x * cells;
+    double inv = 1.0 / 4294967296.0;
+    if (normalize) {
+        unsigned long long m = 0;
+        for (uint32_t i = threadIdx.x; i < cells; i += blockDim.x) { const unsigned long long x = pv[i]; m = x > m ? x : m; }
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) { const unsigned long long o = __shfl_xor_sync(0xFFFFFFFFu, m, d); m = o > m ? o : m; }
+        if ((threadIdx.x & 31) == 0) s_m[threadIdx.x >> 5] = m;
+        __syncthreads();
+        m = 0;
+        for (int w = 0; w < 8; ++w) m = s_m[w] > m ? s_m[w] : m;
+        if (m) inv = 1.0 / (double)m;
+    }
+    for (uint32_t i = threadIdx.x; i < cells; i += blockDim.x) po[i] = (float)((double)pv[i] * inv);
+}
+
+cudaError_t launch_voxel_finish(const unsigned long long *v, float *out, uint32_t planes, uint32_t cells, int normalize,
+                                cudaStream_t st)
+{
+    k_voxel_finish<<<planes, 256, 0, st>>>(v, out, cells, normalize);
     return cudaGetLastError();
 }
 

@@ -7,6 +7,7 @@ import pytest
 import torch
 
 from paper_2607_08098_b200 import binding, scenes
+from oracle import evis_oracle as orc
 from tests import parity
 
 pytestmark = pytest.mark.gpu
@@ -841,3 +842,117 @@ def test_generator_is_device_independent():
             g = scenes.render_keyframe(sc, k, device="cuda")
             for key in c:
                 assert torch.equal(c[key], g[key].cpu()), (i, k, key)
+
+
+# ------------------------------------------------------------------------------------------------
+# voxel grid / accumulation image (reading R30)
+# ------------------------------------------------------------------------------------------------
+def _voxel_tolerance(bins, duration, counts):
+    """|V_gpu - V_oracle| per cell: every event's tau differs by at most (B-1)/D * (TOL_T + rounding of the binary32
+    window time, 2^-23 of D) and the weights are 1-Lipschitz in tau; the fixed-point sum adds 2^-32 per event."""
+    per_event = (bins - 1) * (parity.TOL_T / duration + 2.0 ** -22) + 1e-7
+    return (counts + 1.0) * per_event
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("bins,window,margin,tau_r", [(1, 1, 0, 0.0), (5, 1, 0, 0.0), (8, 3, 0, 0.0), (4, 2, 6, 0.0),
+                                                        (5, 2, 0, 2e-3)])
+def test_voxel_grid_matches_the_oracle(bins, window, margin, tau_r):
+    """evis_set_voxels / evis_read_voxels against oracle/evis_outputs.voxel_grid fed the ORACLE's events: windows of
+    `window` intervals, read when full (with and without normalisation); B = 1 must be exact counts.  Also with the
+    over-render margin (grid has the cropped shape) and in direct mode (refractory period: the copy kernel accumulates)."""
+    from oracle import evis_outputs as oout
+    spec = scenes.small(scenes.config(4), num_envs=3, height=97, width=131, num_keyframes=2 * window + 2)
+    sc = scenes.make_scene(spec)
+    E, H, W, S, T = spec.num_envs, spec.height, spec.width, spec.substeps, spec.keyframe_dt
+    Hc, Wc = H - 2 * margin, W - 2 * margin
+    ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, T, max_motion_px=spec.max_motion_px(),
+                      event_capacity=1 << 23)
+    ora = orc.Oracle(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, T, tau_r=tau_r, margin=margin)
+    if tau_r > 0:
+        ev.set_refractory(tau_r)
+    if margin:
+        ev.set_margin(margin)
+    ev.set_voxels(bins, window_steps=window, keep_events=True)
+    assert ev.voxel_shape() == (E, 2, bins, Hc, Wc)
+    acc = []
+    windows = 0
+    try:
+        for k in range(spec.num_keyframes):
+            kf = scenes.render_keyframe(sc, k, device="cuda")
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+            h = {key: v.cpu().numpy() for key, v in kf.items()}
+            oe = ora.step(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"])
+            if k == 0:
+                continue
+            acc.append(oe)
+            if len(acc) < window:
+                continue
+            j = np.concatenate([np.full(len(a), i, np.float64) for i, a in enumerate(acc)])
+            e = np.concatenate(acc)
+            acc = []
+            want = oout.voxel_grid(e["env"], e["x"], e["y"], e["p"], j * T + e["t_off"], E, Hc, Wc, bins, 0.0, window * T)
+            got, n = ev.read_voxels()
+            assert n == window and got.shape == want.shape
+            counts = want.sum(axis=2, keepdims=True)
+            assert counts.sum() == len(e) > 1000
+            if bins == 1:
+                assert np.array_equal(got.astype(np.float64), want)
+            else:
+                err = np.abs(got.astype(np.float64) - want)
+                assert np.all(err <= _voxel_tolerance(bins, window * T, counts)), float(err.max())
+                assert np.allclose(got.astype(np.float64).sum(axis=2, keepdims=True), counts, atol=1e-4)   # one unit per event
+            gn, _ = ev.read_voxels(normalize=True)
+            wn = oout.voxel_grid(e["env"], e["x"], e["y"], e["p"], j * T + e["t_off"], E, Hc, Wc, bins, 0.0, window * T,
+                                 normalize=True)
+            assert np.allclose(gn, wn, atol=2e-4)
+            ge = ev.read_events()                      # the stream is still there (keep_events)
+            assert len(ge) == len(oe)
+            windows += 1
+    finally:
+        ev.destroy()
+    assert windows >= 2
+
+
+@pytest.mark.gpu
+def test_voxels_only_mode_and_api_contract():
+    """keep_events = 0: the grid is the same, the event read calls report BAD_STATE, evis_get_info still counts the
+    events; restart begins a new window early; bins < 1 is INVALID_ARG; the margin cannot change under a grid."""
+    spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=4)
+    sc = scenes.make_scene(spec)
+    E, H, W = spec.num_envs, spec.height, spec.width
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(4)]
+
+    def run(keep, restart_after=None):
+        ev = binding.Evis(E, H, W, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                          max_motion_px=spec.max_motion_px(), event_capacity=1 << 22)
+        ev.set_voxels(3, window_steps=3, keep_events=keep)
+        grids, counts = [], []
+        for k, kf in enumerate(kfs):
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+            if k:
+                counts.append(ev.info().last_events)
+                grids.append(ev.read_voxels(restart=(restart_after == k)))
+        return ev, grids, counts
+
+    ev_a, ga, ca = run(True)
+    ev_b, gb, cb = run(False)
+    assert ca == cb and sum(ca) > 0
+    for (a, na), (b, nb) in zip(ga, gb):
+        assert na == nb and np.array_equal(a, b)
+    assert [n for _, n in ga] == [1, 2, 3]
+    assert abs(float(ga[-1][0].sum()) - sum(ca)) < 1e-2 * max(1, sum(ca)) * 1e-3 + 0.5      # one unit per event over the window
+    with pytest.raises(binding.EvisError) as ei:
+        ev_b.read_events()
+    assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    with pytest.raises(binding.EvisError) as ei:
+        ev_b.set_margin(2)
+    assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    with pytest.raises(binding.EvisError) as ei:
+        ev_b.set_voxels(0)
+    assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+    ev_a.destroy(); ev_b.destroy()
+    ev_c, gc, cc = run(True, restart_after=1)
+    assert [n for _, n in gc] == [1, 1, 2]                 # the window restarted after the first interval
+    assert abs(float(gc[1][0].sum()) - cc[1]) < 0.5
+    ev_c.destroy()
