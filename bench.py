@@ -33,21 +33,28 @@ ALGO_BYTES_PER_PIXEL = 52          # per pixel per keyframe interval, DESIGN.md 
 ALGO_BYTES_PER_EVENT = 16
 FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 ISSUE_PEAK = 148 * 4 * 32 * 1.965e9   # thread-instructions/s: SMs x schedulers x lanes x clocks.max.sm
-INSTR_PER_PXSS = 189.0                # issued thread-instruction slots per pixel-substep (ncu, profiles/r03_README.md)
+SURVEY_INSTR_BOUNDS = (60.0, 150.0)   # algorithmic estimate of issued instructions per pixel-substep
+# whole-step counters of a committed ncu capture (profiles/round2_a_range_cfg4.md says how it was made): the range is
+# RANGE_STEPS steps of RANGE_WORKLOAD.  Instruction counts do not depend on the schedule; the DRAM bytes of that capture
+# do (ncu serialises the streams), so they are reported as what they are.
+RANGE_CAPTURE = os.path.join("profiles", "round2_a_range_cfg4.csv")
+RANGE_WORKLOAD, RANGE_STEPS = "cfg4_256env_346x260_S16_rl", 5
 
 
-def ncu_traffic(workload: str, stage: str):
-    """DRAM bytes (read + write) per launch of the dominant kernel from the committed `ncu --set full`
-    capture (profiles/r03_dram_traffic.csv: workload,stage,bytes_per_launch), or None."""
+def range_capture(workload: str):
+    """{metric: value per step} from the committed whole-step ncu capture when it describes `workload`, else None."""
+    if workload != RANGE_WORKLOAD:
+        return None
+    out = {}
     try:
-        with open(os.path.join(ROOT, "profiles", "r03_dram_traffic.csv")) as f:
-            for line in f:
-                c = [x.strip() for x in line.split(",")]
-                if len(c) >= 3 and c[0] == workload and c[1] == stage:
-                    return float(c[2])
-    except OSError:
-        pass
-    return None
+        import csv
+        with open(os.path.join(ROOT, RANGE_CAPTURE)) as f:
+            for row in csv.reader(f):
+                if len(row) >= 13 and row[4] == "range":
+                    out[row[10]] = float(row[12].replace(",", "")) / RANGE_STEPS
+    except (OSError, ValueError):
+        return None
+    return out or None
 
 
 def parse_args():
@@ -287,30 +294,37 @@ def run_ours(args, spec) -> None:
     pxss_rank = E * H * W * S * K
     value = world * pxss_rank / (ms * 1e-3)
 
-    # ---- roofline of the dominant stage ---------------------------------------------------------------
+    # ---- roofline: the WHOLE step's algorithmic bytes over the WHOLE step's time (the path is one fused pass over the
+    #      keyframes: its stages overlap on several streams, so no stage is charged the bytes alone) --------------------
     peak, peak_src = hbm_peak()
     stage_ms = {k: v / K for k, v in prof["ms"].items()}
     dom = max(stage_ms, key=stage_ms.get)
     ev_per_step = events / world / K
     algo_bytes_step = ALGO_BYTES_PER_PIXEL * E * H * W + ALGO_BYTES_PER_EVENT * ev_per_step
-    # the dominant stage is charged the WHOLE step's algorithmic bytes (the other stages are its
-    # helpers: with a fully fused path there is only one kernel); its duration is its own.  Per launch:
-    # bytes and duration are both divided by the stage's launches per step.
-    dom_launches = max(1.0, prof["launches"][dom] / K)
-    achieved = algo_bytes_step / (stage_ms[dom] * 1e-3) / 1e9
+    step_s = ms / K * 1e-3
+    achieved = algo_bytes_step / step_s / 1e9
     pxss_step = E * H * W * S
+    cap_ = range_capture(spec.name)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(spec.name, dom), "peak_source": peak_src,
-                "algorithmic_bytes_per_step": algo_bytes_step,
-                "algorithmic_bytes_per_launch": algo_bytes_step / dom_launches,
-                "launch_ms": stage_ms[dom] / dom_launches, "launches_per_step": dom_launches,
-                "stage_ms_per_step": stage_ms, "stage_launches_per_step": {k: v / K for k, v in prof["launches"].items()},
-                "whole_step_frac": algo_bytes_step / (ms / K * 1e-3) / 1e9 / peak,
-                # the binding roof: issued thread-instruction slots, ~189 per pixel-substep
-                "issue_roof": {"bound": "alu", "unit": "thread-instr/s", "peak": ISSUE_PEAK,
-                               "instr_per_pixel_substep": INSTR_PER_PXSS,
-                               "achieved": INSTR_PER_PXSS * pxss_step / (ms / K * 1e-3),
-                               "frac": INSTR_PER_PXSS * pxss_step / (ms / K * 1e-3) / ISSUE_PEAK}}
+                "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": None, "traffic_note": "no DRAM-byte measurement of the concurrent schedule exists: ncu serialises the "
+                "streams (profiles/round2_README.md); the serialised capture's bytes are in `capture` below",
+                "algorithmic_bytes_per_step": algo_bytes_step, "basis": "whole step: algorithmic bytes / ms_per_step",
+                "dominant_stage_ms": stage_ms[dom], "dominant_stage_launches_per_step": max(1.0, prof["launches"][dom] / K),
+                "stage_ms_per_step": stage_ms, "stage_launches_per_step": {k: v / K for k, v in prof["launches"].items()}}
+    if cap_ and "smsp__inst_executed.sum" in cap_:
+        ipp = cap_["smsp__inst_executed.sum"] * 32.0 / pxss_step           # issue slots (thread-instructions) per pixel-substep
+        roofline["capture"] = {"file": RANGE_CAPTURE, "steps": RANGE_STEPS, "schedule": "serialised by ncu",
+                               "warp_instructions_per_step": cap_["smsp__inst_executed.sum"],
+                               "dram_bytes_per_step": cap_.get("dram__bytes_read.sum", 0.0) + cap_.get("dram__bytes_write.sum", 0.0),
+                               "l2_red_sectors_per_step": cap_.get("lts__t_sectors_op_red.sum")}
+        roofline["issue_roof"] = {"bound": "alu", "unit": "thread-instr/s", "peak": ISSUE_PEAK, "derived_from": RANGE_CAPTURE,
+                                  "instr_per_pixel_substep": ipp, "achieved": ipp * pxss_step / step_s,
+                                  "frac": ipp * pxss_step / step_s / ISSUE_PEAK,
+                                  "note": "utilisation of issue slots by the kernels' own instruction stream; against "
+                                          "SURVEY.md 8(d)'s algorithmic estimate of 60 / 150 instructions per pixel-substep "
+                                          "the throughput is the fractions below",
+                                  "frac_vs_survey_bounds": [n * pxss_step / step_s / ISSUE_PEAK for n in SURVEY_INSTR_BOUNDS]}
 
     out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": K, "warmup": Wm,
            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -319,7 +333,10 @@ def run_ours(args, spec) -> None:
            "x_realtime": spec.keyframe_dt / (ms / K * 1e-3),
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
 
-    # ---- e2e: HOST buffers through evis_step_host + evis_read_events -------------------------------------
+    # ---- e2e: HOST buffers through evis_step_host; every step uploads its keyframe from pinned memory and downloads
+    #      its result.  Two arms: the result is (a) the per-polarity accumulation image of the step (evis_set_voxels,
+    #      bins = 1, no 16-byte event leaves the GPU) -- `e2e` --, (b) the full ordered event stream -- `e2e_events`.
+    #      The upload of step k + 1 overlaps the kernels of step k (two staging sets) and the download of step k.
     if not args.no_e2e and not args.profile_range:
         Ke = max(1, min(args.e2e_steps, K))
         hk = []
@@ -327,35 +344,59 @@ def run_ours(args, spec) -> None:
             hk.append({a: b.cpu().pin_memory() for a, b in kfs[k].items()})
         del kfs
         torch.cuda.empty_cache()
-        ev = mk()
-        # two pinned host buffers: the events of step k go down (evis_read_events_begin / _end) while the keyframe of
-        # step k + 1 goes up; sized from the device-resident run (a step's events, with headroom)
-        hcap = int(min(cap, 2 * ev_per_step + (1 << 20)))
-        hbufs = [torch.empty((hcap, 16), dtype=torch.uint8).pin_memory() for _ in range(2)]
-        harrs = [hb.numpy().view(binding.EVENT_DTYPE).reshape(-1) for hb in hbufs]
-        for k in range(Wm + 1):
-            f = hk[k]
-            ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
-        barrier()
-        tt0 = time.perf_counter()
-        got = 0
-        for k in range(Wm + 1, Wm + 1 + Ke):
-            f = hk[k]
-            n_step = ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
-            n_copy = ev.read_events_begin(harrs[k & 1])        # ends the previous copy first
-            if n_copy != n_step:
-                raise SystemExit("bench.py: e2e host buffer too small for a step's events")
-            got += n_copy
-        ev.read_events_end()
-        barrier()
-        dt = time.perf_counter() - tt0
-        ev.destroy()
-        (dt,), _ = sharding.reduce_max_sum([dt], [], dev)
-        out["e2e"] = {"value": world * E * H * W * S * Ke / dt, "unit": METRIC, "steps": Ke,
-                      "h2d_bytes_per_step": int(E * H * W * 32), "d2h_bytes_per_step": int(16 * got / Ke),
-                      "ms_per_step": dt / Ke * 1e3,
-                      "api": "evis_step_host (pinned host keyframes) + evis_read_events_begin / _end (pinned host stream, "
-                             "overlapping the next upload)"}
+        h2d = int(E * H * W * 32)
+
+        def e2e_arm(voxels: bool):
+            ev = mk()
+            if voxels:
+                ev.set_voxels(1, window_steps=1, keep_events=False)
+                nel = int(np.prod(ev.voxel_shape()))
+                hbufs = [torch.empty(nel, dtype=torch.float32).pin_memory() for _ in range(2)]
+                harrs = [hb.numpy() for hb in hbufs]
+            else:
+                hcap = int(min(cap, 2 * ev_per_step + (1 << 20)))
+                hbufs = [torch.empty((hcap, 16), dtype=torch.uint8).pin_memory() for _ in range(2)]
+                harrs = [hb.numpy().view(binding.EVENT_DTYPE).reshape(-1) for hb in hbufs]
+            for k in range(Wm + 1):
+                f = hk[k]
+                ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
+            barrier()
+            tt0 = time.perf_counter()
+            got = 0
+            for k in range(Wm + 1, Wm + 1 + Ke):
+                f = hk[k]
+                if voxels:
+                    ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"], sync=False)
+                    ev.read_voxels_begin(harrs[k & 1])             # ends the previous copy first
+                    got += harrs[0].nbytes
+                else:
+                    n_step = ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
+                    n_copy = ev.read_events_begin(harrs[k & 1])        # ends the previous copy first
+                    if n_copy != n_step:
+                        raise SystemExit("bench.py: e2e host buffer too small for a step's events")
+                    got += 16 * n_copy
+            if voxels:
+                ev.read_voxels_end()
+                total = float(harrs[(Wm + Ke) & 1].sum())             # the last image really arrived: one unit per event
+                if abs(total - ev.info().last_events) > 0.5:
+                    raise SystemExit("bench.py: the downloaded accumulation image does not hold the step's events")
+            else:
+                ev.read_events_end()
+            barrier()
+            dt = time.perf_counter() - tt0
+            ev.destroy()
+            (dt,), _ = sharding.reduce_max_sum([dt], [], dev)
+            return {"value": world * E * H * W * S * Ke / dt, "unit": METRIC, "steps": Ke,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(got / Ke), "ms_per_step": dt / Ke * 1e3,
+                    "x_realtime": spec.keyframe_dt / (dt / Ke)}
+
+        out["e2e"] = dict(e2e_arm(True), result="per-polarity accumulation image of the step [E,2,1,H,W] float32 "
+                          "(evis_set_voxels bins=1, keep_events=0)",
+                          api="evis_step_host (pinned host keyframes, upload overlapping the previous step) + "
+                              "evis_read_voxels_begin / _end (pinned host image, overlapping the next upload)")
+        out["e2e_events"] = dict(e2e_arm(False), result="the full ordered event stream, 16 B per event",
+                                 api="evis_step_host (pinned host keyframes) + evis_read_events_begin / _end (pinned host "
+                                     "stream, overlapping the next upload)")
 
     if rank == 0 and not args.no_cpu and not args.profile_range:
         out["cpu_baseline"] = cpu_baseline(scenes.small(spec, seed=spec.seed - 1000 * rank), args.cpu_seconds)

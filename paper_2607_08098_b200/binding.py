@@ -258,16 +258,17 @@ class Evis:
         st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
         _check(self._lib.evis_wait_events(self._ctx, C.c_void_p(st)), "evis_wait_events")
 
-    def step_host(self, rad, mv_bwd, depth, mv_fwd=None, allow=()) -> int:
-        """evis_step_host: HOST buffers (numpy or CPU tensors); copies, runs and synchronises."""
+    def step_host(self, rad, mv_bwd, depth, mv_fwd=None, allow=(), sync: bool = True) -> Optional[int]:
+        """evis_step_host: HOST buffers (numpy or CPU tensors).  sync: wait for the step and return its event count;
+        else return once the upload is done (the step keeps running and overlaps the next upload)."""
         E, H, W = self.E, self.H, self.W
         n = C.c_uint64(0)
         rc = self._lib.evis_step_host(self._ctx, _host_ptr(rad, (E, H, W, 3), "rad"),
                                       _host_ptr(mv_bwd, (E, H, W, 2), "mv_bwd"),
                                       _host_ptr(mv_fwd, (E, H, W, 2), "mv_fwd"),
-                                      _host_ptr(depth, (E, H, W), "depth"), C.byref(n))
+                                      _host_ptr(depth, (E, H, W), "depth"), C.byref(n) if sync else None)
         _check(rc, "evis_step_host", allow)
-        return int(n.value)
+        return int(n.value) if sync else None
 
     # -- evis_read_events --------------------------------------------------------------------------
     def read_events(self, max_events: Optional[int] = None, allow=()) -> np.ndarray:

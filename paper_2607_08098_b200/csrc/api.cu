@@ -85,7 +85,12 @@ struct evis_ctx {
     size_t vox_cells;                 // E * 2 * bins * H' * W'
 
     // host-buffer entry point staging
-    float *st_rad, *st_mv, *st_fwd, *st_depth;
+    // two staging sets: the keyframe of step k + 1 goes up (up_stream) while step k computes (own_stream)
+    float *st_rad[2], *st_mv[2], *st_fwd[2], *st_depth[2];
+    cudaStream_t up_stream;
+    cudaEvent_t ev_up[2], ev_used[2];     // set uploaded / the step that read the set has been enqueued and has run
+    bool set_used[2];
+    uint64_t host_steps;
 
     uint64_t steps, launches, device_bytes;
     uint32_t kf_next;                 // index the next closed interval gets (evis_set_interval_index)
@@ -207,7 +212,12 @@ void free_all(evis_ctx *ctx)
     cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
     cudaFree(ctx->vox_v); cudaFree(ctx->vox_out);
-    cudaFree(ctx->st_rad); cudaFree(ctx->st_mv); cudaFree(ctx->st_fwd); cudaFree(ctx->st_depth);
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(ctx->st_rad[k]); cudaFree(ctx->st_mv[k]); cudaFree(ctx->st_fwd[k]); cudaFree(ctx->st_depth[k]);
+        if (ctx->ev_up[k]) cudaEventDestroy(ctx->ev_up[k]);
+        if (ctx->ev_used[k]) cudaEventDestroy(ctx->ev_used[k]);
+    }
+    if (ctx->up_stream) cudaStreamDestroy(ctx->up_stream);
     if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
     prof_drain(ctx);
     for (cudaEvent_t e : ctx->prof_free) cudaEventDestroy(e);
@@ -842,21 +852,40 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     const size_t P = (size_t)ctx->g.E * ctx->g.HW;
-    if (!ctx->st_rad) {
-        CU(dalloc(ctx, &ctx->st_rad, 3 * P));
-        CU(dalloc(ctx, &ctx->st_mv, 2 * P));
-        CU(dalloc(ctx, &ctx->st_depth, P));
+    if (!ctx->up_stream) {
+        CU(cudaStreamCreateWithFlags(&ctx->up_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < 2; ++k) {
+            CU(cudaEventCreateWithFlags(&ctx->ev_up[k], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&ctx->ev_used[k], cudaEventDisableTiming));
+            CU(dalloc(ctx, &ctx->st_rad[k], 3 * P));
+            CU(dalloc(ctx, &ctx->st_mv[k], 2 * P));
+            CU(dalloc(ctx, &ctx->st_depth[k], P));
+        }
     }
-    if (mv_fwd && !ctx->st_fwd) CU(dalloc(ctx, &ctx->st_fwd, 2 * P));
-    cudaStream_t st = ctx->own_stream;
-    CU(cudaMemcpyAsync(ctx->st_rad, rad, 3 * P * sizeof(float), cudaMemcpyHostToDevice, st));
-    CU(cudaMemcpyAsync(ctx->st_mv, mv_bwd, 2 * P * sizeof(float), cudaMemcpyHostToDevice, st));
-    if (mv_fwd) CU(cudaMemcpyAsync(ctx->st_fwd, mv_fwd, 2 * P * sizeof(float), cudaMemcpyHostToDevice, st));
-    CU(cudaMemcpyAsync(ctx->st_depth, depth, P * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (mv_fwd && !ctx->st_fwd[0])
+        for (int k = 0; k < 2; ++k) CU(dalloc(ctx, &ctx->st_fwd[k], 2 * P));
+    // set k & 1: free once the step that read it two calls ago has run; its upload overlaps the previous step
+    const int set = (int)(ctx->host_steps & 1);
+    cudaStream_t up = ctx->up_stream, st = ctx->own_stream;
+    if (ctx->set_used[set]) CU(cudaStreamWaitEvent(up, ctx->ev_used[set], 0));
+    CU(cudaMemcpyAsync(ctx->st_rad[set], rad, 3 * P * sizeof(float), cudaMemcpyHostToDevice, up));
+    CU(cudaMemcpyAsync(ctx->st_mv[set], mv_bwd, 2 * P * sizeof(float), cudaMemcpyHostToDevice, up));
+    if (mv_fwd) CU(cudaMemcpyAsync(ctx->st_fwd[set], mv_fwd, 2 * P * sizeof(float), cudaMemcpyHostToDevice, up));
+    CU(cudaMemcpyAsync(ctx->st_depth[set], depth, P * sizeof(float), cudaMemcpyHostToDevice, up));
+    CU(cudaEventRecord(ctx->ev_up[set], up));
+    CU(cudaStreamWaitEvent(st, ctx->ev_up[set], 0));
     uint64_t n = 0;
-    const int rc = evis_step(ctx, ctx->st_rad, ctx->st_mv, mv_fwd ? ctx->st_fwd : nullptr, ctx->st_depth,
-                             (void *)st, &n);
+    const int rc = evis_step(ctx, ctx->st_rad[set], ctx->st_mv[set], mv_fwd ? ctx->st_fwd[set] : nullptr, ctx->st_depth[set],
+                             (void *)st, n_events ? &n : nullptr);
+    cudaEventRecord(ctx->ev_used[set], st);
+    ctx->set_used[set] = true;
+    ctx->host_steps += 1;
     if (n_events) *n_events = n;
+    else if (rc == EVIS_OK) {
+        // asynchronous form: the host buffers must stay untouched until their upload has run; waiting for the
+        // UPLOAD (not the step) keeps that promise inside the call and still lets the step overlap the next upload
+        CU(cudaEventSynchronize(ctx->ev_up[set]));
+    }
     return rc;
 }
 
