@@ -67,7 +67,7 @@ def parse_args():
     ap.add_argument("--envs", type=int, default=0, help="override the number of envs (0 = the config's)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--e2e-steps", type=int, default=6)
+    ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--profile-range", action="store_true",
                     help="bracket the timed region with cudaProfilerStart / Stop (for `ncu --replay-mode app-range`: "
@@ -377,13 +377,14 @@ def run_ours(args, spec) -> None:
                     got += 16 * n_copy
             if voxels:
                 ev.read_voxels_end()
-                total = float(harrs[(Wm + Ke) & 1].sum())             # the last image really arrived: one unit per event
-                if abs(total - ev.info().last_events) > 0.5:
-                    raise SystemExit("bench.py: the downloaded accumulation image does not hold the step's events")
             else:
                 ev.read_events_end()
             barrier()
             dt = time.perf_counter() - tt0
+            if voxels:                                                # (outside the timed region) the last image really arrived:
+                total = float(harrs[(Wm + Ke) & 1].sum(dtype=np.float64))             # one unit per event
+                if abs(total - ev.info().last_events) > 0.5:
+                    raise SystemExit("bench.py: the downloaded accumulation image does not hold the step's events")
             ev.destroy()
             (dt,), _ = sharding.reduce_max_sum([dt], [], dev)
             return {"value": world * E * H * W * S * Ke / dt, "unit": METRIC, "steps": Ke,

@@ -141,9 +141,10 @@ int evis_wait_events(evis_ctx *ctx, void *cuda_stream);
 
 /* Same step with HOST buffers (pageable or pinned): copies them to device staging owned by the context and runs the
  * step on the context's own streams.  With n_events the call waits for the step and stores its event count.  With
- * n_events = NULL it returns as soon as the UPLOAD has finished (the host buffers are free again) and leaves the step
- * running: there are two staging sets, so the upload of the next keyframe overlaps this step's kernels; every call that
- * returns results waits for the step as usual. */
+ * n_events = NULL it only enqueues: the host buffers must then stay untouched until the NEXT evis_step_host call (or
+ * any call that synchronises, e.g. evis_get_info) has returned.  There are two staging sets, so the upload of the next
+ * keyframe starts the moment this one's is over and overlaps this step's kernels; every call that returns results
+ * waits for the step as usual. */
 int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd,
                    const float *depth, uint64_t *n_events);
 

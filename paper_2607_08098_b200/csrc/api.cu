@@ -867,6 +867,8 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
     // set k & 1: free once the step that read it two calls ago has run; its upload overlaps the previous step
     const int set = (int)(ctx->host_steps & 1);
     cudaStream_t up = ctx->up_stream, st = ctx->own_stream;
+    // the previous call's host buffers are released when this call returns: its upload has to be over
+    if (ctx->set_used[set ^ 1]) CU(cudaEventSynchronize(ctx->ev_up[set ^ 1]));
     if (ctx->set_used[set]) CU(cudaStreamWaitEvent(up, ctx->ev_used[set], 0));
     CU(cudaMemcpyAsync(ctx->st_rad[set], rad, 3 * P * sizeof(float), cudaMemcpyHostToDevice, up));
     CU(cudaMemcpyAsync(ctx->st_mv[set], mv_bwd, 2 * P * sizeof(float), cudaMemcpyHostToDevice, up));
@@ -881,11 +883,6 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
     ctx->set_used[set] = true;
     ctx->host_steps += 1;
     if (n_events) *n_events = n;
-    else if (rc == EVIS_OK) {
-        // asynchronous form: the host buffers must stay untouched until their upload has run; waiting for the
-        // UPLOAD (not the step) keeps that promise inside the call and still lets the step overlap the next upload
-        CU(cudaEventSynchronize(ctx->ev_up[set]));
-    }
     return rc;
 }
 
