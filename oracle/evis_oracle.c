@@ -23,7 +23,8 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 zero motion identity, P2 substep S reproduces
  * keyframe B, P3 integer translation, P4 8x8 gather-form brute force, P5 analytic two-rectangle
  * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8), P12 refractory period, P13 margin, P14 colour, P15 noise events,
- * P16 composite mode 1 (every case of the rule by hand; linear time ramp along a translation).  UNPINNED by paper or
+ * P16 composite mode 1 (every case of the rule by hand; linear time ramp along a translation), P19 defocus (library
+ * Gaussian filter, blur-before-log, holes held unblurred).  UNPINNED by paper or
  * mathematics (fixed by DESIGN.md readings only): log base R1, epsilon R2, initial reference
  * level R6, nearest-pixel depth lookup R16, hole handling R20, the composite choice R19, and among the
  * non-idealities the choices of R26 (L_ref follows suppressed crossings) and R29 (Ibar's normalisation, stamps,
@@ -337,6 +338,66 @@ int64_t evo_event_frame(int H, int W, int env, int kf, int i, int S, float T,
     return made;
 }
 
+/* ---- Defocus [R31] ------------------------------------------------------------------------------
+ * "Prior to the event generation, the linear intensity is convolved with a separable Gaussian kernel."
+ * The frame the event model sees at every substep is the warped frame in LINEAR intensity, blurred, then logged:
+ *   I_X[p]  = (float) max(0, 0.2126 R + 0.7152 G + 0.0722 B)        (binary64 sums as in Eq. 3, rounded once; or the
+ *                                                                     chosen channel for colour events)
+ *   Ihat_i  = the composite of Sec. 3.3 applied to I_A, I_B (values are copied, so the winners are those of the
+ *             log path); a pixel reached by neither keyframe holds its previous UNBLURRED value Ihat_{i-1} [R20]
+ *   Iblur_i = G_sigma * Ihat_i, separable: rows first, then columns; taps k = -R..R, R = ceil(3 sigma),
+ *             w_k = exp(-k^2 / (2 sigma^2)) / sum (binary64, rounded to binary32); the border replicates the edge
+ *             pixel; every pass accumulates in binary32, acc = fmaf(w_k, v_k, acc) for k = -R..R in that order
+ *   L_i     = (float) log((double) Iblur_i + eps)                    -> Eq. 4
+ * With a margin the blur runs on the whole over-rendered frame and the crop follows.                              */
+void evo_linear_luminance(const float *rad /* [n][3] */, int64_t n, int channel /* -1: Rec.709 */, float *I /* [n] */)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        double v;
+        if (channel >= 0) v = (double)rad[3 * i + channel];
+        else {
+            double r = (double)rad[3 * i + 0], g = (double)rad[3 * i + 1], b = (double)rad[3 * i + 2];
+            v = (0.2126 * r + 0.7152 * g) + 0.0722 * b;
+        }
+        if (!(v > 0.0)) v = 0.0;
+        I[i] = (float)v;
+    }
+}
+
+/* taps of the Gaussian: returns R = ceil(3 sigma) (0 for sigma <= 0) and fills w[0 .. 2R] for k = -R .. R */
+int evo_gauss_taps(float sigma, float *w, int max_taps)
+{
+    if (!(sigma > 0.0f)) { w[0] = 1.0f; return 0; }
+    int R = (int)ceil(3.0 * (double)sigma);
+    if (2 * R + 1 > max_taps) return -1;
+    double sum = 0.0;
+    for (int k = -R; k <= R; ++k) sum += exp(-(double)(k * k) / (2.0 * (double)sigma * (double)sigma));
+    for (int k = -R; k <= R; ++k) w[k + R] = (float)(exp(-(double)(k * k) / (2.0 * (double)sigma * (double)sigma)) / sum);
+    return R;
+}
+
+void evo_blur(int H, int W, int R, const float *w, const float *src, float *tmp /* [H*W] scratch */, float *dst)
+{
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            float acc = 0.0f;
+            for (int k = -R; k <= R; ++k) {
+                int xx = x + k; if (xx < 0) xx = 0; if (xx > W - 1) xx = W - 1;
+                acc = fmaf(w[k + R], src[y * W + xx], acc);
+            }
+            tmp[y * W + x] = acc;
+        }
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            float acc = 0.0f;
+            for (int k = -R; k <= R; ++k) {
+                int yy = y + k; if (yy < 0) yy = 0; if (yy > H - 1) yy = H - 1;
+                acc = fmaf(w[k + R], tmp[yy * W + x], acc);
+            }
+            dst[y * W + x] = acc;
+        }
+}
+
 /* ---- one keyframe interval of one env: A -> B, substeps i = 1..S ------------------------------
  * i < S are the paper's K-1 intermediates (f = i/K); i = S is keyframe B itself [R10].
  * fwdA: displacement of A's pixels towards B: -m_A or the explicit forward field.
@@ -353,7 +414,11 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, int margin,
                      uint64_t *zA, uint64_t *zB, float *Lhat,              /* scratch [H*W] each */
                      evo_event *ev, int64_t cap, int64_t n_have,
                      uint32_t *dbg_winA, uint32_t *dbg_winB, uint8_t *dbg_dir, uint32_t *dbg_idx,
-                     float *dbg_Lhat, float *dbg_dL, int64_t *holes)
+                     float *dbg_Lhat, float *dbg_dL, int64_t *holes,
+                     /* defocus [R31]: blur_R < 0 = off (everything below unused).  IA / IB: linear intensity of the keyframes,
+                      * Iprev: carried unblurred warped frame, eps: the log epsilon, scratch [H*W] each */
+                     int blur_R, const float *blur_w, const float *IA, const float *IB, float *Iprev, float eps,
+                     float *blur_tmp, float *blur_out)
 {
     const int64_t P = (int64_t)H * W;
     int64_t made = 0;
@@ -363,7 +428,15 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, int margin,
         evo_splat(H, W, i, S, 1, mB, ZB, ZA, zB);
         uint8_t *dd = dbg_dir ? dbg_dir + (int64_t)(i - 1) * P : 0;
         uint32_t *di = dbg_idx ? dbg_idx + (int64_t)(i - 1) * P : 0;
-        evo_composite(H, W, i, S, mode, zA, zB, LA, LB, Lprev, Lhat, dd, di);
+        if (blur_R < 0) {
+            evo_composite(H, W, i, S, mode, zA, zB, LA, LB, Lprev, Lhat, dd, di);
+        } else {
+            /* defocus: composite the LINEAR frame (holes hold the previous unblurred value), blur it, take the log */
+            evo_composite(H, W, i, S, mode, zA, zB, IA, IB, Iprev, blur_out, dd, di);
+            for (int64_t q = 0; q < P; ++q) Iprev[q] = blur_out[q];
+            evo_blur(H, W, blur_R, blur_w, Iprev, blur_tmp, blur_out);
+            for (int64_t q = 0; q < P; ++q) Lhat[q] = (float)log((double)blur_out[q] + (double)eps);
+        }
         for (int64_t q = 0; q < P; ++q) {
             if (dbg_winA) dbg_winA[(int64_t)(i - 1) * P + q] = zA[q] == EVO_EMPTY ? EVO_NONE : (uint32_t)zA[q];
             if (dbg_winB) dbg_winB[(int64_t)(i - 1) * P + q] = zB[q] == EVO_EMPTY ? EVO_NONE : (uint32_t)zB[q];

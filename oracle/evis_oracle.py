@@ -46,8 +46,15 @@ def lib():
         L.evo_event_frame.restype = C.c_int64
         L.evo_interval.argtypes = ([C.c_int] * 7 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [C.c_void_p] + [fp] * 8 + [u64p, u64p, fp]
                                    + [C.c_void_p, C.c_int64, C.c_int64]
-                                   + [u32p, u32p, u8p, u32p, fp, fp, C.POINTER(C.c_int64)])
+                                   + [u32p, u32p, u8p, u32p, fp, fp, C.POINTER(C.c_int64)]
+                                   + [C.c_int, fp, fp, fp, fp, C.c_float, fp, fp])
         L.evo_interval.restype = C.c_int64
+        L.evo_linear_luminance.argtypes = [fp, C.c_int64, C.c_int, fp]
+        L.evo_linear_luminance.restype = None
+        L.evo_gauss_taps.argtypes = [C.c_float, fp, C.c_int]
+        L.evo_gauss_taps.restype = C.c_int
+        L.evo_blur.argtypes = [C.c_int, C.c_int, C.c_int, fp, fp, fp, fp]
+        L.evo_blur.restype = None
         L.evo_exp32.argtypes = [C.c_float]
         L.evo_exp32.restype = C.c_float
         L.evo_noise_key.argtypes = [C.c_uint64, C.c_int, C.c_int, C.c_int64]
@@ -78,6 +85,32 @@ def log_luminance(rad: np.ndarray, eps: float, channel: Optional[int] = None) ->
         assert channel in (0, 1, 2)
         lib().evo_log_channel(_f(rad), out.size, float(eps), int(channel), _f(out))
     return out
+
+
+def linear_luminance(rad: np.ndarray, channel: Optional[int] = None) -> np.ndarray:
+    """Linear intensity of Eq. 3 (or of one channel), clamped at 0, float32 [R31].  rad [...,3] -> I [...]."""
+    rad = np.ascontiguousarray(rad, dtype=np.float32)
+    out = np.empty(rad.shape[:-1], dtype=np.float32)
+    lib().evo_linear_luminance(_f(rad), out.size, -1 if channel is None else int(channel), _f(out))
+    return out
+
+
+def gauss_taps(sigma: float) -> np.ndarray:
+    """The 2R+1 taps of the defocus kernel, R = ceil(3 sigma) [R31]."""
+    w = np.zeros(257, np.float32)
+    R = lib().evo_gauss_taps(float(sigma), _f(w), w.size)
+    assert R >= 0, "sigma too large"
+    return w[:2 * R + 1].copy()
+
+
+def blur(frame: np.ndarray, taps: np.ndarray) -> np.ndarray:
+    """Separable convolution of one [H,W] float32 frame with `taps` (rows, then columns; replicated border) [R31]."""
+    frame = np.ascontiguousarray(frame, np.float32)
+    H, W = frame.shape
+    taps = np.ascontiguousarray(taps, np.float32)
+    tmp, dst = np.empty((H, W), np.float32), np.empty((H, W), np.float32)
+    lib().evo_blur(H, W, (taps.size - 1) // 2, _f(taps), _f(frame), _f(tmp), _f(dst))
+    return dst
 
 
 def splat(i: int, S: int, src_is_B: bool, disp: np.ndarray, Zsrc: np.ndarray, Zoth: np.ndarray
@@ -162,7 +195,8 @@ class Oracle:
     def __init__(self, num_envs: int, height: int, width: int, substeps: int, c_pos: float, c_neg: float,
                  log_eps: float, keyframe_dt: float, composite_mode: int = 0, debug: bool = False,
                  theta_on: Optional[np.ndarray] = None, theta_off: Optional[np.ndarray] = None,
-                 tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None, noise: Optional[dict] = None):
+                 tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None, noise: Optional[dict] = None,
+                 defocus_sigma: Optional[float] = None):
         self.E, self.H, self.W, self.S = num_envs, height, width, substeps
         self.c_pos, self.c_neg, self.eps, self.T = c_pos, c_neg, log_eps, keyframe_dt
         self.mode = composite_mode
@@ -179,6 +213,10 @@ class Oracle:
         self.channel = channel                     # colour events: None = luminance, 0/1/2 = R/G/B
         self.margin = int(margin)
         assert 0 <= 2 * self.margin < min(height, width)
+        # defocus [R31]: None = off; a sigma (>= 0) = the warped LINEAR frame of every substep is blurred
+        self.taps = None if defocus_sigma is None else gauss_taps(defocus_sigma)
+        assert self.taps is None or composite_mode == 0, "defocus is defined for the B-primary composite"
+        self.Iprev = None
         self.tau_r = float(tau_r)
         self.t_last = np.full((num_envs, height, width), -np.inf, np.float32)
         self.calls = 0
@@ -201,7 +239,17 @@ class Oracle:
         fwd = -mB if mv_fwd is None else np.ascontiguousarray(mv_fwd, np.float32).reshape(E, H, W, 2)
         fwd = np.ascontiguousarray(fwd)
         cur = dict(L=LB, m=mB, Z=ZB, fwd=fwd)
+        if self.taps is not None:
+            cur["I"] = linear_luminance(rad, self.channel)
         if self.calls == 0:
+            if self.taps is not None:                  # the event model's first frame is the blurred keyframe too
+                self.Iprev = cur["I"].copy()
+                LB0 = np.stack([np.log(blur(cur["I"][e], self.taps).astype(np.float64) + np.float64(np.float32(self.eps)))
+                                for e in range(E)]).astype(np.float32)
+                self.Lref, self.Lprev = LB0.copy(), LB0.copy()
+                self.prev = cur
+                self.calls = 1
+                return np.zeros(0, dtype=EVENT_DTYPE)
             self.Lref = LB.copy()
             self.Lprev = LB.copy()
             self.prev = cur
@@ -223,6 +271,8 @@ class Oracle:
             ev = np.zeros(cap, dtype=EVENT_DTYPE)
             Lref, Lprev = self.Lref.copy(), self.Lprev.copy()
             t_last = self.t_last.copy()
+            Iprev = None if self.taps is None else self.Iprev.copy()
+            btmp, bout = np.empty(P, np.float32), np.empty(P, np.float32)
             holes.value = 0
             n = 0
             for e in range(E):
@@ -238,11 +288,16 @@ class Oracle:
                     ev.ctypes.data, cap, n,
                     _p(d["winA"][e], C.c_uint32) if d else None, _p(d["winB"][e], C.c_uint32) if d else None,
                     _p(d["dir"][e], C.c_uint8) if d else None, _p(d["idx"][e], C.c_uint32) if d else None,
-                    _f(d["Lhat"][e]) if d else None, _f(d["dL"][e]) if d else None, C.byref(holes))
+                    _f(d["Lhat"][e]) if d else None, _f(d["dL"][e]) if d else None, C.byref(holes),
+                    -1 if self.taps is None else (self.taps.size - 1) // 2,
+                    _f(self.taps) if self.taps is not None else None,
+                    _f(A["I"][e]) if self.taps is not None else None, _f(cur["I"][e]) if self.taps is not None else None,
+                    _f(Iprev[e]) if self.taps is not None else None, float(self.eps), _f(btmp), _f(bout))
             if n <= cap:
                 break
             cap = int(n)
         self.Lref, self.Lprev, self.t_last = Lref, Lprev, t_last
+        self.Iprev = Iprev
         self.holes = holes.value
         self.prev = cur
         self.calls += 1

@@ -775,3 +775,109 @@ def test_p15e_hot_pixels_and_signal_untouched():
     b, lrb = orc.event_frames(frames, L0, 0.2, 0.3, 1.0, noise=dict(seed=3, r_leak=2.0, r_shot=2.0, r_hot=9.0, eps=1e-3, hot=hot))
     sig = b[b["k"] < 1000]
     assert np.array_equal(lra, lrb) and len(b) > len(a) and np.array_equal(sig, a)
+
+
+# ------------------------------------------------------------------------------------------------
+# P19: defocus (reading R31): separable Gaussian on the warped LINEAR frame, then the log
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sigma", [0.1, 0.3, 0.5, 1.0, 2.3])
+def test_p19_defocus_kernel_is_the_library_gaussian_filter(sigma):
+    """Taps: R = ceil(3 sigma), symmetric, sum 1; the two-pass blur equals scipy.ndimage.gaussian_filter (truncated at
+    the same radius, replicated border) and the 2-D correlation with the outer product of the taps (separability)."""
+    from scipy import ndimage
+    w = orc.gauss_taps(sigma)
+    R = (w.size - 1) // 2
+    assert R == math.ceil(3 * sigma) and np.array_equal(w, w[::-1]) and abs(float(w.astype(np.float64).sum()) - 1) < 1e-6
+    assert abs(w[R + 1] / w[R] - math.exp(-1 / (2 * sigma * sigma))) < 1e-6 * max(1.0, w[R + 1] / w[R])
+    f = _rng(19).uniform(0.0, 7.0, (23, 31)).astype(np.float32)
+    got = orc.blur(f, w).astype(np.float64)
+    lib_ = ndimage.gaussian_filter(f.astype(np.float64), sigma, mode="nearest", radius=R)
+    assert np.abs(got - lib_).max() < 3e-6
+    two_d = ndimage.correlate(f.astype(np.float64), np.outer(w, w).astype(np.float64), mode="nearest")
+    assert np.abs(got - two_d).max() < 3e-6
+    const = np.full((9, 11), 3.25, np.float32)
+    assert np.abs(orc.blur(const, w) - 3.25).max() < 1e-6 * 3.25 * (2 * R + 2)
+
+
+def test_p19b_defocus_blurs_the_linear_frame_with_holes_held_unblurred():
+    """The frame the event model sees = log(blur(warped LINEAR frame) + eps), a hole holding its previous UNBLURRED
+    value: rebuilt here from the plain run's winners (pinned by P3 / P4 / P5), numpy's luminance, scipy's filter and
+    np.log.  The alternatives (blur of the log frame; holes holding the blurred value) miss by far more than the
+    tolerance on this scene, so the pin tells them apart."""
+    from scipy import ndimage
+    H, W, S, dx, dy, sigma, eps = 20, 26, 4, 2, -1, 0.8, 1e-3
+    r = _rng(23)
+    big = r.uniform(-3, 3, size=(H + 64, W + 64)).astype(np.float32)
+    ys, xs = np.mgrid[0:H, 0:W]
+    tex = lambda px, py: big[ys - py + 32, xs - px + 32]
+    mv = np.empty((1, H, W, 2), np.float32)
+    mv[..., 0], mv[..., 1] = -S * dx, -S * dy
+    depth = np.full((1, H, W), 3.0, np.float32)
+    rads = [_rad_from_L(tex(0, 0))[None], _rad_from_L(tex(S * dx, S * dy))[None], _rad_from_L(tex(2 * S * dx, 2 * S * dy))[None]]
+    plain = orc.Oracle(1, H, W, S, 0.2, 0.2, eps, 1 / 60, debug=True)
+    blur_ = orc.Oracle(1, H, W, S, 0.2, 0.2, eps, 1 / 60, debug=True, defocus_sigma=sigma)
+    lin = lambda rad: ((0.2126 * rad[..., 0].astype(np.float64) + 0.7152 * rad[..., 1]) + 0.0722 * rad[..., 2]).clip(0).astype(np.float32)
+    w = orc.gauss_taps(sigma)
+    R = (w.size - 1) // 2
+    filt = lambda f: ndimage.gaussian_filter(f.astype(np.float64), sigma, mode="nearest", radius=R)
+    e32 = np.float64(np.float32(eps))
+    held = lin(rads[0])[0]                               # the unblurred warped frame carried through the holes
+    held_alt = filt(held)                                # alternative: holes hold the BLURRED value
+    n_holes, worst_alt1, worst_alt2 = 0, 0.0, 0.0
+    for k, rad in enumerate(rads):
+        plain.step(rad, mv, depth)
+        ev = blur_.step(rad, mv, depth)
+        if k == 0:
+            L0 = np.log(filt(lin(rad)[0]) + e32)
+            assert np.abs(blur_.Lref[0] - L0).max() < 3e-6 and len(ev) == 0
+            continue
+        IA, IB = lin(rads[k - 1])[0].ravel(), lin(rad)[0].ravel()
+        for i in range(S):
+            d, idx = plain.dbg["dir"][0, i], plain.dbg["idx"][0, i].astype(np.int64)
+            assert np.array_equal(d, blur_.dbg["dir"][0, i]) and np.array_equal(idx, blur_.dbg["idx"][0, i].astype(np.int64))
+            safe = np.where(d == 3, 0, idx)
+            frame = np.where(d == 0, IB[safe], np.where(d == 1, IA[safe], held))
+            frame_alt = np.where(d == 0, IB[safe], np.where(d == 1, IA[safe], held_alt))
+            n_holes += int((d == 3).sum())
+            want = np.log(filt(frame) + e32)
+            got = blur_.dbg["Lhat"][0, i].astype(np.float64)
+            assert np.abs(got - want).max() < 5e-6, (k, i, float(np.abs(got - want).max()))
+            worst_alt1 = max(worst_alt1, float(np.abs(got - filt(np.log(frame.astype(np.float64) + e32))).max()))
+            worst_alt2 = max(worst_alt2, float(np.abs(got - np.log(filt(frame_alt) + e32)).max()))
+            held, held_alt = frame, filt(frame_alt)
+    assert n_holes > 0 and worst_alt1 > 1e-2 and worst_alt2 > 1e-3
+
+
+def test_p19c_zero_sigma_is_the_plain_run():
+    """sigma = 0 (one tap of weight 1): the frames are the plain frames up to the rounding of the linear intensity to
+    binary32 before the log, and the events are the plain events."""
+    spec = scenes.small(scenes.config(1), height=40, width=56, num_keyframes=3)
+    sc = scenes.make_scene(spec)
+    a = orc.Oracle(1, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, debug=True)
+    b = orc.Oracle(1, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, debug=True,
+                   defocus_sigma=0.0)
+    na = nb = 0
+    for k in range(3):
+        kf = {key: v.numpy() for key, v in scenes.render_keyframe(sc, k).items()}
+        ea = a.step(kf["rad"], kf["mv_bwd"], kf["depth"], kf["mv_fwd"])
+        eb = b.step(kf["rad"], kf["mv_bwd"], kf["depth"], kf["mv_fwd"])
+        na, nb = na + len(ea), nb + len(eb)
+        if k:
+            assert np.abs(a.dbg["Lhat"].astype(np.float64) - b.dbg["Lhat"]).max() < 1e-6
+    assert na > 100 and abs(na - nb) <= max(2, na // 500)          # rounding of I before the log moves a few ties
+
+
+def test_p19d_defocus_softens_edges_and_a_static_scene_stays_silent():
+    """A static scene fires nothing with defocus on (the blurred frame is constant in time); on the moving scene the
+    blur lowers the largest log step between neighbouring pixels."""
+    spec = scenes.small(scenes.config(1), height=40, width=56, num_keyframes=3)
+    sc = scenes.make_scene(spec)
+    kf = {key: v.numpy() for key, v in scenes.render_keyframe(sc, 0).items()}
+    o = orc.Oracle(1, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                   defocus_sigma=0.5)
+    zero = np.zeros_like(kf["mv_bwd"])
+    assert len(o.step(kf["rad"], zero, kf["depth"])) == 0
+    assert len(o.step(kf["rad"], zero, kf["depth"])) == 0 and o.holes == 0
+    sharp = orc.log_luminance(kf["rad"], spec.log_eps)[0]
+    soft = o.Lprev[0]
+    assert np.abs(np.diff(soft, axis=1)).max() < np.abs(np.diff(sharp, axis=1)).max()
