@@ -65,6 +65,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based, 1..4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--envs", type=int, default=0, help="override the number of envs (0 = the config's)")
+    ap.add_argument("--defocus", type=float, default=None,
+                    help="switch the defocus blur on (sigma in pixels, PAPER.md:158): a variant measurement, not the headline")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
@@ -230,8 +232,12 @@ def run_ours(args, spec) -> None:
     kfs = [scenes.render_keyframe(sc, k, device=dev) for k in range(n_kf)]
     path = binding.PATH_AUTO
     cap = int(min(0x7FFFFFFF, max(1 << 22, 10 * E * H * W)))          # events stored per step
-    mk = lambda: binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
-                              max_motion_px=spec.max_motion_px(), path=path, device=local, event_capacity=cap)
+    def mk():
+        e = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                         max_motion_px=spec.max_motion_px(), path=path, device=local, event_capacity=cap)
+        if args.defocus is not None:
+            e.set_defocus(args.defocus)
+        return e
     ev = mk()
     stream = torch.cuda.current_stream(dev)
 
@@ -328,7 +334,8 @@ def run_ours(args, spec) -> None:
 
     out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": K, "warmup": Wm,
            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "f32", "data": "synthetic", "config": workload_config(spec, path_used),
+           "dtype": "f32", "data": "synthetic",
+           "config": dict(workload_config(spec, path_used), **({"defocus_sigma": args.defocus} if args.defocus is not None else {})),
            "events_per_s": events / (ms * 1e-3), "events_per_step": ev_per_step,
            "x_realtime": spec.keyframe_dt / (ms / K * 1e-3),
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}

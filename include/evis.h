@@ -189,6 +189,18 @@ int evis_set_interval_index(evis_ctx *ctx, uint32_t next_kf);
  * later evis_step calls: set it before the first one.  Errors: INVALID_ARG. */
 int evis_set_channel(evis_ctx *ctx, int channel);
 
+/* Defocus ("Prior to the event generation, the linear intensity is convolved with a separable Gaussian
+ * kernel"; 0.1-0.5 px in the paper's sim-to-real data; R31).  With sigma >= 0 (pixels) the
+ * frame the event model sees at every substep is log(G_sigma * I_hat + eps): the warped frame in LINEAR intensity
+ * (the composite applied to the keyframes' linear luminance or channel; a hole holds its previous unblurred value),
+ * convolved with a separable Gaussian -- taps k = -R..R, R = ceil(3 sigma) <= 8, w_k = exp(-k^2 / (2 sigma^2)) / sum,
+ * rows then columns, the frame's border replicated -- and only then logged.  With a margin the blur runs on the whole
+ * over-rendered frame.  sigma = 0 is a single tap (the plain path up to the rounding of the linear intensity).  Call it
+ * before the first evis_step (L_ref starts from the blurred first keyframe); composite mode 0 only.
+ * Errors: INVALID_ARG (negative or non-finite sigma, sigma > 8/3, composite mode 1), BAD_STATE (after the first
+ * step), CUDA, OOM. */
+int evis_set_defocus(evis_ctx *ctx, float sigma);
+
 /* Over-render margin (Supp. B 317-319; R27): the frames handed to evis_step (height x
  * width of the configuration) were rendered with `margin` extra pixels on each side.  The warp uses all of them;
  * the margin is cropped off afterwards: the event model runs and events exist only for the inner

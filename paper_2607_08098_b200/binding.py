@@ -55,7 +55,7 @@ class evis_profile(C.Structure):
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
            "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end",
-           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end"]
+           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus"]
 
 _lib = None
 
@@ -98,6 +98,7 @@ def load() -> C.CDLL:
     L.evis_read_voxels.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_uint32)]
     L.evis_read_voxels_begin.argtypes = [vp, vp, C.c_int, C.c_int]
     L.evis_read_voxels_end.argtypes = [vp]
+    L.evis_set_defocus.argtypes = [vp, C.c_float]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
     for name in SYMBOLS:
@@ -235,6 +236,10 @@ class Evis:
 
     def read_voxels_end(self) -> None:
         _check(self._lib.evis_read_voxels_end(self._ctx), "evis_read_voxels_end")
+
+    def set_defocus(self, sigma: float) -> None:
+        """evis_set_defocus: Gaussian blur of the warped linear frame before the event model."""
+        _check(self._lib.evis_set_defocus(self._ctx, float(sigma)), "evis_set_defocus")
 
     def set_channel(self, channel: int) -> None:
         """evis_set_channel (colour events): 0 / 1 / 2 = log of R / G / B, -1 = Rec.709 luminance."""

@@ -2,6 +2,7 @@
 // No step of the path runs on the host: this file only allocates, validates and enqueues kernels.
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -75,6 +76,15 @@ struct evis_ctx {
     unsigned long long *h_counters;   // pinned host mirror
     unsigned long long arrival_cap;   // slots of the arrival buffer (capacity + slab slack)
     DebugOut dbg;
+
+    // defocus (evis_set_defocus, R31): taps, the keyframes' linear intensity (one allocation, A and B
+    // alternate like kf[].L), the carried unblurred frame and the warped linear frames of one chunk per region
+    bool defocus;
+    BlurTaps taps;
+    float *lin[2];
+    float *i_prev;
+    float *frames;                    // nreg regions of frames_elems floats
+    size_t frames_elems;
 
     // voxel grid (evis_set_voxels): V in 32.32 fixed point, its float32 image for the read calls
     bool vox_on, vox_restart;
@@ -212,6 +222,7 @@ void free_all(evis_ctx *ctx)
     cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
     cudaFree(ctx->vox_v); cudaFree(ctx->vox_out);
+    cudaFree(ctx->lin[0]); cudaFree(ctx->i_prev); cudaFree(ctx->frames);
     for (int k = 0; k < 2; ++k) {
         cudaFree(ctx->st_rad[k]); cudaFree(ctx->st_mv[k]); cudaFree(ctx->st_fwd[k]); cudaFree(ctx->st_depth[k]);
         if (ctx->ev_up[k]) cudaEventDestroy(ctx->ev_up[k]);
@@ -489,7 +500,13 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         Span sp(ctx, st, EVIS_STAGE_PREP, 1);
         CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, ctx->channel_set ? ctx->channel : -1, B.L, B.mv, B.fwd, B.Z,
                        first ? ctx->l_ref : nullptr, first ? ctx->l_prev : nullptr,
-                       ctx->cfg.max_motion_px, ctx->counters + C_MOTION, st));
+                       ctx->cfg.max_motion_px, ctx->counters + C_MOTION, ctx->defocus ? ctx->lin[ctx->cur] : nullptr, st));
+        if (ctx->defocus && first) {
+            // the event model's first frame is the blurred keyframe too; the carried unblurred frame is the keyframe
+            CU(launch_blur_log(ctx->lin[ctx->cur], g.E, g.H, g.W, ctx->taps, ctx->cfg.log_eps, ctx->l_ref, ctx->l_prev, st));
+            CU(cudaMemcpyAsync(ctx->i_prev, ctx->lin[ctx->cur], P * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            ctx->launches += 2;
+        }
     }
     ctx->last_stream = st;
     if (first) {
@@ -572,7 +589,15 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                     zc.tag = (uint32_t)--ctx->ztag[r];
                 }
                 { Span sp(ctx, cs, EVIS_STAGE_SPLAT, multi ? 0 : 1, !multi); CU(launch_global_splat(g, zc, A, B, ctx->h_tab, cs)); }
-                {
+                if (ctx->defocus) {
+                    // two passes (R31): the warped LINEAR frames of the chunk, then blur + log + Eq. 4
+                    Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 2, !multi);
+                    FrameIO fio{ctx->frames + (size_t)r * ctx->frames_elems, ctx->taps, ctx->cfg.log_eps};
+                    CU(launch_resolve_frames(g, zc, ctx->lin[ctx->cur ^ 1], ctx->lin[ctx->cur], ctx->h_tab, ctx->i_prev, ctx->ep,
+                                             cnt + C_HOLES, ctx->dbg, fio, cs));
+                    CU(launch_resolve_blurred(g, zc, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, th, rf, sink, cnt + C_HOLES,
+                                              ctx->dbg, fio, cs));
+                } else {
                     Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 1, !multi);
                     CU(launch_global_resolve(g, zc, A, B, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, th, rf, sink,
                                              cnt + C_HOLES, ctx->dbg, cs));
@@ -733,6 +758,7 @@ int evis_set_voxels(evis_ctx *ctx, const evis_voxel_config *cfg)
     if (ctx->vox_v) {
         ctx->device_bytes -= ctx->vox_cells * (sizeof(unsigned long long) + sizeof(float));
         cudaFree(ctx->vox_v); cudaFree(ctx->vox_out);
+    cudaFree(ctx->lin[0]); cudaFree(ctx->i_prev); cudaFree(ctx->frames);
         ctx->vox_v = nullptr; ctx->vox_out = nullptr;
     }
     ctx->vox_on = false;
@@ -799,6 +825,34 @@ int evis_read_voxels_begin(evis_ctx *ctx, float *host_dst, int normalize, int re
 }
 
 int evis_read_voxels_end(evis_ctx *ctx) { return evis_read_events_end(ctx); }
+
+int evis_set_defocus(evis_ctx *ctx, float sigma)
+{
+    if (!ctx || !(sigma >= 0.0f) || !(sigma < 3.0e38f)) return EVIS_ERR_INVALID_ARG;
+    if (ctx->cfg.composite_mode != EVIS_COMPOSITE_B_PRIMARY) return EVIS_ERR_INVALID_ARG;
+    if (ctx->steps) return EVIS_ERR_BAD_STATE;          // the first keyframe already fixed L_ref
+    // R = ceil(3 sigma); w_k = exp(-k^2 / (2 sigma^2)) / sum in binary64, rounded to binary32 (R31)
+    const double sg = (double)sigma;
+    const int R = sigma > 0.0f ? (int)ceil(3.0 * sg) : 0;
+    if (R > BLUR_RMAX) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    memset(&ctx->taps, 0, sizeof ctx->taps);
+    ctx->taps.R = R;
+    double sum = 0.0;
+    for (int k = -R; k <= R; ++k) sum += R ? exp(-(double)(k * k) / (2.0 * sg * sg)) : 1.0;
+    for (int k = -R; k <= R; ++k) ctx->taps.w[k + R] = (float)((R ? exp(-(double)(k * k) / (2.0 * sg * sg)) : 1.0) / sum);
+    if (!ctx->lin[0]) {
+        const size_t P = (size_t)ctx->g.E * ctx->g.HW;
+        CU(dalloc(ctx, &ctx->lin[0], 2 * P));
+        ctx->lin[1] = ctx->lin[0] + P;
+        CU(dalloc(ctx, &ctx->i_prev, P));
+        ctx->frames_elems = (size_t)ctx->chunk_ne * ctx->chunk_ni * ctx->g.HW;
+        CU(dalloc(ctx, &ctx->frames, ctx->frames_elems * ctx->nreg));
+    }
+    ctx->defocus = true;
+    return EVIS_OK;
+}
 
 int evis_set_interval_index(evis_ctx *ctx, uint32_t next_kf)
 {

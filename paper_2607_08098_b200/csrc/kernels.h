@@ -59,7 +59,21 @@ struct DebugOut {  // all nullable; [S,E,H,W]
 cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, const float *depth, long long n,
                         float eps, int channel, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
                         float *l_prev, float motion_bound /* 0 = unchecked */, unsigned long long *viol,
-                        cudaStream_t st);
+                        float *lin_out /* nullable: the linear intensity, binary32 (defocus) */, cudaStream_t st);
+
+// ---- defocus (R31) -----------------------------------------------------------------------------------
+constexpr int BLUR_RMAX = 8;                      // R = ceil(3 sigma) <= 8
+struct BlurTaps { int R; float w[2 * BLUR_RMAX + 1]; };   // w[k + R], k = -R..R
+// the resolve kernel's two passes with defocus on: pass 1 leaves the warped LINEAR frames of the chunk,
+// frames [ni_alloc][ne_alloc][HW]; pass 2 blurs them, takes the log and runs Eq. 4
+struct FrameIO {
+    float *frames;
+    BlurTaps taps;
+    float eps;
+};
+// first keyframe: l_ref = l_prev = log(G * I + eps)
+cudaError_t launch_blur_log(const float *I, int E, int H, int W, const BlurTaps &taps, float eps, float *l_ref, float *l_prev,
+                            cudaStream_t st);
 
 // ---- global z-buffer path (global_path.cu): any motion -----------------------------------------
 // z-buffers of one chunk = envs [e0, e0+ne) x substeps [i0, i0+ni):
@@ -97,6 +111,13 @@ cudaError_t launch_global_resolve(const Geom &g, const ZChunk &zc, const Keyfram
                                   const SubstepTable &tab, float *l_ref, float *l_prev,
                                   const EventParams &ep, const Thresholds &th, const Refractory &rf,
                                   const EventSink &sink, unsigned long long *holes, const DebugOut &dbg, cudaStream_t st);
+// the two defocus passes (resolve_defocus.cu)
+cudaError_t launch_resolve_frames(const Geom &g, const ZChunk &zc, const float *IA, const float *IB, const SubstepTable &tab,
+                                  float *i_prev, const EventParams &ep, unsigned long long *holes, const DebugOut &dbg,
+                                  const FrameIO &fio, cudaStream_t st);
+cudaError_t launch_resolve_blurred(const Geom &g, const ZChunk &zc, const SubstepTable &tab, float *l_ref, float *l_prev,
+                                   const EventParams &ep, const Thresholds &th, const Refractory &rf, const EventSink &sink,
+                                   unsigned long long *holes, const DebugOut &dbg, const FrameIO &fio, cudaStream_t st);
 // its four instantiation units (resolve_m*.cu): composite mode 0 / 1, without / with the debug capture
 #define EVIS_DECL_RESOLVE(name)                                                                                     \
     cudaError_t name(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B, const SubstepTable &tab,  \

@@ -15,12 +15,14 @@
 namespace evis {
 
 // channel < 0: Rec.709 luminance (Eq. 3); 0 / 1 / 2: that channel alone -- colour events (R28)
-__device__ __forceinline__ float log_lum(float r, float g, float b, double eps, int channel)
+// lin: the same intensity in LINEAR form, rounded once to binary32 (defocus, R31)
+__device__ __forceinline__ float log_lum(float r, float g, float b, double eps, int channel, float &lin)
 {
     double I = __dadd_rn(__dadd_rn(__dmul_rn(0.2126, (double)r), __dmul_rn(0.7152, (double)g)),
                          __dmul_rn(0.0722, (double)b));
     if (channel >= 0) I = (double)(channel == 0 ? r : (channel == 1 ? g : b));
     if (!(I > 0.0)) I = 0.0;
+    lin = __double2float_rn(I);
     return __double2float_rn(log(__dadd_rn(I, eps)));
 }
 
@@ -31,7 +33,7 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
        const float *__restrict__ depth, long long n, float eps_f, int channel,
        float *__restrict__ L, float2 *__restrict__ mv_out, float2 *__restrict__ fwd_out,
        float *__restrict__ Z, float *__restrict__ l_ref, float *__restrict__ l_prev, float bound,
-       unsigned long long *__restrict__ viol)
+       unsigned long long *__restrict__ viol, float *__restrict__ lin_out /* nullable: linear intensity (defocus) */)
 {
     bool over = false;       // a motion vector beyond the bound the caller declared (max_motion_px)
     const double eps = (double)eps_f;
@@ -41,12 +43,13 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
         if (p >= n) return;
         const float4 *r4 = reinterpret_cast<const float4 *>(rad + 3 * p);
         const float4 a = __ldcs(r4), b = __ldcs(r4 + 1), c = __ldcs(r4 + 2);
-        float4 l;
-        l.x = log_lum(a.x, a.y, a.z, eps, channel);
-        l.y = log_lum(a.w, b.x, b.y, eps, channel);
-        l.z = log_lum(b.z, b.w, c.x, eps, channel);
-        l.w = log_lum(c.y, c.z, c.w, eps, channel);
+        float4 l, li;
+        l.x = log_lum(a.x, a.y, a.z, eps, channel, li.x);
+        l.y = log_lum(a.w, b.x, b.y, eps, channel, li.y);
+        l.z = log_lum(b.z, b.w, c.x, eps, channel, li.z);
+        l.w = log_lum(c.y, c.z, c.w, eps, channel, li.w);
         *reinterpret_cast<float4 *>(L + p) = l;
+        if (lin_out) *reinterpret_cast<float4 *>(lin_out + p) = li;
         if (l_ref) {                                  // first keyframe: L_ref = L_prev = L   (R6)
             *reinterpret_cast<float4 *>(l_ref + p) = l;
             *reinterpret_cast<float4 *>(l_prev + p) = l;
@@ -70,8 +73,10 @@ k_prep(const float *__restrict__ rad, const float *__restrict__ mv, const float 
         *reinterpret_cast<float4 *>(Z + p) = __ldcs(reinterpret_cast<const float4 *>(depth + p));
     } else {
         if (t >= n) return;
-        const float l = log_lum(rad[3 * t], rad[3 * t + 1], rad[3 * t + 2], eps, channel);
+        float li;
+        const float l = log_lum(rad[3 * t], rad[3 * t + 1], rad[3 * t + 2], eps, channel, li);
         L[t] = l;
+        if (lin_out) lin_out[t] = li;
         if (l_ref) { l_ref[t] = l; l_prev[t] = l; }
         mv_out[t] = make_float2(mv[2 * t], mv[2 * t + 1]);
         over = fmaxf(fabsf(mv[2 * t]), fabsf(mv[2 * t + 1])) > bound;
@@ -88,18 +93,51 @@ static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 
 
 cudaError_t launch_prep(const float *rad, const float *mv, const float *fwd, const float *depth, long long n,
                         float eps, int channel, float *L, float2 *mv_out, float2 *fwd_out, float *Z, float *l_ref,
-                        float *l_prev, float bound, unsigned long long *viol, cudaStream_t st)
+                        float *l_prev, float bound, unsigned long long *viol, float *lin_out, cudaStream_t st)
 {
     if (!(bound > 0.0f)) bound = __builtin_inff();      // no bound declared: nothing to check
-    const bool vec = (n % 4 == 0) && aligned16(rad) && aligned16(mv) && aligned16(depth) && (!fwd || aligned16(fwd));
+    const bool vec = (n % 4 == 0) && aligned16(rad) && aligned16(mv) && aligned16(depth) && (!fwd || aligned16(fwd)) && (!lin_out || aligned16(lin_out));
     if (vec) {
         const long long threads = n / 4;
         k_prep<true><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, channel, L, mv_out,
-                                                                         fwd_out, Z, l_ref, l_prev, bound, viol);
+                                                                         fwd_out, Z, l_ref, l_prev, bound, viol, lin_out);
     } else {
         k_prep<false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(rad, mv, fwd, depth, n, eps, channel, L, mv_out,
-                                                                    fwd_out, Z, l_ref, l_prev, bound, viol);
+                                                                    fwd_out, Z, l_ref, l_prev, bound, viol, lin_out);
     }
+    return cudaGetLastError();
+}
+
+// Defocus (R31): the event model's first frame is the blurred keyframe as well: L_ref = L_prev =
+// log(G * I + eps).  One thread per pixel; the row sums it needs are recomputed with the pass order of the reading
+// (rows first, each rounded to binary32, then the column sum; replicated border; acc = fmaf(w_k, v_k, acc), k = -R..R).
+__global__ void __launch_bounds__(256)
+k_blur_log(const float *__restrict__ I, int E, int H, int W, const BlurTaps taps, float eps_f, float *__restrict__ l_ref,
+           float *__restrict__ l_prev)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long HW = (long long)H * W;
+    if (t >= (long long)E * HW) return;
+    const int e = (int)(t / HW), p = (int)(t - (long long)e * HW), y = p / W, x = p - y * W;
+    const float *src = I + (size_t)e * HW;
+    const int R = taps.R;
+    float acc = 0.0f;
+    for (int ky = -R; ky <= R; ++ky) {
+        const int yy = min(max(y + ky, 0), H - 1);
+        float row = 0.0f;
+        for (int kx = -R; kx <= R; ++kx) row = __fmaf_rn(taps.w[kx + R], __ldg(src + yy * W + min(max(x + kx, 0), W - 1)), row);
+        acc = __fmaf_rn(taps.w[ky + R], row, acc);
+    }
+    const float l = __double2float_rn(log(__dadd_rn((double)acc, (double)eps_f)));
+    l_ref[t] = l;
+    l_prev[t] = l;
+}
+
+cudaError_t launch_blur_log(const float *I, int E, int H, int W, const BlurTaps &taps, float eps, float *l_ref, float *l_prev,
+                            cudaStream_t st)
+{
+    const long long n = (long long)E * H * W;
+    k_blur_log<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(I, E, H, W, taps, eps, l_ref, l_prev);
     return cudaGetLastError();
 }
 

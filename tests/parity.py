@@ -133,7 +133,7 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
                mode: int = 0, path: int = binding.PATH_GLOBAL, use_fwd: bool = True, debug: bool = True,
                capacity: int = 1 << 24, max_motion: Optional[float] = None, thresholds=None,
                tau_r: float = 0.0, margin: int = 0, channel: Optional[int] = None, mutate=None,
-               render_device: str = "cuda") -> ParityReport:
+               render_device: str = "cuda", defocus: Optional[float] = None) -> ParityReport:
     """GPU runs the whole batch; the oracle runs ``envs`` (default: all).  Returns the report after
     asserting every bit-exact criterion; tolerances are asserted by the caller on the report."""
     sc = scenes.make_scene(spec)
@@ -152,10 +152,13 @@ def run_parity(spec: scenes.SceneSpec, n_keyframes: int, *, envs: Optional[Seque
         ev.set_channel(channel)
     if margin:                                      # over-render margin: spec = the over-rendered frame
         ev.set_margin(margin)
+    if defocus is not None:                         # defocus
+        ev.set_defocus(defocus)
     inner = (Ellipsis, slice(margin, H - margin), slice(margin, W - margin))
     ora = orc.Oracle(len(sel), H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
                      composite_mode=mode, debug=True, theta_on=None if th_np is None else th_np[0],
-                     theta_off=None if th_np is None else th_np[1], tau_r=tau_r, margin=margin, channel=channel)
+                     theta_off=None if th_np is None else th_np[1], tau_r=tau_r, margin=margin, channel=channel,
+                     defocus_sigma=defocus)
     rep = ParityReport()
     try:
         for k in range(n_keyframes):

@@ -956,3 +956,43 @@ def test_voxels_only_mode_and_api_contract():
     assert [n for _, n in gc] == [1, 1, 2]                 # the window restarted after the first interval
     assert abs(float(gc[1][0].sum()) - cc[1]) < 0.5
     ev_c.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# defocus (reading R31)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("sigma,cfg,kw", [(0.5, 1, {}), (0.3, 4, {}), (1.2, 2, {}), (2.5, 1, {}), (0.0, 1, {}),
+                                          (0.5, 4, {"margin": 7}), (0.4, 1, {"tau_r": 1e-3}), (0.5, 1, {"channel": 2})])
+def test_defocus_matches_the_oracle(sigma, cfg, kw):
+    """evis_set_defocus: winners bit-exact, the blurred log frame within 1e-5, events exact up to reported ties, carried
+    L_ref / L_prev -- over the paper's range of sigma (0.1-0.5 px) and beyond (R up to 8), with holes (cfg 2 / 4 scenes),
+    the margin crop, the refractory period and a colour channel."""
+    spec = scenes.small(scenes.config(cfg), num_envs=2 if cfg != 1 else 1, height=83, width=117, num_keyframes=4)
+    rep = parity.run_parity(spec, 4, defocus=sigma, **kw)
+    _assert_tolerances(rep)
+    assert rep.events_oracle > 500
+
+
+@pytest.mark.gpu
+def test_defocus_api_contract():
+    spec = scenes.small(scenes.config(1), height=65, width=87, num_keyframes=2)
+    mk = lambda mode: binding.Evis(1, 65, 87, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                                   composite_mode=mode, event_capacity=1 << 20)
+    ev = mk(0)
+    for bad in (-0.1, float("nan"), float("inf"), 2.7):          # ceil(3 * 2.7) = 9 > 8 taps per side
+        with pytest.raises(binding.EvisError) as ei:
+            ev.set_defocus(bad)
+        assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+    ev.set_defocus(0.5)
+    kf = scenes.render_keyframe(scenes.make_scene(spec), 0, device="cuda")
+    ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], sync=True)
+    with pytest.raises(binding.EvisError) as ei:
+        ev.set_defocus(0.3)
+    assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    ev.destroy()
+    ev = mk(1)
+    with pytest.raises(binding.EvisError) as ei:
+        ev.set_defocus(0.5)
+    assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+    ev.destroy()
