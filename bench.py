@@ -67,6 +67,9 @@ def parse_args():
     ap.add_argument("--envs", type=int, default=0, help="override the number of envs (0 = the config's)")
     ap.add_argument("--defocus", type=float, default=None,
                     help="switch the defocus blur on (sigma in pixels, PAPER.md:158): a variant measurement, not the headline")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank its own batch of the config's shape (default); strong = ONE batch of the "
+                         "config's shape, rank r takes the envs sharding.env_block(r, N, E) (sharding.ShardedEvis)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
@@ -223,13 +226,24 @@ def run_ours(args, spec) -> None:
         dist.init_process_group("nccl", device_id=dev)
     binding.load()                                     # fails loudly when libevis.so is missing
 
-    # every rank: its own batch of the same shape (envs are independent: no exchange step)
-    spec = scenes.small(spec, seed=sharding.rank_seed(spec.seed, rank))
-    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
     K, Wm = args.steps, args.warmup
-    sc = scenes.make_scene(spec)
     n_kf = Wm + K + 1
-    kfs = [scenes.render_keyframe(sc, k, device=dev) for k in range(n_kf)]
+    if args.scaling == "strong" and world > 1:
+        # ONE batch: rank r owns the envs env_block(r, world, E) of it (no exchange step); it renders only those
+        e0, e1 = sharding.env_block(rank, world, spec.num_envs)
+        if e1 == e0:
+            raise SystemExit("bench.py: more ranks than environments")
+        sc = scenes.make_scene(spec)
+        kfs = [scenes.render_keyframe(sc, k, device=dev, envs=list(range(e0, e1))) for k in range(n_kf)]
+        global_envs = spec.num_envs
+        spec = scenes.small(spec, num_envs=e1 - e0)
+    else:
+        # every rank: its own batch of the same shape (envs are independent: no exchange step)
+        spec = scenes.small(spec, seed=sharding.rank_seed(spec.seed, rank))
+        sc = scenes.make_scene(spec)
+        kfs = [scenes.render_keyframe(sc, k, device=dev) for k in range(n_kf)]
+        global_envs = spec.num_envs * world
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
     path = binding.PATH_AUTO
     cap = int(min(0x7FFFFFFF, max(1 << 22, 10 * E * H * W)))          # events stored per step
     def mk():
@@ -297,8 +311,7 @@ def run_ours(args, spec) -> None:
 
     (ms,), (events, launches) = sharding.reduce_max_sum([ms], [float(events), float(launches)], dev)
     launches = int(launches)
-    pxss_rank = E * H * W * S * K
-    value = world * pxss_rank / (ms * 1e-3)
+    value = global_envs * H * W * S * K / (ms * 1e-3)        # all ranks' pixel-substeps over the slowest rank's time
 
     # ---- roofline: the WHOLE step's algorithmic bytes over the WHOLE step's time (the path is one fused pass over the
     #      keyframes: its stages overlap on several streams, so no stage is charged the bytes alone) --------------------
@@ -333,7 +346,7 @@ def run_ours(args, spec) -> None:
                                   "frac_vs_survey_bounds": [n * pxss_step / step_s / ISSUE_PEAK for n in SURVEY_INSTR_BOUNDS]}
 
     out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": K, "warmup": Wm,
-           "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "ms_per_step": ms / K, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic",
            "config": dict(workload_config(spec, path_used), **({"defocus_sigma": args.defocus} if args.defocus is not None else {})),
            "events_per_s": events / (ms * 1e-3), "events_per_step": ev_per_step,
@@ -394,7 +407,7 @@ def run_ours(args, spec) -> None:
                     raise SystemExit("bench.py: the downloaded accumulation image does not hold the step's events")
             ev.destroy()
             (dt,), _ = sharding.reduce_max_sum([dt], [], dev)
-            return {"value": world * E * H * W * S * Ke / dt, "unit": METRIC, "steps": Ke,
+            return {"value": global_envs * H * W * S * Ke / dt, "unit": METRIC, "steps": Ke,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(got / Ke), "ms_per_step": dt / Ke * 1e3,
                     "x_realtime": spec.keyframe_dt / (dt / Ke)}
 

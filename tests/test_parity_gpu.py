@@ -996,3 +996,50 @@ def test_defocus_api_contract():
         ev.set_defocus(0.5)
     assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
     ev.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# env-sharded multi-GPU entry; one GPU here, so the two shards run one after the other
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("world", [2, 3])
+def test_env_shards_reproduce_the_single_context_stream(world):
+    """sharding.ShardedEvis: the union of the ranks' event streams (local env + e0) is the single-context stream of the
+    whole batch, event for event and bit for bit, and the carried state is the slice of the single context's."""
+    from paper_2607_08098_b200 import sharding
+    spec = scenes.small(scenes.config(4), num_envs=5, height=70, width=93, num_keyframes=4)
+    sc = scenes.make_scene(spec)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    args = (H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(spec.num_keyframes)]
+    key = lambda e: np.sort(e, order=["kf", "env", "substep", "y", "x", "t_off"])
+
+    one = binding.Evis(E, *args, event_capacity=1 << 22)
+    ref = []
+    for kf in kfs:
+        one.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        ref.append(one.read_events().copy())
+    ref_state = one.get_state()
+    one.destroy()
+    ref = np.concatenate(ref)
+
+    got, covered = [], []
+    for rank in range(world):
+        sh = sharding.ShardedEvis(E, *args, rank=rank, world=world, event_capacity=1 << 22)
+        covered += list(range(sh.e0, sh.e1))
+        for k, kf in enumerate(kfs):
+            if k % 2:          # either the rank slices the batch tensors, or it renders its own envs
+                loc = {a: sh.local(b) for a, b in kf.items()}
+            else:
+                loc = scenes.render_keyframe(sc, k, device="cuda", envs=list(range(sh.e0, sh.e1)))
+            n = sh.step(loc["rad"], loc["mv_bwd"], loc["depth"], mv_fwd=loc["mv_fwd"], sync=True)
+            e = sh.read_events().copy()
+            assert len(e) == n and sh.gather_counts(n) == [n]        # no process group: identity
+            e["env"] = sh.global_env(e).astype(e["env"].dtype)
+            got.append(e)
+        lr, lp = sh.ctx.get_state()
+        assert np.array_equal(lr, ref_state[0][sh.e0:sh.e1]) and np.array_equal(lp, ref_state[1][sh.e0:sh.e1])
+        sh.destroy()
+    assert covered == list(range(E))
+    got = np.concatenate(got)
+    assert len(ref) > 1000 and key(got).tobytes() == key(ref).tobytes()

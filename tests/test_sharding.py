@@ -33,7 +33,16 @@ def _worker(rank, world, port, out):
         e0, e1 = sharding.env_block(rank, world, 5)
         ms = 10.0 + 3.0 * rank                       # rank 1 is the slow one
         mx, sm = sharding.reduce_max_sum([ms], [float(e1 - e0), 100.0 * (rank + 1)], torch.device("cpu"))
-        out[rank] = (mx, sm, sharding.rank_seed(42, rank))
+        # strong scaling: the rank renders ITS envs of the one shared batch; the slices tile the whole keyframe
+        from paper_2607_08098_b200 import scenes
+        import hashlib
+        spec = scenes.small(scenes.config(4), num_envs=5, height=24, width=32, num_keyframes=2)
+        sc = scenes.make_scene(spec)
+        mine = scenes.render_keyframe(sc, 1, envs=list(range(e0, e1)))
+        whole = scenes.render_keyframe(sc, 1)
+        same = all(torch.equal(mine[k], whole[k][e0:e1]) for k in mine)
+        counts = sharding.gather_counts(1000 * (rank + 1) + (e1 - e0), torch.device("cpu"))
+        out[rank] = (mx, sm, sharding.rank_seed(42, rank), same, counts, (e0, e1))
     finally:
         dist.destroy_process_group()
 
@@ -46,9 +55,14 @@ def test_two_gloo_ranks_reduce_max_time_and_sum_counters():
     out = mgr.dict()
     mp.spawn(_worker, args=(2, port, out), nprocs=2, join=True)
     assert out[0][:2] == out[1][:2]
-    mx, sm, _ = out[0]
+    mx, sm = out[0][:2]
     assert mx == [13.0] and sm == [5.0, 300.0]       # max time; all 5 envs accounted for; counters summed
     assert out[0][2] != out[1][2]                     # different batches per rank (weak scaling)
+    # strong scaling (ShardedEvis): the ranks' renders are the slices of the one batch; the count all-gather (the only
+    # collective of the sharded path) returns every rank's count to every rank, in rank order
+    assert out[0][3] and out[1][3]
+    assert out[0][4] == out[1][4] == [1003, 2002]
+    assert out[0][5] == (0, 3) and out[1][5] == (3, 5)
 
 
 def test_single_process_reduction_is_identity():
