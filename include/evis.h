@@ -251,6 +251,13 @@ int evis_read_voxels(evis_ctx *ctx, float *dst, int dst_is_device, int normalize
 int evis_read_voxels_begin(evis_ctx *ctx, float *host_dst, int normalize, int restart);
 int evis_read_voxels_end(evis_ctx *ctx);
 
+/* Time-sorted per-environment stream (the stream E = {(u_k, t_k, p_k)} of PAPER.md:90 in time order): with on != 0 the
+ * stored stream of every later step is ordered by (env, t_off); events of one environment with equal timestamps keep
+ * the deterministic order described at evis_read_events, so the result does not depend on scheduling.  A stable
+ * segmented radix sort on the device, behind the step like the rest of the ordering stage (about 9 extra passes over
+ * the stored events).  Needs the event stream (not a voxels-only context).  Synchronises.  Errors: INVALID_ARG, CUDA, OOM. */
+int evis_set_time_sorted(evis_ctx *ctx, int on);
+
 /* Copy the events of the last step, in the deterministic order
  * (env, substep, tile row, tile column, y, x, crossing k), to `dst` (room for `max` events;
  * device pointer if dst_is_device != 0, else host).  Synchronises.  *n_out = events copied

@@ -55,7 +55,7 @@ class evis_profile(C.Structure):
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
            "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end",
-           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus"]
+           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus", "evis_set_time_sorted"]
 
 _lib = None
 
@@ -99,6 +99,7 @@ def load() -> C.CDLL:
     L.evis_read_voxels_begin.argtypes = [vp, vp, C.c_int, C.c_int]
     L.evis_read_voxels_end.argtypes = [vp]
     L.evis_set_defocus.argtypes = [vp, C.c_float]
+    L.evis_set_time_sorted.argtypes = [vp, C.c_int]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
     for name in SYMBOLS:
@@ -236,6 +237,10 @@ class Evis:
 
     def read_voxels_end(self) -> None:
         _check(self._lib.evis_read_voxels_end(self._ctx), "evis_read_voxels_end")
+
+    def set_time_sorted(self, on: bool = True) -> None:
+        """evis_set_time_sorted: the stored stream of later steps is ordered by (env, t_off), stable."""
+        _check(self._lib.evis_set_time_sorted(self._ctx, int(bool(on))), "evis_set_time_sorted")
 
     def set_defocus(self, sigma: float) -> None:
         """evis_set_defocus: Gaussian blur of the warped linear frame before the event model."""

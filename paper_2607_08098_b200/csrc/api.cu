@@ -86,6 +86,11 @@ struct evis_ctx {
     float *frames;                    // nreg regions of frames_elems floats
     size_t frames_elems;
 
+    // time-sorted stream (evis_set_time_sorted): workspace of the segmented radix sort
+    bool time_sorted;
+    void *sort_ws;
+    size_t sort_ws_bytes;
+
     // voxel grid (evis_set_voxels): V in 32.32 fixed point, its float32 image for the read calls
     bool vox_on, vox_restart;
     evis_voxel_config vox;
@@ -221,7 +226,7 @@ void free_all(evis_ctx *ctx)
     cudaFree(ctx->l_ref); cudaFree(ctx->l_prev); cudaFree(ctx->th_on); cudaFree(ctx->th_off); cudaFree(ctx->t_last); cudaFree(ctx->hot); cudaFree(ctx->tab); cudaFree(ctx->zmem);
     cudaFree(ctx->arrival); cudaFree(ctx->ordered); cudaFree(ctx->directory); cudaFree(ctx->bsum);
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
-    cudaFree(ctx->vox_v); cudaFree(ctx->vox_out);
+    cudaFree(ctx->vox_v); cudaFree(ctx->vox_out); cudaFree(ctx->sort_ws);
     cudaFree(ctx->lin[0]); cudaFree(ctx->i_prev); cudaFree(ctx->frames);
     for (int k = 0; k < 2; ++k) {
         cudaFree(ctx->st_rad[k]); cudaFree(ctx->st_mv[k]); cudaFree(ctx->st_fwd[k]); cudaFree(ctx->st_depth[k]);
@@ -644,6 +649,13 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
             CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
                             cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, vs, os));
         }
+        if (ctx->time_sorted && vs.store_events) {
+            // the arrival buffer of this slot is free once the stream has been laid out: it is the sort's scratch
+            CU(launch_time_sort(sink.directory, ctx->dir_entries, rf.t_last ? 0 : DIR_EV_SHIFT, (uint32_t)g.E,
+                                ctx->cfg.event_capacity < ctx->arrival_cap ? ctx->cfg.event_capacity : ctx->arrival_cap,
+                                ctx->ordered, ctx->arrival_s[sl], ctx->sort_ws, os));
+            ctx->launches += 14;
+        }
         CU(cudaMemcpyAsync(ctx->h_counters, cnt, C_STEP_END * sizeof(unsigned long long), cudaMemcpyDeviceToHost, os));
         CU(cudaMemcpyAsync(ctx->h_counters + C_MOTION, sticky + C_MOTION, (NCOUNTERS - C_MOTION) * sizeof(unsigned long long),
                            cudaMemcpyDeviceToHost, os));
@@ -757,7 +769,7 @@ int evis_set_voxels(evis_ctx *ctx, const evis_voxel_config *cfg)
     if (ctx->copy_pending) { CU(cudaStreamSynchronize(ctx->copy_stream)); ctx->copy_pending = false; }
     if (ctx->vox_v) {
         ctx->device_bytes -= ctx->vox_cells * (sizeof(unsigned long long) + sizeof(float));
-        cudaFree(ctx->vox_v); cudaFree(ctx->vox_out);
+        cudaFree(ctx->vox_v); cudaFree(ctx->vox_out); cudaFree(ctx->sort_ws);
     cudaFree(ctx->lin[0]); cudaFree(ctx->i_prev); cudaFree(ctx->frames);
         ctx->vox_v = nullptr; ctx->vox_out = nullptr;
     }
@@ -825,6 +837,21 @@ int evis_read_voxels_begin(evis_ctx *ctx, float *host_dst, int normalize, int re
 }
 
 int evis_read_voxels_end(evis_ctx *ctx) { return evis_read_events_end(ctx); }
+
+int evis_set_time_sorted(evis_ctx *ctx, int on)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->steps) CU(sync_all(ctx));
+    if (on && !ctx->sort_ws) {
+        ctx->sort_ws_bytes = sort_workspace_bytes((uint32_t)ctx->g.E, ctx->cfg.event_capacity);
+        CU(cudaMalloc(&ctx->sort_ws, ctx->sort_ws_bytes));
+        ctx->device_bytes += ctx->sort_ws_bytes;
+    }
+    ctx->time_sorted = on != 0;
+    return EVIS_OK;
+}
 
 int evis_set_defocus(evis_ctx *ctx, float sigma)
 {

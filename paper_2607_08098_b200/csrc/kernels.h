@@ -160,6 +160,11 @@ cudaError_t launch_expand(const EventSink &sink, uint32_t num_entries, unsigned 
                           unsigned long long capacity, const unsigned long long *step_events,
                           unsigned long long *total_events, unsigned long long *overflow_steps, const EventParams &ep, const Thresholds &th, uint32_t W,
                           uint32_t HW, uint32_t margin, uint32_t tiles_x, uint32_t tiles, uint32_t S, const VoxelSink &vox, cudaStream_t st);
+// ---- time-sorted per-env stream (sort.cu): stable segmented radix sort of the ordered stream by (env, t_off) -------
+size_t sort_workspace_bytes(uint32_t E, unsigned long long capacity);
+cudaError_t launch_time_sort(const uint2 *directory, uint32_t num_entries, int dir_shift, uint32_t E, unsigned long long capacity,
+                             uint4 *a /* ordered stream, sorted in place */, uint4 *b /* scratch, same size */, void *ws,
+                             cudaStream_t st);
 // number of values among theta[0..n) that are not (finite and > 0), added to *bad (prep.cu)
 cudaError_t launch_check_positive(const float *theta, long long n, unsigned long long *bad, cudaStream_t st);
 

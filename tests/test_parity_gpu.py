@@ -1043,3 +1043,56 @@ def test_env_shards_reproduce_the_single_context_stream(world):
     assert covered == list(range(E))
     got = np.concatenate(got)
     assert len(ref) > 1000 and key(got).tobytes() == key(ref).tobytes()
+
+
+# ------------------------------------------------------------------------------------------------
+# time-sorted per-env stream
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,E,tau_r", [(4, 5, 0.0), (1, 1, 0.0), (2, 3, 0.0), (4, 3, 1e-3)])
+def test_time_sorted_stream(cfg, E, tau_r):
+    """evis_set_time_sorted: the stored stream is the unsorted stream stably sorted by (env, t_off) -- checked byte for
+    byte against numpy's stable lexsort of the library's own unsorted stream --, and it agrees with the oracle's stream
+    in time order (oracle/evis_outputs.sort_by_time): same pixels and polarities wherever the stamps are distinct, stamps
+    within 1e-7 s."""
+    from oracle import evis_outputs as oout
+    spec = scenes.small(scenes.config(cfg), num_envs=E, height=97, width=131, num_keyframes=3)
+    sc = scenes.make_scene(spec)
+    H, W, S = spec.height, spec.width, spec.substeps
+    mk = lambda: binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                              max_motion_px=spec.max_motion_px(), event_capacity=1 << 22)
+    plain, srt = mk(), mk()
+    ora = orc.Oracle(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, tau_r=tau_r)
+    if tau_r > 0:
+        plain.set_refractory(tau_r); srt.set_refractory(tau_r)
+    srt.set_time_sorted(True)
+    total = 0
+    for k in range(spec.num_keyframes):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        for ev in (plain, srt):
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        h = {key: v.cpu().numpy() for key, v in kf.items()}
+        oe = ora.step(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"])
+        if k == 0:
+            continue
+        a, b = plain.read_events(), srt.read_events()
+        assert len(a) == len(b) == len(oe)
+        total += len(a)
+        want = a[np.lexsort((a["t_off"].view(np.uint32), a["env"]))]        # lexsort is stable
+        assert b.tobytes() == want.tobytes()
+        assert np.all(np.diff(b["env"].astype(np.int64)) >= 0)
+        same_env = np.diff(b["env"].astype(np.int64)) == 0
+        assert np.all(np.diff(b["t_off"])[same_env] >= 0)
+        o = oe[oout.sort_by_time(oe["env"], oe["t_off"], oe["y"], oe["x"], oe["k"])]
+        assert np.array_equal(b["env"], o["env"]) and np.abs(b["t_off"].astype(np.float64) - o["t_off"]).max() <= parity.TOL_T
+        # where a stamp is isolated by more than the tolerance on both sides the event itself must be the oracle's
+        t = o["t_off"]
+        iso = np.ones(len(t), bool)
+        near = (np.abs(np.diff(t)) <= 4 * parity.TOL_T) & (np.diff(o["env"]) == 0)
+        iso[1:] &= ~near
+        iso[:-1] &= ~near
+        assert iso.sum() > 100          # (cfg 4 ramps the brightness of a whole env: most stamps are shared by many pixels)
+        for f in ("x", "y", "p", "substep"):
+            assert np.array_equal(b[f][iso].astype(np.int64), o[f][iso].astype(np.int64)), f
+    assert total > 2000
+    plain.destroy(); srt.destroy()
