@@ -85,36 +85,48 @@ void evo_log_luminance(const float *rad /* [n][3] */, int64_t n, float eps, floa
  * Every integer pixel with positive bilinear weight is covered [R14]; per target the smallest
  * (Zt bits, source index) is kept [R15] (Eq. 6: nearest surface only).
  * zbuf[H*W] must be EVO_EMPTY-initialised by the caller.                                        */
-void evo_splat(int H, int W, int i, int S, int src_is_B,
-               const float *disp /* [H][W][2] */, const float *Zsrc, const float *Zoth,
-               uint64_t *zbuf)
+/* One source pixel (x, y) at substep i in one direction: landing position q (Eq. 5), interpolated depth zt (Eq. 7),
+ * floor cell (x0, y0) and whether the +1 neighbours carry positive weight (hx, hy).  Returns 0 when the source is
+ * skipped (invalid depth [R17] or a floor cell outside [-1, W-1] x [-1, H-1]).                                   */
+static int evo_source(int H, int W, int i, int S, int src_is_B, const float *disp, const float *Zsrc, const float *Zoth,
+                      int x, int y, float *qx_, float *qy_, float *zt_, int *x0_, int *y0_, int *hx_, int *hy_)
 {
     const float f = (float)i / (float)S;
     const float g = 1.0f - f;
     const float w = src_is_B ? g : f;
+    const int p = y * W + x;
+    const float dx = disp[2 * p + 0], dy = disp[2 * p + 1];
+    const float qx = fmaf(w, dx, (float)x);
+    const float qy = fmaf(w, dy, (float)y);
+    /* depth at the two endpoints of the correspondence */
+    const float ex = (float)x + dx, ey = (float)y + dy;
+    const float jx = floorf(ex + 0.5f), jy = floorf(ey + 0.5f);
+    const float zs = Zsrc[p];
+    float zo = zs;
+    if (jx >= 0.0f && jx <= (float)(W - 1) && jy >= 0.0f && jy <= (float)(H - 1))
+        zo = Zoth[(int)jy * W + (int)jx];
+    const float za = src_is_B ? zo : zs;
+    const float zb = src_is_B ? zs : zo;
+    const float zt = fmaf(f, zb, g * za);
+    if (!(zt > 0.0f) || isinf(zt)) return 0;                    /* [R17] */
+    const float x0f = floorf(qx), y0f = floorf(qy);
+    if (!(x0f >= -1.0f && x0f <= (float)(W - 1))) return 0;     /* also drops NaN/inf */
+    if (!(y0f >= -1.0f && y0f <= (float)(H - 1))) return 0;
+    *qx_ = qx; *qy_ = qy; *zt_ = zt;
+    *x0_ = (int)x0f; *y0_ = (int)y0f;
+    *hx_ = qx > x0f; *hy_ = qy > y0f;                           /* positive weight on the +1 neighbour */
+    return 1;
+}
+
+void evo_splat(int H, int W, int i, int S, int src_is_B,
+               const float *disp /* [H][W][2] */, const float *Zsrc, const float *Zoth,
+               uint64_t *zbuf)
+{
     for (int y = 0; y < H; ++y)
         for (int x = 0; x < W; ++x) {
-            const int p = y * W + x;
-            const float dx = disp[2 * p + 0], dy = disp[2 * p + 1];
-            const float qx = fmaf(w, dx, (float)x);
-            const float qy = fmaf(w, dy, (float)y);
-            /* depth at the two endpoints of the correspondence */
-            const float ex = (float)x + dx, ey = (float)y + dy;
-            const float jx = floorf(ex + 0.5f), jy = floorf(ey + 0.5f);
-            const float zs = Zsrc[p];
-            float zo = zs;
-            if (jx >= 0.0f && jx <= (float)(W - 1) && jy >= 0.0f && jy <= (float)(H - 1))
-                zo = Zoth[(int)jy * W + (int)jx];
-            const float za = src_is_B ? zo : zs;
-            const float zb = src_is_B ? zs : zo;
-            const float zt = fmaf(f, zb, g * za);
-            if (!(zt > 0.0f) || isinf(zt)) continue;                    /* [R17] */
-            const float x0f = floorf(qx), y0f = floorf(qy);
-            if (!(x0f >= -1.0f && x0f <= (float)(W - 1))) continue;     /* also drops NaN/inf */
-            if (!(y0f >= -1.0f && y0f <= (float)(H - 1))) continue;
-            const int x0 = (int)x0f, y0 = (int)y0f;
-            const int hx = qx > x0f, hy = qy > y0f;     /* positive weight on the +1 neighbour */
-            const uint64_t key = ((uint64_t)f32_bits(zt) << 32) | (uint32_t)p;
+            float qx, qy, zt; int x0, y0, hx, hy;
+            if (!evo_source(H, W, i, S, src_is_B, disp, Zsrc, Zoth, x, y, &qx, &qy, &zt, &x0, &y0, &hx, &hy)) continue;
+            const uint64_t key = ((uint64_t)f32_bits(zt) << 32) | (uint32_t)(y * W + x);
             for (int oy = 0; oy <= hy; ++oy)
                 for (int ox = 0; ox <= hx; ++ox) {
                     const int tx = x0 + ox, ty = y0 + oy;
@@ -122,6 +134,61 @@ void evo_splat(int H, int W, int i, int S, int src_is_B,
                     if (key < zbuf[ty * W + tx]) zbuf[ty * W + tx] = key;
                 }
         }
+}
+
+/* ---- Weighted front-surface splat [R32] --------------------------------------------------------------
+ * "These target values are then bilinearly interpolated to integer pixels.  When multiple sources land on the same
+ * target, we resolve the occlusion with a per-pixel z-buffer that retains only the nearest surface."  Read as weights
+ * (the alternative to [R14]'s winner-take-all): per direction and target q, with Z*(q) the z-buffer's depth (evo_splat),
+ * the FRONT surface is the sources covering q whose depth is within 1 % of it, zt <= 1.01f * Z*, and the target takes
+ * their bilinear-weighted mean
+ *     Lhat_X(q) = sum_s W_s L_X(p_s) / sum_s W_s ,   w_s = (1 - |q.x - qs.x|)(1 - |q.y - qs.y|)  (binary32),
+ * in the log domain like the blend of [R19]/[R23].  So that the sums do not depend on the order of the sources (the
+ * kernel adds them with integer atomics) both are integers: W_s = max(1, rint(w_s 2^20)), L in units of 2^-24
+ * (rint(L 2^24)); the quotient is taken in binary64 and rounded once to binary32.  acc[q] = {sum W L, sum W} must be
+ * zeroed by the caller; zbuf = this direction's z-buffer of the same substep.                                      */
+void evo_wsplat(int H, int W, int i, int S, int src_is_B, const float *disp, const float *Zsrc, const float *Zoth,
+                const float *Lsrc, const uint64_t *zbuf, int64_t *acc /* [H*W][2] */)
+{
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            float qx, qy, zt; int x0, y0, hx, hy;
+            if (!evo_source(H, W, i, S, src_is_B, disp, Zsrc, Zoth, x, y, &qx, &qy, &zt, &x0, &y0, &hx, &hy)) continue;
+            const float Lv = Lsrc[y * W + x];
+            if (!(fabsf(Lv) < 120.0f)) continue;                /* a non-finite log value carries no weight */
+            const int64_t Lq = (int64_t)rint((double)Lv * 16777216.0);
+            const float fx = qx - (float)x0, fy = qy - (float)y0;            /* exact */
+            for (int oy = 0; oy <= hy; ++oy)
+                for (int ox = 0; ox <= hx; ++ox) {
+                    const int tx = x0 + ox, ty = y0 + oy;
+                    if (tx < 0 || tx >= W || ty < 0 || ty >= H) continue;   /* [R18] */
+                    const uint64_t zk = zbuf[ty * W + tx];
+                    float zmin; uint32_t zb_ = (uint32_t)(zk >> 32); memcpy(&zmin, &zb_, 4);
+                    if (!(zt <= 1.01f * zmin)) continue;                     /* behind the front surface */
+                    const float wx = ox ? fx : 1.0f - fx, wy = oy ? fy : 1.0f - fy;
+                    const float w = wx * wy;
+                    int64_t Wq = (int64_t)rint((double)w * 1048576.0);
+                    if (Wq < 1) Wq = 1;
+                    acc[2 * (ty * W + tx) + 0] += Wq * Lq;
+                    acc[2 * (ty * W + tx) + 1] += Wq;
+                }
+        }
+}
+
+/* composite of the weighted mode: B primary, A fills B's holes, else hold [R19 mode 0, R20] */
+void evo_wcomposite(int H, int W, const uint64_t *zA, const uint64_t *zB, const int64_t *accA, const int64_t *accB,
+                    const float *Lprev, float *Lhat, uint8_t *win_dir, uint32_t *win_idx)
+{
+    for (int q = 0; q < H * W; ++q) {
+        const int64_t *a = zB[q] != EVO_EMPTY ? accB + 2 * q : (zA[q] != EVO_EMPTY ? accA + 2 * q : 0);
+        const uint8_t d = zB[q] != EVO_EMPTY ? 0 : (zA[q] != EVO_EMPTY ? 1 : 3);
+        /* the nearest source always belongs to its own front surface, so a reached pixel has weight unless every
+         * contributor's log value was non-finite: then it holds, like a hole                                     */
+        if (a && a[1] > 0) Lhat[q] = (float)(((double)a[0] / (double)a[1]) / 16777216.0);
+        else Lhat[q] = Lprev[q];
+        if (win_dir) win_dir[q] = d;
+        if (win_idx) win_idx[q] = d == 0 ? (uint32_t)zB[q] : (d == 1 ? (uint32_t)zA[q] : EVO_NONE);
+    }
 }
 
 /* ---- composite -----------------------------------------------------------------
@@ -418,7 +485,9 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, int margin,
                      /* defocus [R31]: blur_R < 0 = off (everything below unused).  IA / IB: linear intensity of the keyframes,
                       * Iprev: carried unblurred warped frame, eps: the log epsilon, scratch [H*W] each */
                      int blur_R, const float *blur_w, const float *IA, const float *IB, float *Iprev, float eps,
-                     float *blur_tmp, float *blur_out)
+                     float *blur_tmp, float *blur_out,
+                     /* mode 2 (weighted front-surface splat [R32]): scratch [H*W][2] each, else unused */
+                     int64_t *waccA, int64_t *waccB)
 {
     const int64_t P = (int64_t)H * W;
     int64_t made = 0;
@@ -428,7 +497,13 @@ int64_t evo_interval(int H, int W, int S, int mode, int env, int kf, int margin,
         evo_splat(H, W, i, S, 1, mB, ZB, ZA, zB);
         uint8_t *dd = dbg_dir ? dbg_dir + (int64_t)(i - 1) * P : 0;
         uint32_t *di = dbg_idx ? dbg_idx + (int64_t)(i - 1) * P : 0;
-        if (blur_R < 0) {
+        if (mode == 2) {
+            /* weighted front-surface splat [R32]: a second walk over the sources against the finished z-buffers */
+            for (int64_t q = 0; q < 2 * P; ++q) { waccA[q] = 0; waccB[q] = 0; }
+            evo_wsplat(H, W, i, S, 0, fwdA, ZA, ZB, LA, zA, waccA);
+            evo_wsplat(H, W, i, S, 1, mB, ZB, ZA, LB, zB, waccB);
+            evo_wcomposite(H, W, zA, zB, waccA, waccB, Lprev, Lhat, dd, di);
+        } else if (blur_R < 0) {
             evo_composite(H, W, i, S, mode, zA, zB, LA, LB, Lprev, Lhat, dd, di);
         } else {
             /* defocus: composite the LINEAR frame (holes hold the previous unblurred value), blur it, take the log */

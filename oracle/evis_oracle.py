@@ -47,8 +47,11 @@ def lib():
         L.evo_interval.argtypes = ([C.c_int] * 7 + [C.c_float] * 3 + [fp, fp] + [C.c_float, fp] + [C.c_void_p] + [fp] * 8 + [u64p, u64p, fp]
                                    + [C.c_void_p, C.c_int64, C.c_int64]
                                    + [u32p, u32p, u8p, u32p, fp, fp, C.POINTER(C.c_int64)]
-                                   + [C.c_int, fp, fp, fp, fp, C.c_float, fp, fp])
+                                   + [C.c_int, fp, fp, fp, fp, C.c_float, fp, fp]
+                                   + [C.POINTER(C.c_int64), C.POINTER(C.c_int64)])
         L.evo_interval.restype = C.c_int64
+        L.evo_wsplat.argtypes = [C.c_int] * 5 + [fp, fp, fp, fp, u64p, C.POINTER(C.c_int64)]
+        L.evo_wsplat.restype = None
         L.evo_linear_luminance.argtypes = [fp, C.c_int64, C.c_int, fp]
         L.evo_linear_luminance.restype = None
         L.evo_gauss_taps.argtypes = [C.c_float, fp, C.c_int]
@@ -122,6 +125,19 @@ def splat(i: int, S: int, src_is_B: bool, disp: np.ndarray, Zsrc: np.ndarray, Zo
                     _f(np.ascontiguousarray(Zsrc, np.float32)), _f(np.ascontiguousarray(Zoth, np.float32)),
                     _p(z, C.c_uint64))
     return z
+
+
+def wsplat(i: int, S: int, src_is_B: bool, disp: np.ndarray, Zsrc: np.ndarray, Zoth: np.ndarray, Lsrc: np.ndarray,
+           zbuf: np.ndarray) -> np.ndarray:
+    """Weighted front-surface accumulation [R32] of one direction against its finished z-buffer ``zbuf`` (from
+    ``splat``).  Returns acc [H,W,2] int64: (sum W L 2^24, sum W), W in units of 2^-20."""
+    H, W = Zsrc.shape
+    acc = np.zeros((H, W, 2), np.int64)
+    lib().evo_wsplat(H, W, i, S, int(src_is_B), _f(np.ascontiguousarray(disp, np.float32)),
+                     _f(np.ascontiguousarray(Zsrc, np.float32)), _f(np.ascontiguousarray(Zoth, np.float32)),
+                     _f(np.ascontiguousarray(Lsrc, np.float32)), _p(np.ascontiguousarray(zbuf, np.uint64), C.c_uint64),
+                     _p(acc, C.c_int64))
+    return acc
 
 
 def composite(i: int, S: int, mode: int, zA: np.ndarray, zB: np.ndarray, LA: np.ndarray, LB: np.ndarray,
@@ -216,6 +232,7 @@ class Oracle:
         # defocus [R31]: None = off; a sigma (>= 0) = the warped LINEAR frame of every substep is blurred
         self.taps = None if defocus_sigma is None else gauss_taps(defocus_sigma)
         assert self.taps is None or composite_mode == 0, "defocus is defined for the B-primary composite"
+        assert composite_mode in (0, 1, 2)         # 2 = weighted front-surface splat [R32]
         self.Iprev = None
         self.tau_r = float(tau_r)
         self.t_last = np.full((num_envs, height, width), -np.inf, np.float32)
@@ -273,6 +290,7 @@ class Oracle:
             t_last = self.t_last.copy()
             Iprev = None if self.taps is None else self.Iprev.copy()
             btmp, bout = np.empty(P, np.float32), np.empty(P, np.float32)
+            waA, waB = np.zeros(2 * P, np.int64), np.zeros(2 * P, np.int64)
             holes.value = 0
             n = 0
             for e in range(E):
@@ -292,7 +310,8 @@ class Oracle:
                     -1 if self.taps is None else (self.taps.size - 1) // 2,
                     _f(self.taps) if self.taps is not None else None,
                     _f(A["I"][e]) if self.taps is not None else None, _f(cur["I"][e]) if self.taps is not None else None,
-                    _f(Iprev[e]) if self.taps is not None else None, float(self.eps), _f(btmp), _f(bout))
+                    _f(Iprev[e]) if self.taps is not None else None, float(self.eps), _f(btmp), _f(bout),
+                    _p(waA, C.c_int64), _p(waB, C.c_int64))
             if n <= cap:
                 break
             cap = int(n)

@@ -881,3 +881,104 @@ def test_p19d_defocus_softens_edges_and_a_static_scene_stays_silent():
     sharp = orc.log_luminance(kf["rad"], spec.log_eps)[0]
     soft = o.Lprev[0]
     assert np.abs(np.diff(soft, axis=1)).max() < np.abs(np.diff(sharp, axis=1)).max()
+
+
+# ------------------------------------------------------------------------------------------------
+# P20: weighted front-surface splat (reading R32; composite mode 2)
+# ------------------------------------------------------------------------------------------------
+def _brute_weighted(H, W, i, S, src_is_B, disp, Zsrc, Zoth, Lsrc):
+    """Gather form straight from the definition: per target, the sources covering it with positive bilinear weight,
+    the nearest depth Z*, the front set zt <= 1.01 Z*, the weighted mean of their log values -- in exact float64
+    (dyadic inputs).  Returns (mean [H,W] float64 with NaN where nothing lands, spread of L among the contributors)."""
+    f = i / S
+    wgt = (1 - f) if src_is_B else f
+    out = np.full((H, W), np.nan)
+    spread = np.zeros((H, W))
+    for ty in range(H):
+        for tx in range(W):
+            c = []
+            for sy in range(H):
+                for sx in range(W):
+                    dx, dy = float(disp[sy, sx, 0]), float(disp[sy, sx, 1])
+                    qx, qy = sx + wgt * dx, sy + wgt * dy
+                    if not (abs(qx - tx) < 1 and abs(qy - ty) < 1):
+                        continue
+                    jx, jy = math.floor(sx + dx + 0.5), math.floor(sy + dy + 0.5)
+                    zs = float(Zsrc[sy, sx])
+                    zo = float(Zoth[jy, jx]) if (0 <= jx < W and 0 <= jy < H) else zs
+                    za, zb = (zo, zs) if src_is_B else (zs, zo)
+                    c.append(((1 - f) * za + f * zb, (1 - abs(qx - tx)) * (1 - abs(qy - ty)), float(Lsrc[sy, sx])))
+            if c:
+                zmin = min(z for z, _, _ in c)
+                front = [(w_, l_) for z, w_, l_ in c if z <= float(np.float32(1.01)) * zmin]
+                out[ty, tx] = sum(w_ * l_ for w_, l_ in front) / sum(w_ for w_, _ in front)
+                spread[ty, tx] = max(l_ for _, l_ in front) - min(l_ for _, l_ in front)
+    return out, spread
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_p20_weighted_splat_is_the_front_surface_mean_8x8(seed):
+    """The oracle's integer sums (weights in units of 2^-20, at least one; log values in units of 2^-24) against the exact
+    float64 gather form: within the quantisation bound 2^-19 x (spread of the contributors' L) + 2^-23."""
+    H = W = 8
+    S = 4
+    r = _rng(200 + seed)
+    levels = np.array([1.0, 1.005, 1.5, 2.0, 3.0], np.float32)     # 1.0 / 1.005: inside the 1 % band; the rest outside
+    n_multi = 0
+    for src_is_B in (True, False):
+        disp = (r.integers(-12, 13, size=(H, W, 2)) / 4.0).astype(np.float32)
+        Zsrc = levels[r.integers(0, len(levels), size=(H, W))]
+        Zoth = Zsrc.copy()                                           # both ends alike: zt = the source's level, exactly
+        Lsrc = (r.integers(-40, 41, size=(H, W)) / 8.0).astype(np.float32)
+        for i in range(1, S + 1):
+            z = orc.splat(i, S, src_is_B, disp, Zsrc, Zoth)
+            acc = orc.wsplat(i, S, src_is_B, disp, Zsrc, Zoth, Lsrc, z)
+            want, spread = _brute_weighted(H, W, i, S, src_is_B, disp, Zsrc, Zoth, Lsrc)
+            hit = z != EMPTY
+            assert np.array_equal(hit, ~np.isnan(want)) and np.all(acc[..., 1][hit] > 0) and not acc[~hit].any()
+            got = acc[..., 0][hit] / acc[..., 1][hit] / 2.0 ** 24
+            assert np.all(np.abs(got - want[hit]) <= 2.0 ** -19 * spread[hit] + 2.0 ** -23), (seed, src_is_B, i)
+            n_multi += int((spread[hit] > 0).sum())
+    assert n_multi > 50                                             # the mean really mixes different values
+
+
+def test_p20b_weighted_splat_closed_forms():
+    """(a) Integer translation: every weight is 0 or 1, the weighted mode IS the winner-take-all mode, frames and events.
+    (b) A half-pixel shift of a fronto-parallel plane: every target is the mean of its two neighbours' log values.
+    (c) A near square over a far plane: the far sources under it are behind the front surface and carry no weight; a
+    source within 1 % of the front depth does."""
+    H, W, S = 12, 16, 4
+    r = _rng(31)
+    L0 = (r.integers(-24, 25, size=(H, W)) / 8.0).astype(np.float32)
+    depth = np.full((H, W), 4.0, np.float32)
+    # (a)
+    mv = np.zeros((1, H, W, 2), np.float32); mv[..., 0] = -S * 1.0
+    big = r.uniform(-2, 2, size=(H + 64, W + 64)).astype(np.float32)
+    ys, xs = np.mgrid[0:H, 0:W]
+    tex = lambda px: big[ys + 32, xs - px + 32]
+    frames = {}
+    for mode in (0, 2):
+        o = orc.Oracle(1, H, W, S, 0.2, 0.2, 1e-3, 1 / 60, composite_mode=mode, debug=True)
+        o.step(_rad_from_L(tex(0))[None], mv, depth[None])
+        ev = o.step(_rad_from_L(tex(S))[None], mv, depth[None])
+        frames[mode] = (o.dbg["Lhat"].copy(), o.dbg["dir"].copy(), len(ev))
+    assert np.array_equal(frames[0][1], frames[2][1]) and frames[0][2] == frames[2][2] > 0
+    assert np.abs(frames[0][0].astype(np.float64) - frames[2][0]).max() <= 2.0 ** -24      # only the 2^-24 grid of L
+    # (b)
+    disp = np.zeros((H, W, 2), np.float32); disp[..., 0] = 2.0       # at i = 1 of S = 4 the shift is (1 - f) 2 = 1.5 px
+    z = orc.splat(1, S, True, disp, depth, depth)
+    acc = orc.wsplat(1, S, True, disp, depth, depth, L0, z)
+    got = acc[..., 0] / np.maximum(acc[..., 1], 1) / 2.0 ** 24
+    want = (L0[:, 1:-2].astype(np.float64) + L0[:, 2:-1]) / 2        # target x >= 3: sources x - 2 and x - 1, half a weight each
+    assert np.array_equal(acc[:, 3:, 1], np.full((H, W - 3), 2 ** 20))  # two half weights
+    assert np.abs(got[:, 3:] - want).max() < 2.0 ** -23
+    # (c)
+    Z = np.full((H, W), 8.0, np.float32); Z[4:8, 5:9] = 2.0; Z[4, 5] = 2.01                # 2.01 <= 1.01 * 2.0
+    disp = np.full((H, W, 2), 0.5, np.float32)                      # everything moves by (1 - f) 0.5: fractional weights
+    Lc = np.where(Z > 3, 5.0, -3.0).astype(np.float32); Lc[4, 5] = -1.0
+    z = orc.splat(2, S, True, disp, Z, Z)
+    acc = orc.wsplat(2, S, True, disp, Z, Z, Lc, z)
+    got = acc[..., 0] / np.maximum(acc[..., 1], 1) / 2.0 ** 24
+    inside = got[5:8, 6:9]                                           # fully under the square: only near sources count
+    assert np.all(inside < -0.9) and np.all(np.abs(got[9:, 10:] - 5.0) < 1e-6)
+    assert -3.0 < got[5, 6] < -2.0                                   # the 2.01-deep source (L = -1) is mixed in with the -3s
