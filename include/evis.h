@@ -45,7 +45,14 @@ typedef enum {
 /* One path: z-buffers in global memory (L2-resident chunks), any motion.  The per-tile shared-memory path of
  * round 1 (value 2) was measured 3-4x slower on every workload and retired: 2 is INVALID_ARG. */
 enum { EVIS_PATH_AUTO = 0, EVIS_PATH_GLOBAL = 1 };
-enum { EVIS_COMPOSITE_B_PRIMARY = 0, EVIS_COMPOSITE_BLEND = 1 };
+/* 0: Eq. 6 literally, the nearest source's value is copied; B primary, A fills B's holes (R14, R19).
+ * 1: nearest of the two directions, time-weighted blend where both see the same surface (R19).
+ * 2: weighted front-surface splat ("These target values are then bilinearly interpolated to integer
+ *    pixels ... a per-pixel z-buffer that retains only the nearest surface"; R32): per direction, a target takes the
+ *    bilinear-weighted mean of the log values of the sources that cover it and lie within 1 % of the z-buffer's depth;
+ *    B primary, A fills B's holes.  Integer sums (weights in units of 2^-20, log values in units of 2^-24): the result
+ *    does not depend on scheduling. */
+enum { EVIS_COMPOSITE_B_PRIMARY = 0, EVIS_COMPOSITE_BLEND = 1, EVIS_COMPOSITE_WEIGHTED = 2 };
 
 typedef struct {
     int32_t  num_envs, height, width;   /* E, H, W  (> 0; H, W <= 32767; E <= 65535)            */

@@ -20,7 +20,7 @@ EVIS_OK = 0
 EVIS_ERR_INVALID_ARG, EVIS_ERR_CUDA, EVIS_ERR_OOM = -1, -2, -3
 EVIS_ERR_OVERFLOW, EVIS_ERR_MOTION_BOUND, EVIS_ERR_BAD_STATE = -4, -5, -6
 PATH_AUTO, PATH_GLOBAL = 0, 1
-COMPOSITE_B_PRIMARY, COMPOSITE_BLEND = 0, 1
+COMPOSITE_B_PRIMARY, COMPOSITE_BLEND, COMPOSITE_WEIGHTED = 0, 1, 2
 
 EVENT_DTYPE = np.dtype([("x", "<u2"), ("y", "<u2"), ("env", "<u2"), ("p", "i1"), ("substep", "u1"),
                         ("t_off", "<f4"), ("kf", "<u4")])

@@ -86,6 +86,11 @@ struct evis_ctx {
     float *frames;                    // nreg regions of frames_elems floats
     size_t frames_elems;
 
+    // weighted front-surface splat (composite mode 2, R32): per region the front depth and the sums of one chunk
+    uint32_t *zfront;
+    long long *wacc;
+    size_t wchunk_elems;              // chunk_ne * chunk_ni * HW
+
     // time-sorted stream (evis_set_time_sorted): workspace of the segmented radix sort
     bool time_sorted;
     void *sort_ws;
@@ -228,6 +233,7 @@ void free_all(evis_ctx *ctx)
     cudaFree(ctx->counters); cudaFree(ctx->dbg.win); cudaFree(ctx->dbg.dir); cudaFree(ctx->dbg.l_hat);
     cudaFree(ctx->vox_v); cudaFree(ctx->vox_out); cudaFree(ctx->sort_ws);
     cudaFree(ctx->lin[0]); cudaFree(ctx->i_prev); cudaFree(ctx->frames);
+    cudaFree(ctx->zfront); cudaFree(ctx->wacc);
     for (int k = 0; k < 2; ++k) {
         cudaFree(ctx->st_rad[k]); cudaFree(ctx->st_mv[k]); cudaFree(ctx->st_fwd[k]); cudaFree(ctx->st_depth[k]);
         if (ctx->ev_up[k]) cudaEventDestroy(ctx->ev_up[k]);
@@ -291,7 +297,7 @@ int create_impl(evis_ctx *ctx)
     volatile float dt = c.keyframe_dt / (float)g.S;
     ctx->ep.c_pos = c.c_pos; ctx->ep.c_neg = c.c_neg; ctx->ep.dt = dt; ctx->ep.kf = 0;
 
-    ctx->nset = g.mode == 0 ? 1 : 2;
+    ctx->nset = g.mode == EVIS_COMPOSITE_BLEND ? 2 : 1;
     uint32_t tiles_x, tiles_y;
     {
         // chunk = envs x substeps whose z-buffers fit one region's budget.  Defaults (measured on B200, DESIGN.md
@@ -387,6 +393,11 @@ int create_impl(evis_ctx *ctx)
             CU(cudaEventCreateWithFlags(&ctx->ev_order[k], cudaEventDisableTiming));
         }
     }
+    if (g.mode == EVIS_COMPOSITE_WEIGHTED) {
+        ctx->wchunk_elems = (size_t)ctx->chunk_ne * ctx->chunk_ni * g.HW;
+        CU(dalloc(ctx, &ctx->zfront, ctx->wchunk_elems * ctx->nreg));
+        CU(dalloc(ctx, &ctx->wacc, 2 * ctx->wchunk_elems * ctx->nreg));
+    }
     if (c.debug_capture) {
         CU(dalloc(ctx, &ctx->dbg.win, P * g.S));
         CU(dalloc(ctx, &ctx->dbg.dir, P * g.S));
@@ -455,7 +466,8 @@ int evis_create(const evis_config *cfg, evis_ctx **out)
     if (!(cfg->c_pos > 0.0f) || !(cfg->c_neg > 0.0f) || !(cfg->log_eps > 0.0f) || !(cfg->keyframe_dt > 0.0f))
         return EVIS_ERR_INVALID_ARG;
     if (!(cfg->max_motion_px >= 0.0f)) return EVIS_ERR_INVALID_ARG;
-    if (cfg->composite_mode != EVIS_COMPOSITE_B_PRIMARY && cfg->composite_mode != EVIS_COMPOSITE_BLEND)
+    if (cfg->composite_mode != EVIS_COMPOSITE_B_PRIMARY && cfg->composite_mode != EVIS_COMPOSITE_BLEND &&
+        cfg->composite_mode != EVIS_COMPOSITE_WEIGHTED)
         return EVIS_ERR_INVALID_ARG;
     if (cfg->path != EVIS_PATH_AUTO && cfg->path != EVIS_PATH_GLOBAL) return EVIS_ERR_INVALID_ARG;
     if (cfg->event_capacity == 0 || cfg->event_capacity > 0x7FFFFFFFull) return EVIS_ERR_INVALID_ARG;
@@ -594,7 +606,16 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                     zc.tag = (uint32_t)--ctx->ztag[r];
                 }
                 { Span sp(ctx, cs, EVIS_STAGE_SPLAT, multi ? 0 : 1, !multi); CU(launch_global_splat(g, zc, A, B, ctx->h_tab, cs)); }
-                if (ctx->defocus) {
+                if (g.mode == EVIS_COMPOSITE_WEIGHTED) {
+                    // R32: front depth per target, the weighted sums of its front surface, then Eq. 4 on their quotient
+                    Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 3, !multi);
+                    FrameIO fio{};
+                    fio.wacc = ctx->wacc + 2 * (size_t)r * ctx->wchunk_elems;
+                    CU(launch_front_wsplat(g, zc, A, B, ctx->h_tab, ctx->zfront + (size_t)r * ctx->wchunk_elems,
+                                           ctx->wacc + 2 * (size_t)r * ctx->wchunk_elems, cnt + C_HOLES, ctx->dbg, cs));
+                    CU(launch_resolve_weighted(g, zc, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, th, rf, sink, cnt + C_HOLES,
+                                               ctx->dbg, fio, cs));
+                } else if (ctx->defocus) {
                     // two passes (R31): the warped LINEAR frames of the chunk, then blur + log + Eq. 4
                     Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 2, !multi);
                     FrameIO fio{ctx->frames + (size_t)r * ctx->frames_elems, ctx->taps, ctx->cfg.log_eps};
@@ -771,6 +792,7 @@ int evis_set_voxels(evis_ctx *ctx, const evis_voxel_config *cfg)
         ctx->device_bytes -= ctx->vox_cells * (sizeof(unsigned long long) + sizeof(float));
         cudaFree(ctx->vox_v); cudaFree(ctx->vox_out); cudaFree(ctx->sort_ws);
     cudaFree(ctx->lin[0]); cudaFree(ctx->i_prev); cudaFree(ctx->frames);
+    cudaFree(ctx->zfront); cudaFree(ctx->wacc);
         ctx->vox_v = nullptr; ctx->vox_out = nullptr;
     }
     ctx->vox_on = false;

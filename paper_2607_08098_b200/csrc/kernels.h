@@ -70,6 +70,7 @@ struct FrameIO {
     float *frames;
     BlurTaps taps;
     float eps;
+    const long long *wacc;       // weighted splat (R32): [ni_alloc][ne_alloc][HW][2] = (sum W L 2^24, sum W), else null
 };
 // first keyframe: l_ref = l_prev = log(G * I + eps)
 cudaError_t launch_blur_log(const float *I, int E, int H, int W, const BlurTaps &taps, float eps, float *l_ref, float *l_prev,
@@ -118,6 +119,13 @@ cudaError_t launch_resolve_frames(const Geom &g, const ZChunk &zc, const float *
 cudaError_t launch_resolve_blurred(const Geom &g, const ZChunk &zc, const SubstepTable &tab, float *l_ref, float *l_prev,
                                    const EventParams &ep, const Thresholds &th, const Refractory &rf, const EventSink &sink,
                                    unsigned long long *holes, const DebugOut &dbg, const FrameIO &fio, cudaStream_t st);
+// weighted front-surface splat (R32; composite mode 2): front depth per target + the weighted sums
+// (global_path.cu), then the event pass (resolve_defocus.cu)
+cudaError_t launch_front_wsplat(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B, const SubstepTable &tab,
+                                uint32_t *zfront, long long *wacc, unsigned long long *holes, const DebugOut &dbg, cudaStream_t st);
+cudaError_t launch_resolve_weighted(const Geom &g, const ZChunk &zc, const SubstepTable &tab, float *l_ref, float *l_prev,
+                                    const EventParams &ep, const Thresholds &th, const Refractory &rf, const EventSink &sink,
+                                    unsigned long long *holes, const DebugOut &dbg, const FrameIO &fio, cudaStream_t st);
 // its four instantiation units (resolve_m*.cu): composite mode 0 / 1, without / with the debug capture
 #define EVIS_DECL_RESOLVE(name)                                                                                     \
     cudaError_t name(const Geom &g, const ZChunk &zc, const Keyframe &A, const Keyframe &B, const SubstepTable &tab,  \

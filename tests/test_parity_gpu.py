@@ -704,11 +704,11 @@ def test_refractory_api_contract():
 
 
 
-def _run_stream(spec, n_kf, path, seed_offset=0):
+def _run_stream(spec, n_kf, path, seed_offset=0, mode=0):
     sc = scenes.make_scene(spec)
     ev = binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg,
                       spec.log_eps, spec.keyframe_dt, max_motion_px=spec.max_motion_px(), path=path,
-                      event_capacity=1 << 24)
+                      composite_mode=mode, event_capacity=1 << 24)
     outs = []
     for k in range(n_kf):
         kf = scenes.render_keyframe(sc, k, device="cuda")
@@ -1096,3 +1096,34 @@ def test_time_sorted_stream(cfg, E, tau_r):
             assert np.array_equal(b[f][iso].astype(np.int64), o[f][iso].astype(np.int64)), f
     assert total > 2000
     plain.destroy(); srt.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# weighted front-surface splat (reading R32; composite mode 2)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,kw", [(1, {}), (2, {}), (4, {}), (3, {}), (4, {"margin": 5}), (1, {"tau_r": 1e-3}),
+                                    (2, {"use_fwd": False})])
+def test_weighted_splat_matches_the_oracle(cfg, kw):
+    """Composite mode 2: nearest sources and holes bit-exact, the weighted frame bit-exact too (integer sums on both
+    sides, one binary64 division), events exact; occluding rectangles (cfg 2 / 4), the rotating disk (cfg 3), the margin
+    crop, the direct mode, and the paper's -m_A forward field."""
+    spec = scenes.small(scenes.config(cfg), num_envs=2 if cfg != 1 else 1, height=83, width=117, num_keyframes=4)
+    rep = parity.run_parity(spec, 4, mode=binding.COMPOSITE_WEIGHTED, **kw)
+    _assert_tolerances(rep)
+    assert rep.max_dL == 0.0 and rep.ties == 0 and rep.events_oracle > 500
+
+
+@pytest.mark.gpu
+def test_weighted_splat_noise_stress_and_determinism():
+    """Hashed per-pixel motion with depth ties (every footprint class, many sources per target, holes) in mode 2, twice:
+    equal to the oracle and byte-identical between the runs (integer atomics)."""
+    spec = scenes.SceneSpec("noise", 2, 75, 131, 3, 1.0 / 60.0, 5, 0.3, 0.2, kind="noise", num_rects=0, v_max=480.0, seed=33)
+    rep = parity.run_parity(spec, 3, mode=binding.COMPOSITE_WEIGHTED)
+    _assert_tolerances(rep)
+    assert rep.max_dL == 0.0 and rep.holes > 0
+    a, _ = _run_stream(spec, 3, binding.PATH_GLOBAL, mode=binding.COMPOSITE_WEIGHTED)
+    b, _ = _run_stream(spec, 3, binding.PATH_GLOBAL, mode=binding.COMPOSITE_WEIGHTED)
+    assert sum(len(x) for x in a) > 100
+    for x, y in zip(a, b):
+        assert x.tobytes() == y.tobytes()
