@@ -70,6 +70,9 @@ def parse_args():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank its own batch of the config's shape (default); strong = ONE batch of the "
                          "config's shape, rank r takes the envs sharding.env_block(r, N, E) (sharding.ShardedEvis)")
+    ap.add_argument("--composite-mode", type=int, default=0, choices=[0, 1, 2],
+                    help="0 = B primary / A fills (the paper's, headline); 1 = blend; 2 = weighted front-surface splat: variants")
+    ap.add_argument("--time-sorted", action="store_true", help="sort the stored stream by (env, t) on the device: a variant")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
@@ -248,9 +251,12 @@ def run_ours(args, spec) -> None:
     cap = int(min(0x7FFFFFFF, max(1 << 22, 10 * E * H * W)))          # events stored per step
     def mk():
         e = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
-                         max_motion_px=spec.max_motion_px(), path=path, device=local, event_capacity=cap)
+                         max_motion_px=spec.max_motion_px(), path=path, device=local, event_capacity=cap,
+                         composite_mode=args.composite_mode)
         if args.defocus is not None:
             e.set_defocus(args.defocus)
+        if args.time_sorted:
+            e.set_time_sorted(True)
         return e
     ev = mk()
     stream = torch.cuda.current_stream(dev)
@@ -348,7 +354,9 @@ def run_ours(args, spec) -> None:
     out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": K, "warmup": Wm,
            "ms_per_step": ms / K, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic",
-           "config": dict(workload_config(spec, path_used), **({"defocus_sigma": args.defocus} if args.defocus is not None else {})),
+           "config": dict(workload_config(spec, path_used), **({"defocus_sigma": args.defocus} if args.defocus is not None else {}),
+                          **({"composite_mode": args.composite_mode} if args.composite_mode else {}),
+                          **({"time_sorted": True} if args.time_sorted else {})),
            "events_per_s": events / (ms * 1e-3), "events_per_step": ev_per_step,
            "x_realtime": spec.keyframe_dt / (ms / K * 1e-3),
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
