@@ -21,8 +21,9 @@ struct evis_ctx {
     cudaStream_t last_stream;
     int last_cuda;
 
-    Keyframe kf[2];
-    int cur;                          // kf[cur] receives the next keyframe; kf[cur^1] is A
+    Keyframe kf[3];                   // three, so that the prep of step k + 1 can overwrite the oldest while the chunk
+                                      // kernels of step k still read the other two
+    int cur;                          // kf[cur] receives the next keyframe; kf[(cur + 2) % 3] is A
     float *l_ref, *l_prev;
     float *th_on, *th_off;            // Eq. 8 maps [E*H*W] (owned), in force when th_active
     bool th_active;
@@ -81,7 +82,7 @@ struct evis_ctx {
     // alternate like kf[].L), the carried unblurred frame and the warped linear frames of one chunk per region
     bool defocus;
     BlurTaps taps;
-    float *lin[2];
+    float *lin[3];
     float *i_prev;
     float *frames;                    // nreg regions of frames_elems floats
     size_t frames_elems;
@@ -224,7 +225,7 @@ size_t env_size_mb(const char *name, size_t dflt)
 
 void free_all(evis_ctx *ctx)
 {
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < 3; ++k) {
         if (k == 0) cudaFree(ctx->kf[k].L);
         cudaFree(ctx->kf[k].mv); cudaFree(ctx->kf[k].fwd); cudaFree(ctx->kf[k].Z);
     }
@@ -274,10 +275,11 @@ int create_impl(evis_ctx *ctx)
     if (P >= ((size_t)1 << 31)) return EVIS_ERR_INVALID_ARG;    // the kernels keep pixel offsets between planes in 32 bits
 
     CU(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
-    // the two L planes share one allocation: the resolve kernel addresses the winner's value from one base
-    CU(dalloc(ctx, &ctx->kf[0].L, 2 * P));
+    // the L planes share one allocation: the resolve kernel addresses the winner's value from one base
+    CU(dalloc(ctx, &ctx->kf[0].L, 3 * P));
     ctx->kf[1].L = ctx->kf[0].L + P;
-    for (int k = 0; k < 2; ++k) {
+    ctx->kf[2].L = ctx->kf[0].L + 2 * P;
+    for (int k = 0; k < 3; ++k) {
         CU(dalloc(ctx, &ctx->kf[k].mv, P));
         CU(dalloc(ctx, &ctx->kf[k].Z, P));
     }
@@ -505,10 +507,11 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     const Geom &g = ctx->g;
     const size_t P = (size_t)g.E * g.HW;
     Keyframe &B = ctx->kf[ctx->cur];
-    const Keyframe &A = ctx->kf[ctx->cur ^ 1];
+    const int ia = (ctx->cur + 2) % 3;
+    const Keyframe &A = ctx->kf[ia];
 
     if (mv_fwd && !B.fwd) {               // forward fields are optional: allocate on first use
-        for (int k = 0; k < 2; ++k) CU(dalloc(ctx, &ctx->kf[k].fwd, P));
+        for (int k = 0; k < 3; ++k) CU(dalloc(ctx, &ctx->kf[k].fwd, P));
     }
     B.has_fwd = mv_fwd != nullptr;
     const bool first = ctx->steps == 0;
@@ -529,7 +532,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     if (first) {
         ctx->h_counters[C_EVENTS] = ctx->h_counters[C_HOLES] = ctx->h_counters[C_ALLOC] = 0;
         ctx->steps = 1;
-        ctx->cur ^= 1;
+        ctx->cur = (ctx->cur + 1) % 3;
         ctx->have_events = true;
         if (n_events) { CU(cudaStreamSynchronize(st)); *n_events = 0; }
         return EVIS_OK;
@@ -564,9 +567,14 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         CU(cudaMemsetAsync(sink.directory, 0, (size_t)ctx->dir_entries * sizeof(uint2), st));
     }
 
+    // The regions' streams do NOT join `st` again (unless the stage timers are on or EVIS_NO_OVERLAP=1): the order stream
+    // waits for them instead, and every call that returns results waits for the order stream.  `st` is then free to run
+    // the NEXT step's prep (HBM-bound, into the third keyframe buffer) under this step's chunk kernels; it cannot run
+    // further ahead than that, because a step's clears wait for the order stage of two steps before (ev_order).
+    const bool join_st = !ctx->overlap || ctx->prof_on;
     {
-        // nreg > 1: the env chunks are dealt round-robin to the regions' streams, which fork from `st` here and
-        // join it after the loop; the substep chunks of one env chunk stay on one stream (L_ref / L_prev carry)
+        // nreg > 1: the env chunks are dealt round-robin to the regions' streams, which fork from `st` here; the
+        // substep chunks of one env chunk stay on one stream (L_ref / L_prev carry)
         const bool multi = ctx->nreg > 1;
         const int nchunks_e = (g.E + ctx->chunk_ne - 1) / ctx->chunk_ne, nchunks_i = (g.S + ctx->chunk_ni - 1) / ctx->chunk_ni;
         Span sp_all(ctx, st, EVIS_STAGE_WARP, multi ? 2 * nchunks_e * nchunks_i : 0, multi);
@@ -619,7 +627,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
                     // two passes (R31): the warped LINEAR frames of the chunk, then blur + log + Eq. 4
                     Span sp(ctx, cs, EVIS_STAGE_RESOLVE, multi ? 0 : 2, !multi);
                     FrameIO fio{ctx->frames + (size_t)r * ctx->frames_elems, ctx->taps, ctx->cfg.log_eps};
-                    CU(launch_resolve_frames(g, zc, ctx->lin[ctx->cur ^ 1], ctx->lin[ctx->cur], ctx->h_tab, ctx->i_prev, ctx->ep,
+                    CU(launch_resolve_frames(g, zc, ctx->lin[ia], ctx->lin[ctx->cur], ctx->h_tab, ctx->i_prev, ctx->ep,
                                              cnt + C_HOLES, ctx->dbg, fio, cs));
                     CU(launch_resolve_blurred(g, zc, ctx->h_tab, ctx->l_ref, ctx->l_prev, ctx->ep, th, rf, sink, cnt + C_HOLES,
                                               ctx->dbg, fio, cs));
@@ -633,13 +641,15 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         if (multi)
             for (int r = 0; r < ctx->nreg; ++r) {
                 CU(cudaEventRecord(ctx->ev_join[r], ctx->reg_stream[r]));
-                CU(cudaStreamWaitEvent(st, ctx->ev_join[r], 0));
+                if (join_st) CU(cudaStreamWaitEvent(st, ctx->ev_join[r], 0));
             }
     }
     // a8, second half, on the order stream: it starts when this step's chunks are done and overlaps the next step
     cudaStream_t os = ctx->ord_stream;
     CU(cudaEventRecord(ctx->ev_chunks[sl], st));
     CU(cudaStreamWaitEvent(os, ctx->ev_chunks[sl], 0));
+    if (ctx->nreg > 1 && !join_st)
+        for (int r = 0; r < ctx->nreg; ++r) CU(cudaStreamWaitEvent(os, ctx->ev_join[r], 0));
     if (ctx->copy_pending) CU(cudaStreamWaitEvent(os, ctx->ev_copy, 0));   // `ordered` is still being copied out
     VoxelSink vs{};
     vs.store_events = 1;
@@ -686,7 +696,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     ctx->last_slot = sl;
     ctx->steps += 1;
     ctx->kf_next += 1;
-    ctx->cur ^= 1;
+    ctx->cur = (ctx->cur + 1) % 3;
     ctx->have_events = true;
     if (n_events) {
         const int rc = fetch_counters(ctx);
@@ -790,9 +800,7 @@ int evis_set_voxels(evis_ctx *ctx, const evis_voxel_config *cfg)
     if (ctx->copy_pending) { CU(cudaStreamSynchronize(ctx->copy_stream)); ctx->copy_pending = false; }
     if (ctx->vox_v) {
         ctx->device_bytes -= ctx->vox_cells * (sizeof(unsigned long long) + sizeof(float));
-        cudaFree(ctx->vox_v); cudaFree(ctx->vox_out); cudaFree(ctx->sort_ws);
-    cudaFree(ctx->lin[0]); cudaFree(ctx->i_prev); cudaFree(ctx->frames);
-    cudaFree(ctx->zfront); cudaFree(ctx->wacc);
+        cudaFree(ctx->vox_v); cudaFree(ctx->vox_out);          // the grid's two buffers, nothing else
         ctx->vox_v = nullptr; ctx->vox_out = nullptr;
     }
     ctx->vox_on = false;
@@ -893,8 +901,9 @@ int evis_set_defocus(evis_ctx *ctx, float sigma)
     for (int k = -R; k <= R; ++k) ctx->taps.w[k + R] = (float)((R ? exp(-(double)(k * k) / (2.0 * sg * sg)) : 1.0) / sum);
     if (!ctx->lin[0]) {
         const size_t P = (size_t)ctx->g.E * ctx->g.HW;
-        CU(dalloc(ctx, &ctx->lin[0], 2 * P));
+        CU(dalloc(ctx, &ctx->lin[0], 3 * P));
         ctx->lin[1] = ctx->lin[0] + P;
+        ctx->lin[2] = ctx->lin[0] + 2 * P;
         CU(dalloc(ctx, &ctx->i_prev, P));
         ctx->frames_elems = (size_t)ctx->chunk_ne * ctx->chunk_ni * ctx->g.HW;
         CU(dalloc(ctx, &ctx->frames, ctx->frames_elems * ctx->nreg));

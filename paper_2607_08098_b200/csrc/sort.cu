@@ -11,7 +11,8 @@
 // A segment is cut into tiles of SORT_TILE events, one block each (a block never spans two segments):
 //   k_seg_counts    events per environment from the directory (its entries are env-major)
 //   k_seg_scan      segment starts in the stream and first block of every segment (one block)
-// and per pass (the blocks hold other events after every pass, so their histograms are taken again):
+// and per pass (the blocks hold other events after every pass, so their histograms are taken again; counting the next
+// pass's digit per destination block with global atomics inside the scatter was measured slower than the extra read):
 //   k_sort_hist     per block: histogram of the pass's digit
 //   k_sort_scan     per segment: where each block's run of each digit goes (digit-major, block-minor: stable)
 //   k_sort_scatter  stable rank of every event inside its block's digit run, then the move
@@ -115,46 +116,56 @@ k_sort_scan(const uint32_t *__restrict__ seg_block, uint32_t *__restrict__ hist)
     }
 }
 
-// one pass: stable scatter of the block's events by the pass's digit
+// One pass: stable scatter of the block's events by the pass's digit.  Warp w owns the tile's events
+// [w * 512, (w + 1) * 512) and ranks them round by round (32 consecutive events per round) against its own row of digit
+// counters -- __match_any_sync groups the lanes of a round by digit --, keeping events and ranks in registers; one block
+// barrier later the rows are turned into the start of every (warp, digit) run inside the block's run of that digit, and
+// the events are moved.  Order inside a digit = (warp, round, lane) = the order in the tile: stable.
 __global__ void __launch_bounds__(SORT_NT)
 k_sort_scatter(const uint4 *__restrict__ src, uint4 *__restrict__ dst, const unsigned long long *__restrict__ seg_start,
                const uint32_t *__restrict__ seg_block, uint32_t E, const uint32_t *__restrict__ hist, int pass)
 {
-    constexpr int NW = SORT_NT / 32;
-    __shared__ uint32_t s_run[SORT_BINS];            // events of each digit placed by the earlier rounds
-    __shared__ uint32_t s_cnt[NW][SORT_BINS];        // this round: events of each digit per warp
+    constexpr int NW = SORT_NT / 32, PER_WARP = SORT_TILE / NW;
+    __shared__ uint32_t s_cnt[NW][SORT_BINS];
     uint32_t seg, n;
     unsigned long long first;
     if (!sort_block(seg_start, seg_block, E, blockIdx.x, seg, first, n)) return;
-    const uint32_t *off = hist + (size_t)blockIdx.x * SORT_BINS;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    s_run[threadIdx.x] = off[threadIdx.x];
     for (int w = 0; w < NW; ++w) s_cnt[w][threadIdx.x] = 0;
     __syncthreads();
-    const unsigned long long seg0 = seg_start[seg];
-    for (uint32_t r0 = 0; r0 < n; r0 += SORT_NT) {
-        const uint32_t i = r0 + threadIdx.x;
-        const bool have = i < n;
-        uint4 ev = make_uint4(0u, 0u, 0u, 0u);
-        if (have) ev = src[first + i];
-        const uint32_t digit = have ? (ev.z >> (8 * pass)) & 0xFFu : 0xFFFFFFFFu;
-        const unsigned peers = __match_any_sync(0xFFFFFFFFu, digit);
-        const uint32_t rank = __popc(peers & ((1u << lane) - 1u));
-        if (have && rank == 0) s_cnt[warp][digit] = __popc(peers);
-        __syncthreads();
-        if (have) {
-            uint32_t o = s_run[digit] + rank;
-            for (int w = 0; w < warp; ++w) o += s_cnt[w][digit];
-            dst[seg0 + o] = ev;
-        }
-        __syncthreads();
-        {
-            uint32_t add = 0;
+    uint4 ev[SORT_ROUNDS];
+    uint32_t rk[SORT_ROUNDS];                        // rank among the warp's events of the same digit | digit << 16
+    const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
-            for (int w = 0; w < NW; ++w) { add += s_cnt[w][threadIdx.x]; s_cnt[w][threadIdx.x] = 0; }
-            s_run[threadIdx.x] += add;
-        }
-        __syncthreads();
+    for (int r = 0; r < SORT_ROUNDS; ++r) {
+        const uint32_t i = (uint32_t)(warp * PER_WARP + r * 32 + lane);
+        ev[r] = i < n ? __ldcs(src + first + i) : make_uint4(0u, 0u, 0u, 0u);
+    }
+#pragma unroll
+    for (int r = 0; r < SORT_ROUNDS; ++r) {
+        const uint32_t i = (uint32_t)(warp * PER_WARP + r * 32 + lane);
+        const bool have = i < n;
+        const uint32_t digit = have ? (ev[r].z >> (8 * pass)) & 0xFFu : 0x100u;
+        const unsigned peers = __match_any_sync(0xFFFFFFFFu, digit);
+        uint32_t before = 0;
+        if (have) before = s_cnt[warp][digit];
+        __syncwarp();
+        if (have && (peers & lt) == 0u) s_cnt[warp][digit] = before + __popc(peers);
+        __syncwarp();
+        rk[r] = (before + __popc(peers & lt)) | (digit << 16);
+    }
+    __syncthreads();
+    {
+        uint32_t base = hist[(size_t)blockIdx.x * SORT_BINS + threadIdx.x];      // the block's run of digit threadIdx.x
+#pragma unroll
+        for (int w = 0; w < NW; ++w) { const uint32_t c = s_cnt[w][threadIdx.x]; s_cnt[w][threadIdx.x] = base; base += c; }
+    }
+    __syncthreads();
+    const unsigned long long seg0 = seg_start[seg];
+#pragma unroll
+    for (int r = 0; r < SORT_ROUNDS; ++r) {
+        const uint32_t digit = rk[r] >> 16;
+        if (digit < 0x100u) dst[seg0 + s_cnt[warp][digit] + (rk[r] & 0xFFFFu)] = ev[r];
     }
 }
 

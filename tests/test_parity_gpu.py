@@ -1127,3 +1127,38 @@ def test_weighted_splat_noise_stress_and_determinism():
     assert sum(len(x) for x in a) > 100
     for x, y in zip(a, b):
         assert x.tobytes() == y.tobytes()
+
+
+@pytest.mark.gpu
+def test_voxel_setter_leaves_the_other_features_alone():
+    """evis_set_voxels called again (other shape, off, on) must touch the grid's buffers only: with defocus, the
+    time-sorted stream and a weighted context alive, the events stay the oracle's."""
+    spec = scenes.small(scenes.config(2), num_envs=2, height=70, width=93, num_keyframes=3)
+    sc = scenes.make_scene(spec)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    args = (E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt)
+    for mode, sigma in ((0, 0.4), (binding.COMPOSITE_WEIGHTED, None)):
+        ev = binding.Evis(*args, composite_mode=mode, event_capacity=1 << 22)
+        ora = orc.Oracle(*args, composite_mode=mode, defocus_sigma=sigma)
+        if sigma is not None:
+            ev.set_defocus(sigma)
+        ev.set_time_sorted(True)
+        ev.set_voxels(2)
+        ev.set_voxels(3, window_steps=2)
+        ev.set_voxels(None)
+        ev.set_voxels(1)
+        for k in range(spec.num_keyframes):
+            kf = scenes.render_keyframe(sc, k, device="cuda")
+            n = ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+            h = {key: v.cpu().numpy() for key, v in kf.items()}
+            oe = ora.step(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"])
+            if k == 0:
+                continue
+            ge = ev.read_events()
+            assert n == len(ge) == len(oe) > 100
+            key = lambda e: np.stack([e["env"], e["substep"], e["y"], e["x"], e["p"]], 1).astype(np.int64)
+            a, b = key(ge), key(oe)
+            assert np.array_equal(a[np.lexsort(a.T[::-1])], b[np.lexsort(b.T[::-1])])
+            grid, _ = ev.read_voxels()
+            assert abs(float(grid.sum(dtype=np.float64)) - n) < 0.5
+        ev.destroy()
