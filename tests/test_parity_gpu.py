@@ -1162,3 +1162,51 @@ def test_voxel_setter_leaves_the_other_features_alone():
             grid, _ = ev.read_voxels()
             assert abs(float(grid.sum(dtype=np.float64)) - n) < 0.5
         ev.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# the asynchronous host entry point and the new features at multi-region size
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+def test_async_step_host_equals_the_device_path():
+    """evis_step_host with n_events = NULL (two staging sets, the upload of step k + 1 under the kernels of step k) gives
+    the events and the accumulation images of the device-resident path, step after step, also when the host buffers of
+    a call are overwritten right after the NEXT call returned (the contract of the asynchronous form)."""
+    spec = scenes.small(scenes.config(4), num_envs=6, height=120, width=160, num_keyframes=6)
+    sc = scenes.make_scene(spec)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    mk = lambda: binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                              max_motion_px=spec.max_motion_px(), event_capacity=1 << 23)
+    a, b = mk(), mk()
+    a.set_voxels(2); b.set_voxels(2)
+    host = [{k: torch.empty_like(v, device="cpu").pin_memory() for k, v in scenes.render_keyframe(sc, 0).items()} for _ in range(2)]
+    want_ev, want_vx, got_ev, got_vx = [], [], [], []
+    for k in range(spec.num_keyframes):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        a.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        h = host[k & 1]
+        for key in h:
+            h[key].copy_(kf[key])
+        b.step_host(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"], sync=False)
+        for key in host[(k & 1) ^ 1]:                 # the previous call's buffers are free now: scribble over them
+            host[(k & 1) ^ 1][key].fill_(float("nan"))
+        if k:
+            want_ev.append(a.read_events().copy()); want_vx.append(a.read_voxels()[0])
+            got_ev.append(b.read_events().copy()); got_vx.append(b.read_voxels()[0])
+    assert sum(len(x) for x in want_ev) > 5000
+    for x, y in zip(want_ev, got_ev):
+        assert x.tobytes() == y.tobytes()
+    for x, y in zip(want_vx, got_vx):
+        assert np.array_equal(x, y)
+    a.destroy(); b.destroy()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kw", [{"defocus": 0.5}, {"mode": 2}, {"mode": 2, "tau_r": 5e-4}])
+def test_new_features_on_concurrent_regions(kw):
+    """Defocus and the weighted splat with 9 envs at cfg 4's full 346x260 resolution: one env per chunk, four concurrent
+    regions and streams (the launch configuration the bench uses), the oracle on the first, a middle and the last env."""
+    spec = scenes.small(scenes.config(4), num_envs=9, num_keyframes=3)
+    rep = parity.run_parity(spec, 3, envs=[0, 4, 8], debug=False, capacity=1 << 24, **kw)
+    _assert_tolerances(rep)
+    assert rep.events_oracle > 10000
