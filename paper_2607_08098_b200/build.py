@@ -14,7 +14,7 @@ LIB = os.path.join(HERE, "libevis.so")
 SOURCES = ["api.cu", "prep.cu", "global_path.cu", "resolve_m0.cu", "resolve_m0d.cu", "resolve_m1.cu", "resolve_m1d.cu", "resolve_defocus.cu",
            "order.cu", "sort.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("EVIS_NVCC_EXTRA", "").split()   # experiment switches
 
 
 def _deps():
