@@ -41,6 +41,32 @@ RANGE_CAPTURE = os.path.join("profiles", "round2_a_range_cfg4.csv")
 RANGE_WORKLOAD, RANGE_STEPS = "cfg4_256env_346x260_S16_rl", 5
 
 
+def chunk_traffic(workload: str):
+    """DRAM bytes (read + write) of one env chunk = one k_splat_global + one k_resolve_global launch, from the committed
+    `ncu --set full` capture of the two kernels ALONE (profiles/round2_b_ncu_full_cfg4.csv: cold caches, serialised), or
+    None for another workload."""
+    if workload != RANGE_WORKLOAD:
+        return None
+    try:
+        import csv
+        tot = {"k_splat_global": [0.0, 0], "k_resolve_global": [0.0, 0]}
+        with open(os.path.join(ROOT, "profiles", "round2_b_ncu_full_cfg4.csv")) as f:
+            rows = list(csv.reader(f))
+        h = {name: i for i, name in enumerate(rows[0])}
+        for r in rows[2:]:
+            if not r[0].startswith("chunk kernels alone"):
+                continue
+            for k in tot:
+                if r[1].startswith(k):
+                    tot[k][0] += float(r[h["dram__bytes_read.sum"]]) * 1e6 + float(r[h["dram__bytes_write.sum"]])
+                    tot[k][1] += 1
+        if not all(v[1] for v in tot.values()):
+            return None
+        return sum(v[0] / v[1] for v in tot.values())
+    except (OSError, ValueError, KeyError, IndexError):
+        return None
+
+
 def range_capture(workload: str):
     """{metric: value per step} from the committed whole-step ncu capture when it describes `workload`, else None."""
     if workload != RANGE_WORKLOAD:
@@ -332,8 +358,12 @@ def run_ours(args, spec) -> None:
     cap_ = range_capture(spec.name)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": None, "traffic_note": "no DRAM-byte measurement of the concurrent schedule exists: ncu serialises the "
-                "streams (profiles/round2_README.md); the serialised capture's bytes are in `capture` below",
+                "traffic": chunk_traffic(spec.name),
+                "traffic_note": "DRAM bytes of ONE env chunk (one splat + one resolve launch) measured by `ncu --set full` on the "
+                "two kernels alone, cold caches, serialised (profiles/round2_b_ncu_full_cfg4.csv); its algorithmic share is "
+                "`algorithmic_bytes_per_chunk`.  In the bench's schedule the chunk's 23 MB of keys stay in the L2 between the "
+                "two launches; ncu cannot measure that schedule (it serialises the streams, profiles/round2_README.md)",
+                "algorithmic_bytes_per_chunk": algo_bytes_step / E,      # a chunk of this workload = one env; prep's and expand's share included
                 "algorithmic_bytes_per_step": algo_bytes_step, "basis": "whole step: algorithmic bytes / ms_per_step",
                 "dominant_stage_ms": stage_ms[dom], "dominant_stage_launches_per_step": max(1.0, prof["launches"][dom] / K),
                 "stage_ms_per_step": stage_ms, "stage_launches_per_step": {k: v / K for k, v in prof["launches"].items()}}
