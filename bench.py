@@ -404,9 +404,14 @@ def run_ours(args, spec) -> None:
         torch.cuda.empty_cache()
         h2d = int(E * H * W * 32)
 
-        def e2e_arm(voxels: bool):
+        def e2e_arm(voxels: bool, compact: bool = False):
             ev = mk()
-            if voxels:
+            if compact:
+                ev.set_compact_events(True)
+                hcap = int(min(cap, 2 * ev_per_step + (1 << 20)))
+                hbufs = [torch.empty(hcap, dtype=torch.int64).pin_memory() for _ in range(2)]
+                harrs = [hb.numpy().view(np.uint64) for hb in hbufs]
+            elif voxels:
                 ev.set_voxels(1, window_steps=1, keep_events=False)
                 nel = int(np.prod(ev.voxel_shape()))
                 hbufs = [torch.empty(nel, dtype=torch.float32).pin_memory() for _ in range(2)]
@@ -429,10 +434,10 @@ def run_ours(args, spec) -> None:
                     got += harrs[0].nbytes
                 else:
                     n_step = ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
-                    n_copy = ev.read_events_begin(harrs[k & 1])        # ends the previous copy first
+                    n_copy = (ev.read_events8_begin if compact else ev.read_events_begin)(harrs[k & 1])   # ends the previous copy first
                     if n_copy != n_step:
                         raise SystemExit("bench.py: e2e host buffer too small for a step's events")
-                    got += 16 * n_copy
+                    got += (8 if compact else 16) * n_copy
             if voxels:
                 ev.read_voxels_end()
             else:
@@ -453,6 +458,9 @@ def run_ours(args, spec) -> None:
                           "(evis_set_voxels bins=1, keep_events=0)",
                           api="evis_step_host (pinned host keyframes, upload overlapping the previous step) + "
                               "evis_read_voxels_begin / _end (pinned host image, overlapping the next upload)")
+        out["e2e_events8"] = dict(e2e_arm(False, compact=True), result="the full ordered event stream as 8-byte compact events "
+                                  "(evis_set_compact_events; stamps within T/S * 2^-16)",
+                                  api="evis_step_host + evis_read_events8_begin / evis_read_events_end")
         out["e2e_events"] = dict(e2e_arm(False), result="the full ordered event stream, 16 B per event",
                                  api="evis_step_host (pinned host keyframes) + evis_read_events_begin / _end (pinned host "
                                      "stream, overlapping the next upload)")

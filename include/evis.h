@@ -265,6 +265,19 @@ int evis_read_voxels_end(evis_ctx *ctx);
  * the stored events).  Needs the event stream (not a voxels-only context).  Synchronises.  Errors: INVALID_ARG, CUDA, OOM. */
 int evis_set_time_sorted(evis_ctx *ctx, int on);
 
+/* Compact events: with on != 0 the stored stream of every later step holds 8-byte events instead of 16-byte ones (half
+ * the bytes to copy out; the order, the counts and the overflow rules are those of evis_read_events):
+ *   bits  0-11 x | 12-23 y | 24-39 env | 40-47 substep i | 48-62 frac | 63 polarity (1 = ON, 0 = OFF)
+ * frac = min(32767, floor(fr 2^15)), fr in [0, 1] the position of the timestamp inside its substep (R8), so
+ *   t_off = (i - 1 + (frac + 0.5) / 32768) T / S   reproduces the 16-byte event's t_off within T / S * 2^-16
+ * (1.6e-8 s at 1 kHz substeps), and the interval index kf is the step's (every event of a step shares it).  The 16-byte
+ * read calls then return BAD_STATE; not together with the time-sorted stream.  Needs width, height <= 4096.
+ * Synchronises.  Errors: INVALID_ARG, BAD_STATE, CUDA. */
+typedef uint64_t evis_event8;
+int evis_set_compact_events(evis_ctx *ctx, int on);
+int evis_read_events8(evis_ctx *ctx, evis_event8 *dst, int dst_is_device, uint64_t max, uint64_t *n_out);
+int evis_read_events8_begin(evis_ctx *ctx, evis_event8 *host_dst, uint64_t max, uint64_t *n_out);   /* ends with evis_read_events_end */
+
 /* Copy the events of the last step, in the deterministic order
  * (env, substep, tile row, tile column, y, x, crossing k), to `dst` (room for `max` events;
  * device pointer if dst_is_device != 0, else host).  Synchronises.  *n_out = events copied

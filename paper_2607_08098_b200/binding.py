@@ -55,7 +55,7 @@ class evis_profile(C.Structure):
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
            "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end",
-           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus", "evis_set_time_sorted"]
+           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus", "evis_set_time_sorted", "evis_set_compact_events", "evis_read_events8", "evis_read_events8_begin"]
 
 _lib = None
 
@@ -100,6 +100,9 @@ def load() -> C.CDLL:
     L.evis_read_voxels_end.argtypes = [vp]
     L.evis_set_defocus.argtypes = [vp, C.c_float]
     L.evis_set_time_sorted.argtypes = [vp, C.c_int]
+    L.evis_set_compact_events.argtypes = [vp, C.c_int]
+    L.evis_read_events8.argtypes = [vp, vp, C.c_int, C.c_uint64, u64p]
+    L.evis_read_events8_begin.argtypes = [vp, vp, C.c_uint64, u64p]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
     for name in SYMBOLS:
@@ -242,6 +245,26 @@ class Evis:
         """evis_set_time_sorted: the stored stream of later steps is ordered by (env, t_off), stable."""
         _check(self._lib.evis_set_time_sorted(self._ctx, int(bool(on))), "evis_set_time_sorted")
 
+    def set_compact_events(self, on: bool = True) -> None:
+        """evis_set_compact_events: the stored stream holds 8-byte events (read them with read_events8)."""
+        _check(self._lib.evis_set_compact_events(self._ctx, int(bool(on))), "evis_set_compact_events")
+
+    def read_events8(self, max_events: Optional[int] = None, allow=()) -> np.ndarray:
+        """evis_read_events8 to a new host array of uint64 (decode with ``decode_events8``)."""
+        n = min(int(self.info().last_events), int(self.cfg.event_capacity))
+        if max_events is not None:
+            n = min(n, int(max_events))
+        out = np.empty(n, np.uint64)
+        got = C.c_uint64(0)
+        _check(self._lib.evis_read_events8(self._ctx, out.ctypes.data if n else None, 0, n, C.byref(got)), "evis_read_events8", allow)
+        return out[:got.value]
+
+    def read_events8_begin(self, host_buf: np.ndarray) -> int:
+        assert host_buf.dtype == np.uint64 and host_buf.flags.c_contiguous
+        got = C.c_uint64(0)
+        _check(self._lib.evis_read_events8_begin(self._ctx, host_buf.ctypes.data, host_buf.size, C.byref(got)), "evis_read_events8_begin")
+        return int(got.value)
+
     def set_defocus(self, sigma: float) -> None:
         """evis_set_defocus: Gaussian blur of the warped linear frame before the event model."""
         _check(self._lib.evis_set_defocus(self._ctx, float(sigma)), "evis_set_defocus")
@@ -372,3 +395,20 @@ class Evis:
             self.destroy()
         except Exception:
             pass
+
+
+def decode_events8(ev8: np.ndarray, keyframe_dt: float, substeps: int, kf: int = 0) -> np.ndarray:
+    """8-byte events (include/evis.h, evis_event8) -> the 16-byte record layout (EVENT_DTYPE); t_off is the centre of the
+    stamp's 2^-15 cell of its substep."""
+    ev8 = np.asarray(ev8, np.uint64)
+    out = np.zeros(len(ev8), EVENT_DTYPE)
+    out["x"] = (ev8 & np.uint64(0xFFF)).astype(np.uint16)
+    out["y"] = ((ev8 >> np.uint64(12)) & np.uint64(0xFFF)).astype(np.uint16)
+    out["env"] = ((ev8 >> np.uint64(24)) & np.uint64(0xFFFF)).astype(np.uint16)
+    sub = ((ev8 >> np.uint64(40)) & np.uint64(0xFF)).astype(np.int64)
+    out["substep"] = sub.astype(np.uint8)
+    frac = ((ev8 >> np.uint64(48)) & np.uint64(0x7FFF)).astype(np.float64)
+    out["p"] = np.where((ev8 >> np.uint64(63)) != 0, 1, -1).astype(np.int8)
+    out["t_off"] = ((sub - 1) + (frac + 0.5) / 32768.0) * (keyframe_dt / substeps)
+    out["kf"] = kf
+    return out

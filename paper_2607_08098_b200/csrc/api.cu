@@ -92,6 +92,8 @@ struct evis_ctx {
     long long *wacc;
     size_t wchunk_elems;              // chunk_ne * chunk_ni * HW
 
+    bool compact;                     // evis_set_compact_events: the stored stream holds 8-byte events
+
     // time-sorted stream (evis_set_time_sorted): workspace of the segmented radix sort
     bool time_sorted;
     void *sort_ws;
@@ -652,7 +654,8 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         for (int r = 0; r < ctx->nreg; ++r) CU(cudaStreamWaitEvent(os, ctx->ev_join[r], 0));
     if (ctx->copy_pending) CU(cudaStreamWaitEvent(os, ctx->ev_copy, 0));   // `ordered` is still being copied out
     VoxelSink vs{};
-    vs.store_events = 1;
+    vs.store_events = ctx->compact ? 2 : 1;
+    vs.dt = ctx->ep.dt;
     if (ctx->vox_on) {
         if (ctx->vox_restart || ctx->vox_j >= (uint32_t)ctx->vox.window_steps) {     // a new window starts with this interval
             CU(cudaMemsetAsync(ctx->vox_v, 0, ctx->vox_cells * sizeof(unsigned long long), os));
@@ -665,7 +668,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         vs.bins = (uint32_t)ctx->vox.bins;
         vs.hc = (uint32_t)(g.H - 2 * g.margin); vs.wc = (uint32_t)(g.W - 2 * g.margin);
         vs.t_base = tb; vs.scale = sc;
-        vs.store_events = ctx->vox.keep_events != 0;
+        if (!ctx->vox.keep_events) vs.store_events = 0;
         ctx->vox_j += 1;
     }
     {
@@ -680,7 +683,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
             CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
                             cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, vs, os));
         }
-        if (ctx->time_sorted && vs.store_events) {
+        if (ctx->time_sorted && vs.store_events == 1) {
             // the arrival buffer of this slot is free once the stream has been laid out: it is the sort's scratch
             CU(launch_time_sort(sink.directory, ctx->dir_entries, rf.t_last ? 0 : DIR_EV_SHIFT, (uint32_t)g.E,
                                 ctx->cfg.event_capacity < ctx->arrival_cap ? ctx->cfg.event_capacity : ctx->arrival_cap,
@@ -868,9 +871,57 @@ int evis_read_voxels_begin(evis_ctx *ctx, float *host_dst, int normalize, int re
 
 int evis_read_voxels_end(evis_ctx *ctx) { return evis_read_events_end(ctx); }
 
+int evis_set_compact_events(evis_ctx *ctx, int on)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    if (on && (ctx->g.W > 4096 || ctx->g.H > 4096)) return EVIS_ERR_INVALID_ARG;     // 12 bits per coordinate
+    if (on && ctx->time_sorted) return EVIS_ERR_BAD_STATE;                            // the sort moves 16-byte events
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (ctx->steps) CU(sync_all(ctx));
+    if (ctx->copy_pending) { CU(cudaStreamSynchronize(ctx->copy_stream)); ctx->copy_pending = false; }
+    ctx->compact = on != 0;
+    ctx->have_events = false;                     // the stored stream of the last step has the other format
+    return EVIS_OK;
+}
+
+// the 8-byte twin of evis_read_events / _begin: same order, same counts, half the bytes
+static int read_events8(evis_ctx *ctx, uint64_t *dst, int dst_is_device, uint64_t max, uint64_t *n_out, bool async)
+{
+    if (!ctx || (!dst && max > 0)) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->have_events || !ctx->compact || (ctx->vox_on && !ctx->vox.keep_events)) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    const int rc = fetch_counters(ctx);
+    if (rc != EVIS_OK) return rc;
+    if (ctx->copy_pending) { CU(cudaStreamSynchronize(ctx->copy_stream)); ctx->copy_pending = false; }
+    uint64_t n = stored_events(ctx);
+    if (n > max) n = max;
+    if (n && !async)
+        CU(cudaMemcpy(dst, ctx->ordered, n * sizeof(uint64_t), dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    if (n && async) {
+        CU(cudaMemcpyAsync(dst, ctx->ordered, n * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->copy_stream));
+        CU(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
+        ctx->copy_pending = true;
+    }
+    if (n_out) *n_out = n;
+    return ctx->last_overflow ? EVIS_ERR_OVERFLOW : EVIS_OK;
+}
+
+int evis_read_events8(evis_ctx *ctx, uint64_t *dst, int dst_is_device, uint64_t max, uint64_t *n_out)
+{
+    return read_events8(ctx, dst, dst_is_device, max, n_out, false);
+}
+
+int evis_read_events8_begin(evis_ctx *ctx, uint64_t *host_dst, uint64_t max, uint64_t *n_out)
+{
+    return read_events8(ctx, host_dst, 0, max, n_out, true);
+}
+
 int evis_set_time_sorted(evis_ctx *ctx, int on)
 {
     if (!ctx) return EVIS_ERR_INVALID_ARG;
+    if (on && ctx->compact) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     if (ctx->steps) CU(sync_all(ctx));
@@ -1001,7 +1052,7 @@ int evis_step_host(evis_ctx *ctx, const float *rad, const float *mv_bwd, const f
 int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t max, uint64_t *n_out)
 {
     if (!ctx || (!dst && max > 0)) return EVIS_ERR_INVALID_ARG;
-    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events)) return EVIS_ERR_BAD_STATE;
+    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events) || ctx->compact) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     const int rc = fetch_counters(ctx);
@@ -1017,7 +1068,7 @@ int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t
 int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, uint64_t *n_out)
 {
     if (!ctx || (!host_dst && max > 0)) return EVIS_ERR_INVALID_ARG;
-    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events)) return EVIS_ERR_BAD_STATE;
+    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events) || ctx->compact) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     if (!guard.ok) return EVIS_ERR_CUDA;
     const int rc = fetch_counters(ctx);
@@ -1047,7 +1098,7 @@ int evis_read_events_end(evis_ctx *ctx)
 int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_stored)
 {
     if (!ctx || !dev_ptr || !n_stored) return EVIS_ERR_INVALID_ARG;
-    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events)) return EVIS_ERR_BAD_STATE;
+    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events) || ctx->compact) return EVIS_ERR_BAD_STATE;
     DeviceGuard guard(ctx->cfg.device);
     const int rc = fetch_counters(ctx);
     if (rc != EVIS_OK) return rc;

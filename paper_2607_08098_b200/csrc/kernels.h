@@ -148,7 +148,9 @@ struct VoxelSink {
     uint32_t bins, hc, wc;
     float t_base;               // start of this interval relative to the start of the window (j * T)
     float scale;                // (bins - 1) / (window_steps * T)
-    int store_events;           // 0: the ordered stream is not written (voxels only)
+    int store_events;           // 0: the ordered stream is not written (voxels only); 1: 16-byte events; 2: 8-byte
+                                // compact events (evis_event8, include/evis.h) at the same positions of the same buffer
+    float dt;                   // T / S (compact events: the stamp is stored as a fraction of the substep)
 };
 // V -> float32 (out, same shape); normalize: every (env, channel, bin) plane divided by its maximum
 cudaError_t launch_voxel_finish(const unsigned long long *v, float *out, uint32_t planes, uint32_t cells, int normalize,

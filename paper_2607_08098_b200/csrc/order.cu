@@ -57,6 +57,17 @@ __device__ __forceinline__ void voxel_add(const VoxelSink &vox, uint32_t xy, uin
     if (q && b0 + 1u < vox.bins) atomicAdd(vox.v + cell + plane, q);
 }
 
+// The 8-byte event of include/evis.h (evis_event8): x | y << 12 | env << 24 | substep << 40 | frac << 48 | ON << 63, frac =
+// min(32767, floor(fr 2^15)) with fr in [0, 1] the stamp's position inside its substep.
+__device__ __forceinline__ unsigned long long pack_event8(uint32_t xy, uint32_t w1, float fr)
+{
+    const uint32_t frac = min(32767u, (uint32_t)__float2uint_rd(__fmul_rn(fminf(fmaxf(fr, 0.0f), 1.0f), 32768.0f)));
+    const unsigned long long on = ((w1 >> 16) & 0xFFu) == 0x01u ? 1ull : 0ull;
+    return (unsigned long long)(xy & 0xFFFu) | ((unsigned long long)((xy >> 16) & 0xFFFu) << 12) |
+           ((unsigned long long)(w1 & 0xFFFFu) << 24) | ((unsigned long long)(w1 >> 24) << 40) |
+           ((unsigned long long)frac << 48) | (on << 63);
+}
+
 // shift: 0 = the entry's .y is an event count (direct mode: the chunk holds events), DIR_EV_SHIFT = records | events << shift
 __global__ void __launch_bounds__(ORD_NT)
 k_dir_blocksum(const uint2 *__restrict__ dir, uint32_t n, unsigned long long *__restrict__ bsum, int shift)
@@ -144,7 +155,13 @@ k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *
 #pragma unroll
         for (int u = 0; u < U; ++u)
             if (ok[u]) {
-                if (vox.store_events) ordered[out0 + o0 + u * ORD_NT] = val[u];
+                if (vox.store_events == 1) ordered[out0 + o0 + u * ORD_NT] = val[u];
+                else if (vox.store_events == 2) {
+                    // direct mode stamps in seconds: back to the fraction of the substep
+                    const float t0 = __fmul_rn((float)((val[u].y >> 24) - 1u), vox.dt);
+                    reinterpret_cast<unsigned long long *>(ordered)[out0 + o0 + u * ORD_NT] =
+                        pack_event8(val[u].x, val[u].y, __fdividef(__fsub_rn(__uint_as_float(val[u].z), t0), vox.dt));
+                }
                 if (vox.v) voxel_add(vox, val[u].x, val[u].y, __uint_as_float(val[u].z));
             }
     }
@@ -260,7 +277,8 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
                 const unsigned long long o = first + e;
                 if (e < total_ev && o < cap) {
                     const float t_off = __fmaf_rn(fr, ep.dt, t0);
-                    if (vox.store_events) ordered[o] = make_uint4(o_xy, o_w1, __float_as_uint(t_off), ep.kf);
+                    if (vox.store_events == 1) ordered[o] = make_uint4(o_xy, o_w1, __float_as_uint(t_off), ep.kf);
+                    else if (vox.store_events == 2) reinterpret_cast<unsigned long long *>(ordered)[o] = pack_event8(o_xy, o_w1, fr);
                     if (vox.v) voxel_add(vox, o_xy, o_w1, t_off);
                 }
             }

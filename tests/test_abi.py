@@ -20,7 +20,7 @@ def lib():
 def _declared():
     src = open(os.path.join(ROOT, "include", "evis.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(evis_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(evis_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_every_declared_symbol_is_exported(lib):

@@ -1210,3 +1210,52 @@ def test_new_features_on_concurrent_regions(kw):
     rep = parity.run_parity(spec, 3, envs=[0, 4, 8], debug=False, capacity=1 << 24, **kw)
     _assert_tolerances(rep)
     assert rep.events_oracle > 10000
+
+
+# ------------------------------------------------------------------------------------------------
+# compact 8-byte events
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("tau_r", [0.0, 1e-3])
+def test_compact_events_are_the_events(tau_r):
+    """evis_set_compact_events: the 8-byte stream decodes to the 16-byte stream of a twin context, event for event in
+    the same order -- pixel, env, substep, polarity exact, the stamp within T / S * 2^-16 -- in the record path and in
+    the direct path (refractory period); the 16-byte read calls refuse; the API contract around the time sort."""
+    spec = scenes.small(scenes.config(4), num_envs=4, height=97, width=131, num_keyframes=4)
+    sc = scenes.make_scene(spec)
+    E, H, W, S, T = spec.num_envs, spec.height, spec.width, spec.substeps, spec.keyframe_dt
+    mk = lambda: binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, T, max_motion_px=spec.max_motion_px(),
+                              event_capacity=1 << 22)
+    a, b = mk(), mk()
+    if tau_r > 0:
+        a.set_refractory(tau_r); b.set_refractory(tau_r)
+    b.set_compact_events(True)
+    total = 0
+    for k in range(spec.num_keyframes):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        for ev in (a, b):
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        if k == 0:
+            continue
+        want = a.read_events()
+        got = binding.decode_events8(b.read_events8(), T, S, kf=k - 1)
+        assert len(want) == len(got) > 1000
+        for f in ("x", "y", "env", "p", "substep", "kf"):
+            assert np.array_equal(want[f], got[f]), f
+        assert np.abs(want["t_off"].astype(np.float64) - got["t_off"]).max() <= T / S * 2.0 ** -16 + 4e-9
+        total += len(got)
+        with pytest.raises(binding.EvisError) as ei:
+            b.read_events()
+        assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    hb = np.empty(1 << 22, np.uint64)
+    n = b.read_events8_begin(hb)
+    b.read_events_end()
+    assert n == len(got) and np.array_equal(binding.decode_events8(hb[:n], T, S, kf=spec.num_keyframes - 2), got)
+    with pytest.raises(binding.EvisError) as ei:
+        b.set_time_sorted(True)
+    assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    with pytest.raises(binding.EvisError) as ei:
+        a.read_events8()
+    assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    a.destroy(); b.destroy()
+    assert total > 5000
