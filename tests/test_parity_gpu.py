@@ -1259,3 +1259,25 @@ def test_compact_events_are_the_events(tau_r):
     assert ei.value.status == binding.EVIS_ERR_BAD_STATE
     a.destroy(); b.destroy()
     assert total > 5000
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kw", [{"defocus": 0.6}, {"mode": 2}])
+@pytest.mark.parametrize("hook", ["chunks", "no_tma", "no_ztag", "serial"])
+def test_new_features_under_the_launch_variants(kw, hook, monkeypatch):
+    """Defocus and the weighted splat where the z-buffers hold only a few substeps at a time (the carried unblurred frame
+    / state crosses substep chunks through memory), with direct key loads instead of TMA, with untagged 32-bit-index
+    keys, and with the order stage serialised."""
+    if hook == "chunks":
+        monkeypatch.setenv("EVIS_ZBUF_MB", "1")                  # 0.4 MB per env and substep: 2 substeps per chunk
+    elif hook == "no_tma":
+        monkeypatch.setenv("EVIS_NO_TMA", "1")
+    elif hook == "no_ztag":
+        monkeypatch.setenv("EVIS_NO_ZTAG", "1")
+    else:
+        monkeypatch.setenv("EVIS_NO_OVERLAP", "1")
+        monkeypatch.setenv("EVIS_STREAMS", "1")
+    spec = scenes.small(scenes.config(2), num_envs=3, height=121, width=163, num_keyframes=4, substeps=7)
+    rep = parity.run_parity(spec, 4, **kw)
+    _assert_tolerances(rep)
+    assert rep.holes > 0 and rep.events_oracle > 1000
