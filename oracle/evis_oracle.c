@@ -24,11 +24,13 @@
  * keyframe B, P3 integer translation, P4 8x8 gather-form brute force, P5 analytic two-rectangle
  * occlusion, P6-P10 event-count / residual / timestamp closed forms, P11 per-pixel thresholds (Eq. 8), P12 refractory period, P13 margin, P14 colour, P15 noise events,
  * P16 composite mode 1 (every case of the rule by hand; linear time ramp along a translation), P19 defocus (library
- * Gaussian filter, blur-before-log, holes held unblurred).  UNPINNED by paper or
+ * Gaussian filter, blur-before-log, holes held unblurred), P20 weighted front-surface splat (exact float64 gather form on
+ * 8x8, closed forms).  UNPINNED by paper or
  * mathematics (fixed by DESIGN.md readings only): log base R1, epsilon R2, initial reference
  * level R6, nearest-pixel depth lookup R16, hole handling R20, the composite choice R19, and among the
  * non-idealities the choices of R26 (L_ref follows suppressed crossings) and R29 (Ibar's normalisation, stamps,
- * stream order, independence from the refractory period).
+ * stream order, independence from the refractory period), of R31 (truncation radius ceil(3 sigma), replicated border) and of
+ * R32 (the 1 % front-surface band, the mean taken in the log domain, the 2^-20 / 2^-24 grids of its integer sums).
  */
 #include <math.h>
 #include <stdint.h>
