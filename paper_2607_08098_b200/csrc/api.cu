@@ -826,10 +826,7 @@ static int voxel_finish(evis_ctx *ctx, int normalize)
     const Geom &g = ctx->g;
     const uint32_t plane = (uint32_t)(g.H - 2 * g.margin) * (uint32_t)(g.W - 2 * g.margin);
     if (ctx->copy_pending) CU(cudaStreamWaitEvent(ctx->ord_stream, ctx->ev_copy, 0));
-    if (ctx->last_stream || ctx->steps) {                     // a step's order stage follows its chunk phase on ord_stream already;
-        CU(cudaEventRecord(ctx->ev_chunks[0], ctx->last_stream));     // this covers a context that has only seen its first keyframe
-        CU(cudaStreamWaitEvent(ctx->ord_stream, ctx->ev_chunks[0], 0));
-    }
+    // (the order stream already follows every step's chunk phase: nothing else to wait for)
     CU(launch_voxel_finish(ctx->vox_v, ctx->vox_out, (uint32_t)(ctx->vox_cells / plane), plane, normalize, ctx->ord_stream));
     ctx->launches += 1;
     return EVIS_OK;
