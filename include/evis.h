@@ -6,7 +6,7 @@
  *            event count n = floor(|dL|/C), polarity, reference update L_ref += p n C;
  *   Sec. 3.3, Eq. 5-7 (lines 106-131): bidirectional motion-vector warping of keyframes A and B
  *            with z-buffered depth splatting, B primary / A fills holes (line 129).
- * Readings of silent or ambiguous points: DESIGN.md Sec. 2 (R1-R24).
+ * Readings of silent or ambiguous points: DESIGN.md Sec. 2 (R1-R33).
  *
  * Conventions.  E environments, H x W pixels, S substeps per keyframe interval (S = the paper's
  * upsampling factor K).  Pixel (x, y) has its centre at integer coordinates, x right, y down.
