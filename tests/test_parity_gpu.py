@@ -1281,3 +1281,46 @@ def test_new_features_under_the_launch_variants(kw, hook, monkeypatch):
     rep = parity.run_parity(spec, 4, **kw)
     _assert_tolerances(rep)
     assert rep.holes > 0 and rep.events_oracle > 1000
+
+
+@pytest.mark.gpu
+def test_time_sort_with_silent_envs_and_overflow():
+    """Environments without a single event (static: first, middle and last of the batch) leave empty segments; the
+    sorted stream is still the stable (env, t) sort of the unsorted one.  With a capacity below the step's events the
+    stored prefix is sorted and the read call reports the overflow."""
+    spec = scenes.small(scenes.config(4), num_envs=6, height=90, width=120, num_keyframes=3)
+    sc = scenes.make_scene(spec)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    silent = [0, 3, 5]
+    kfs = []
+    for k in range(spec.num_keyframes):
+        kf = scenes.render_keyframe(sc, k, device="cuda")
+        if k == 0:
+            first = {a: b.clone() for a, b in kf.items()}
+        for e in silent:                              # the same frame again, no motion: nothing fires
+            kf["rad"][e] = first["rad"][e]; kf["depth"][e] = first["depth"][e]
+            kf["mv_bwd"][e] = 0; kf["mv_fwd"][e] = 0
+        kfs.append(kf)
+
+    def run(cap, sort):
+        ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, event_capacity=cap)
+        ev.set_time_sorted(sort)
+        out = []
+        for k, kf in enumerate(kfs):
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True,
+                    allow=(binding.EVIS_ERR_OVERFLOW,))
+            if k:
+                out.append((ev.read_events(allow=(binding.EVIS_ERR_OVERFLOW,)).copy(), ev.info().last_events, ev.info().last_overflow))
+        ev.destroy()
+        return out
+
+    plain, srt = run(1 << 22, False), run(1 << 22, True)
+    for (a, na, _), (b, nb, _) in zip(plain, srt):
+        assert na == nb == len(a) == len(b) > 1000
+        assert not np.isin(a["env"], silent).any()
+        assert b.tobytes() == a[np.lexsort((a["t_off"].view(np.uint32), a["env"]))].tobytes()
+    cap = int(plain[0][1] // 3)
+    small_plain, small_sorted = run(cap, False), run(cap, True)
+    for (a, na, oa), (b, nb, ob) in zip(small_plain, small_sorted):
+        assert na == nb > cap and oa == ob == 1 and len(a) == len(b) == cap
+        assert b.tobytes() == a[np.lexsort((a["t_off"].view(np.uint32), a["env"]))].tobytes()
