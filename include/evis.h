@@ -235,7 +235,8 @@ int evis_set_refractory(evis_ctx *ctx, float tau_r);
  * polarity channel -- the two bins that bracket tau share one unit; bins = 1 is the plain per-polarity event count.
  * The sums are kept in 32.32 fixed point with integer atomics, so they do not depend on scheduling.  The first
  * window starts with the next evis_step that closes an interval; when a window is full the next step clears the grid
- * and starts a new one (read it before).  keep_events = 0: the ordered event stream is not stored at all (the read
+ * and starts a new one (read it before).  The grid takes EVERY event of a step, also those beyond event_capacity (only
+ * an overflow of the intermediate records, evis_info last_overflow = 2, loses events).  keep_events = 0: the ordered event stream is not stored at all (the read
  * calls for events then return BAD_STATE) -- no 16-byte event ever leaves the GPU.  cfg = NULL switches the grid off.
  * Synchronises.  Errors: INVALID_ARG (bins < 1, window_steps < 1), CUDA, OOM. */
 typedef struct {

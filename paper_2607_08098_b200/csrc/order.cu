@@ -134,8 +134,10 @@ k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *
     if (threadIdx.x == ORD_NT - 1) s_rel[ORD_PER_BLOCK] = 0xFFFFFFFFu;           // sentinel: the walk stops here
     __syncthreads();
     const unsigned long long out0 = bsum[blockIdx.x];
-    if (out0 >= cap) return;
-    const uint32_t tot = (uint32_t)(total < cap - out0 ? total : cap - out0);   // positions this block may store
+    if (out0 >= cap && !vox.v) return;
+    // positions this block may store; the voxel grid takes every event, stored or not
+    const uint32_t tot_store = out0 >= cap ? 0u : (uint32_t)(total < cap - out0 ? total : cap - out0);
+    const uint32_t tot = vox.v ? (uint32_t)total : tot_store;
     uint32_t e = 0;
     constexpr int U = 4;
     for (uint32_t o0 = threadIdx.x; o0 < tot; o0 += U * ORD_NT) {
@@ -155,8 +157,9 @@ k_dir_copy(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *
 #pragma unroll
         for (int u = 0; u < U; ++u)
             if (ok[u]) {
-                if (vox.store_events == 1) ordered[out0 + o0 + u * ORD_NT] = val[u];
-                else if (vox.store_events == 2) {
+                const bool st_ = o0 + u * ORD_NT < tot_store;
+                if (st_ && vox.store_events == 1) ordered[out0 + o0 + u * ORD_NT] = val[u];
+                else if (st_ && vox.store_events == 2) {
                     // direct mode stamps in seconds: back to the fraction of the substep
                     const float t0 = __fmul_rn((float)((val[u].y >> 24) - 1u), vox.dt);
                     reinterpret_cast<unsigned long long *>(ordered)[out0 + o0 + u * ORD_NT] =
@@ -206,7 +209,7 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
     for (int j = 0; j < ORD_PER_THREAD; ++j) { s_rel[threadIdx.x * ORD_PER_THREAD + j] = (uint32_t)run; run += cnt[j]; }
     __syncthreads();
     const unsigned long long out0 = bsum[blockIdx.x];
-    if (out0 >= cap) return;
+    if (out0 >= cap && !vox.v) return;
     const int lane = threadIdx.x & 31;
     for (;;) {
         uint32_t e = 0;
@@ -275,11 +278,13 @@ k_expand(const uint2 *__restrict__ dir, uint32_t n, const unsigned long long *__
                 float fr = __fmul_rn(__fsub_rn(__fmaf_rn(kf, o_pc, o_ref), o_prev), o_rden);
                 fr = fminf(fmaxf(fr, 0.0f), 1.0f);
                 const unsigned long long o = first + e;
-                if (e < total_ev && o < cap) {
+                if (e < total_ev) {
                     const float t_off = __fmaf_rn(fr, ep.dt, t0);
-                    if (vox.store_events == 1) ordered[o] = make_uint4(o_xy, o_w1, __float_as_uint(t_off), ep.kf);
-                    else if (vox.store_events == 2) reinterpret_cast<unsigned long long *>(ordered)[o] = pack_event8(o_xy, o_w1, fr);
-                    if (vox.v) voxel_add(vox, o_xy, o_w1, t_off);
+                    if (o < cap) {
+                        if (vox.store_events == 1) ordered[o] = make_uint4(o_xy, o_w1, __float_as_uint(t_off), ep.kf);
+                        else if (vox.store_events == 2) reinterpret_cast<unsigned long long *>(ordered)[o] = pack_event8(o_xy, o_w1, fr);
+                    }
+                    if (vox.v) voxel_add(vox, o_xy, o_w1, t_off);        // the grid takes every event, stored or not
                 }
             }
             first += total_ev;

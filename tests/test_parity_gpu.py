@@ -1324,3 +1324,37 @@ def test_time_sort_with_silent_envs_and_overflow():
     for (a, na, oa), (b, nb, ob) in zip(small_plain, small_sorted):
         assert na == nb > cap and oa == ob == 1 and len(a) == len(b) == cap
         assert b.tobytes() == a[np.lexsort((a["t_off"].view(np.uint32), a["env"]))].tobytes()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("tau_r", [0.0, 1e-3])
+def test_voxel_grid_counts_events_beyond_the_stored_capacity(tau_r):
+    """A step with more events than event_capacity stores a prefix of the stream (last_overflow = 1), but its
+    accumulation image still holds every event (expand and copy kernels)."""
+    spec = scenes.small(scenes.config(4), num_envs=3, height=90, width=120, num_keyframes=3)
+    sc = scenes.make_scene(spec)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(spec.num_keyframes)]
+
+    def run(cap):
+        ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt, event_capacity=cap)
+        if tau_r > 0:
+            ev.set_refractory(tau_r)
+        ev.set_voxels(1)
+        out = []
+        for k, kf in enumerate(kfs):
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True, allow=(binding.EVIS_ERR_OVERFLOW,))
+            if k:
+                out.append((ev.read_voxels()[0], ev.info().last_events, ev.info().last_overflow))
+        ev.destroy()
+        return out
+
+    full = run(1 << 22)
+    n_min = min(n for _, n, _ in full)
+    tight = run(int(0.93 * n_min))                     # above the record count (direct mode: just below the events)
+    for (g0, n0, o0), (g1, n1, o1) in zip(full, tight):
+        assert n0 == n1 and o0 == 0 and o1 >= 1
+        if o1 == 1:                                    # a stored prefix: the grid must be whole
+            assert np.array_equal(g0, g1) and abs(float(g1.sum(dtype=np.float64)) - n1) < 0.5
+    # direct mode keeps EVENTS in the arrival buffer, so there the intermediate buffer overflows with the stream (2)
+    assert any(o == (2 if tau_r > 0 else 1) for _, _, o in tight)
