@@ -307,9 +307,11 @@ int create_impl(evis_ctx *ctx)
         // chunk = envs x substeps whose z-buffers fit one region's budget.  Defaults (measured on B200, DESIGN.md
         // Sec. 6): 4 regions on 4 streams; 24 MiB regions when one env's S substeps fit (the live keys stay in the
         // L2 and small grids overlap across streams), else 512 MiB / regions (substep chunks re-read the sources and carry
-        // L_ref / L_prev through memory, so they should be long).  EVIS_ZBUF_MB / EVIS_STREAMS override.
+        // L_ref / L_prev through memory, so they should be long); an env whose whole interval does not even fit that
+        // share (cfg 3: 488 MB) gets 2 regions of 256 MiB (cfg 3: 17.8 -> 16.4 ms).  EVIS_ZBUF_MB / EVIS_STREAMS override.
         const size_t unit = (size_t)ctx->nset * 8u * 2u * (size_t)g.HWp;
-        const size_t default_regions = 4;
+        const bool huge = unit * g.S > ((size_t)128 << 20);
+        const size_t default_regions = huge ? 2 : 4;
         const size_t share = (size_t)512 / ((size_t)g.E < default_regions ? (size_t)g.E : default_regions);   // of 512 MiB
         size_t budget = env_size_mb("EVIS_ZBUF_MB", unit * g.S <= ((size_t)24 << 20) ? 24 : share) << 20;
         if (budget > ((size_t)8 << 30)) budget = (size_t)8 << 30;    // the kernels index a chunk with 32-bit offsets
