@@ -41,29 +41,25 @@ RANGE_CAPTURE = os.path.join("profiles", "round2_a_range_cfg4.csv")
 RANGE_WORKLOAD, RANGE_STEPS = "cfg4_256env_346x260_S16_rl", 5
 
 
-def chunk_traffic(workload: str):
-    """DRAM bytes (read + write) of one env chunk = one k_splat_global + one k_resolve_global launch, from the committed
-    `ncu --set full` capture of the two kernels ALONE (profiles/round2_b_ncu_full_cfg4.csv: cold caches, serialised), or
-    None for another workload."""
+def step_traffic(workload: str):
+    """DRAM bytes (read + write) of ONE WHOLE STEP in the schedule the bench runs: mean over the graph launches of the
+    committed `ncu --graph-profiling graph` capture (profiles/round2_f_graph_cfg4.md), or None for another workload."""
     if workload != RANGE_WORKLOAD:
         return None
     try:
         import csv
-        tot = {"k_splat_global": [0.0, 0], "k_resolve_global": [0.0, 0]}
-        with open(os.path.join(ROOT, "profiles", "round2_b_ncu_full_cfg4.csv")) as f:
-            rows = list(csv.reader(f))
-        h = {name: i for i, name in enumerate(rows[0])}
-        for r in rows[2:]:
-            if not r[0].startswith("chunk kernels alone"):
-                continue
-            for k in tot:
-                if r[1].startswith(k):
-                    tot[k][0] += float(r[h["dram__bytes_read.sum"]]) * 1e6 + float(r[h["dram__bytes_write.sum"]])
-                    tot[k][1] += 1
-        if not all(v[1] for v in tot.values()):
+        rd, wr = [], []
+        with open(os.path.join(ROOT, "profiles", "round2_f_graph_cfg4.csv")) as f:
+            for row in csv.reader(f):
+                if len(row) >= 15 and row[4] == "graph":
+                    if row[12] == "dram__bytes_read.sum":
+                        rd.append(float(row[14].replace(",", "")))
+                    elif row[12] == "dram__bytes_write.sum":
+                        wr.append(float(row[14].replace(",", "")))
+        if not rd or len(rd) != len(wr):
             return None
-        return sum(v[0] / v[1] for v in tot.values())
-    except (OSError, ValueError, KeyError, IndexError):
+        return (sum(rd) + sum(wr)) / len(rd)
+    except (OSError, ValueError):
         return None
 
 
@@ -106,6 +102,10 @@ def parse_args():
     ap.add_argument("--profile-range", action="store_true",
                     help="bracket the timed region with cudaProfilerStart / Stop (for `ncu --replay-mode app-range`: "
                          "counters of the whole step in its real multi-stream schedule); implies no e2e / cpu legs")
+    ap.add_argument("--graph-probe", action="store_true",
+                    help="measurement hook: every timed step is captured and launched as ONE CUDA graph (EVIS_GRAPH=1) on a "
+                         "stream of its own, so that `ncu --graph-profiling graph` measures the whole step in its real "
+                         "multi-stream schedule; the steps are serialised by the capture: no throughput claim; implies no e2e / cpu legs")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json config 5: one JSON line per (envs x resolution x S) point, device-resident")
     return ap.parse_args()
@@ -254,6 +254,10 @@ def run_ours(args, spec) -> None:
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     binding.load()                                     # fails loudly when libevis.so is missing
+    if args.graph_probe:
+        os.environ["EVIS_GRAPH"] = "1"
+        args.no_e2e = args.no_cpu = True
+        args.profile_range = True                      # cudaProfilerStart / Stop around the timed steps (ncu --profile-from-start off)
 
     K, Wm = args.steps, args.warmup
     n_kf = Wm + K + 1
@@ -285,7 +289,7 @@ def run_ours(args, spec) -> None:
             e.set_time_sorted(True)
         return e
     ev = mk()
-    stream = torch.cuda.current_stream(dev)
+    stream = torch.cuda.Stream(dev) if args.graph_probe else torch.cuda.current_stream(dev)   # a capture needs a stream of its own
 
     def step(k):
         f = kfs[k]
@@ -358,12 +362,10 @@ def run_ours(args, spec) -> None:
     cap_ = range_capture(spec.name)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": chunk_traffic(spec.name),
-                "traffic_note": "DRAM bytes of ONE env chunk (one splat + one resolve launch) measured by `ncu --set full` on the "
-                "two kernels alone, cold caches, serialised (profiles/round2_b_ncu_full_cfg4.csv); its algorithmic share is "
-                "`algorithmic_bytes_per_chunk`.  In the bench's schedule the chunk's 23 MB of keys stay in the L2 between the "
-                "two launches; ncu cannot measure that schedule (it serialises the streams, profiles/round2_README.md)",
-                "algorithmic_bytes_per_chunk": algo_bytes_step / E,      # a chunk of this workload = one env; prep's and expand's share included
+                "traffic": step_traffic(spec.name),
+                "traffic_note": "DRAM bytes of one WHOLE step in its real multi-stream schedule: the step captured as one CUDA graph "
+                "and measured by `ncu --graph-profiling graph` (profiles/round2_f_graph_cfg4.md; steps with ~130 M events, "
+                "3.3 GB algorithmic)",
                 "algorithmic_bytes_per_step": algo_bytes_step, "basis": "whole step: algorithmic bytes / ms_per_step",
                 "dominant_stage_ms": stage_ms[dom], "dominant_stage_launches_per_step": max(1.0, prof["launches"][dom] / K),
                 "stage_ms_per_step": stage_ms, "stage_launches_per_step": {k: v / K for k, v in prof["launches"].items()}}

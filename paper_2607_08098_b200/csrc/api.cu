@@ -92,6 +92,7 @@ struct evis_ctx {
     long long *wacc;
     size_t wchunk_elems;              // chunk_ne * chunk_ni * HW
 
+    bool graph_mode;                  // EVIS_GRAPH=1 (measurement hook): every step is captured and launched as one CUDA graph
     bool compact;                     // evis_set_compact_events: the stored stream holds 8-byte events
 
     // time-sorted stream (evis_set_time_sorted): workspace of the segmented radix sort
@@ -381,6 +382,8 @@ int create_impl(evis_ctx *ctx)
     CU(cudaHostAlloc((void **)&ctx->h_counters, NCOUNTERS * sizeof(unsigned long long), cudaHostAllocDefault));
     memset(ctx->h_counters, 0, NCOUNTERS * sizeof(unsigned long long));
     {
+        const char *gm = getenv("EVIS_GRAPH");
+        ctx->graph_mode = gm && gm[0] == '1';
         const char *no = getenv("EVIS_NO_OVERLAP");       // test hook: order stage serialised with the next step
         ctx->overlap = !(no && no[0] == '1');
         ctx->arrival_s[0] = ctx->arrival; ctx->directory_s[0] = ctx->directory; ctx->counters_s[0] = ctx->counters;
@@ -501,13 +504,12 @@ int evis_destroy(evis_ctx *ctx)
     return EVIS_OK;
 }
 
-int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd, const float *depth,
-              void *cuda_stream, uint64_t *n_events)
+// Everything evis_step enqueues.  capturing: `st` is being captured into a CUDA graph (EVIS_GRAPH=1, a measurement
+// hook: ncu can then profile the whole step as ONE workload in its real multi-stream schedule): every stream the
+// step forks must join `st` again before the capture ends.
+static int step_enqueue(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd, const float *depth,
+                        cudaStream_t st, bool capturing)
 {
-    if (!ctx || !rad || !mv_bwd || !depth) return EVIS_ERR_INVALID_ARG;
-    DeviceGuard guard(ctx->cfg.device);
-    if (!guard.ok) return EVIS_ERR_CUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
     const Geom &g = ctx->g;
     const size_t P = (size_t)g.E * g.HW;
     Keyframe &B = ctx->kf[ctx->cur];
@@ -538,7 +540,6 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
         ctx->steps = 1;
         ctx->cur = (ctx->cur + 1) % 3;
         ctx->have_events = true;
-        if (n_events) { CU(cudaStreamSynchronize(st)); *n_events = 0; }
         return EVIS_OK;
     }
 
@@ -575,7 +576,7 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     // waits for them instead, and every call that returns results waits for the order stream.  `st` is then free to run
     // the NEXT step's prep (HBM-bound, into the third keyframe buffer) under this step's chunk kernels; it cannot run
     // further ahead than that, because a step's clears wait for the order stage of two steps before (ev_order).
-    const bool join_st = !ctx->overlap || ctx->prof_on;
+    const bool join_st = !ctx->overlap || ctx->prof_on || capturing;
     {
         // nreg > 1: the env chunks are dealt round-robin to the regions' streams, which fork from `st` here; the
         // substep chunks of one env chunk stay on one stream (L_ref / L_prev carry)
@@ -703,6 +704,47 @@ int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float 
     ctx->kf_next += 1;
     ctx->cur = (ctx->cur + 1) % 3;
     ctx->have_events = true;
+    if (capturing) CU(cudaStreamWaitEvent(st, ctx->ev_order[sl], 0));       // the order stream joins the captured stream
+    return EVIS_OK;
+}
+
+int evis_step(evis_ctx *ctx, const float *rad, const float *mv_bwd, const float *mv_fwd, const float *depth,
+              void *cuda_stream, uint64_t *n_events)
+{
+    if (!ctx || !rad || !mv_bwd || !depth) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const bool first = ctx->steps == 0;
+    if (ctx->graph_mode && !first && st != nullptr) {
+        // measurement hook (EVIS_GRAPH=1): the step as one CUDA graph launch.  Nothing of an earlier step may be pending
+        // (a capture cannot wait for work outside it), so the device is drained first: this is not a fast path.
+        CU(cudaDeviceSynchronize());
+        ctx->ord_pending[0] = ctx->ord_pending[1] = false;
+        ctx->copy_pending = false;
+        CU(cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed));
+        const int rc = step_enqueue(ctx, rad, mv_bwd, mv_fwd, depth, st, true);
+        cudaGraph_t gr = nullptr;
+        cudaError_t e = cudaStreamEndCapture(st, &gr);
+        cudaGraphExec_t ex = nullptr;
+        if (rc == EVIS_OK && e == cudaSuccess) e = cudaGraphInstantiate(&ex, gr, 0);
+        if (rc == EVIS_OK && e == cudaSuccess) e = cudaGraphLaunch(ex, st);
+        if (rc == EVIS_OK && e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (ex) cudaGraphExecDestroy(ex);
+        if (gr) cudaGraphDestroy(gr);
+        // the events recorded inside the capture belong to the graph: nothing outside may wait for them, and nothing
+        // needs to -- the launch has been waited for, order stage included
+        ctx->ord_pending[0] = ctx->ord_pending[1] = false;
+        if (rc != EVIS_OK) return rc;
+        CU(e);
+    } else {
+        const int rc = step_enqueue(ctx, rad, mv_bwd, mv_fwd, depth, st, false);
+        if (rc != EVIS_OK) return rc;
+    }
+    if (first) {
+        if (n_events) { CU(cudaStreamSynchronize(st)); *n_events = 0; }
+        return EVIS_OK;
+    }
     if (n_events) {
         const int rc = fetch_counters(ctx);
         if (rc != EVIS_OK) return rc;

@@ -37,8 +37,8 @@ def test_bench_reads_the_committed_captures():
     cap = bench.range_capture(bench.RANGE_WORKLOAD)
     assert cap and 2.0e9 < cap["smsp__inst_executed.sum"] < 4.0e9          # warp-instructions per cfg 4 step
     assert cap["dram__bytes_read.sum"] > 1e9
-    tr = bench.chunk_traffic(bench.RANGE_WORKLOAD)
-    assert tr and 1.0e7 < tr < 1.0e8                                        # one env chunk: tens of MB cold-cache
-    assert bench.range_capture("cfg2_16env_640x480_S16") is None and bench.chunk_traffic("other") is None
+    tr = bench.step_traffic(bench.RANGE_WORKLOAD)
+    assert tr and 5.0e9 < tr < 3.0e10                                       # one whole step: ~11 GB
+    assert bench.range_capture("cfg2_16env_640x480_S16") is None and bench.step_traffic("other") is None
     peak, src = bench.hbm_peak()
     assert 3000.0 < peak < 9000.0 and src

@@ -1358,3 +1358,39 @@ def test_voxel_grid_counts_events_beyond_the_stored_capacity(tau_r):
             assert np.array_equal(g0, g1) and abs(float(g1.sum(dtype=np.float64)) - n1) < 0.5
     # direct mode keeps EVENTS in the arrival buffer, so there the intermediate buffer overflows with the stream (2)
     assert any(o == (2 if tau_r > 0 else 1) for _, _, o in tight)
+
+
+@pytest.mark.gpu
+def test_graph_capture_hook_gives_the_same_stream(monkeypatch):
+    """EVIS_GRAPH=1 (measurement hook: every step captured and launched as one CUDA graph on a non-default stream, all
+    forked streams joined inside the capture) must not change a bit of the output."""
+    spec = scenes.small(scenes.config(4), num_envs=6, height=120, width=160, num_keyframes=4)
+    sc = scenes.make_scene(spec)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+
+    def run(graph):
+        if graph:
+            monkeypatch.setenv("EVIS_GRAPH", "1")
+        else:
+            monkeypatch.delenv("EVIS_GRAPH", raising=False)
+        ev = binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                          max_motion_px=spec.max_motion_px(), event_capacity=1 << 23)
+        ev.set_voxels(2)
+        st = torch.cuda.Stream()
+        out = []
+        for k in range(spec.num_keyframes):
+            kf = scenes.render_keyframe(sc, k, device="cuda")
+            torch.cuda.synchronize()
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], stream=st, sync=True)
+            if k:
+                out.append((ev.read_events().copy(), ev.read_voxels()[0], ev.info().last_holes))
+        state = ev.get_state()
+        ev.destroy()
+        return out, state
+
+    a, sa = run(False)
+    b, sb = run(True)
+    assert sum(len(x[0]) for x in a) > 5000
+    for (ea, va, ha), (eb, vb, hb) in zip(a, b):
+        assert ea.tobytes() == eb.tobytes() and np.array_equal(va, vb) and ha == hb
+    assert np.array_equal(sa[0], sb[0]) and np.array_equal(sa[1], sb[1])
