@@ -39,7 +39,8 @@ typedef enum {
                                      last_overflow = 2): a read call then reports 0 events */
     EVIS_ERR_MOTION_BOUND = -5,   /* a motion vector exceeded the max_motion_px the caller declared (the results
                                      are exact all the same: the z-buffers take any motion) */
-    EVIS_ERR_BAD_STATE    = -6    /* call order violated (e.g. read before any step) */
+    EVIS_ERR_BAD_STATE    = -6,   /* call order violated (e.g. read before any step) */
+    EVIS_ERR_TOO_LARGE    = -7    /* evis_voxelize_static: the grid has more cells than the fixed accumulator */
 } evis_status;
 
 /* One path: z-buffers in global memory (L2-resident chunks), any motion.  The per-tile shared-memory path of
@@ -258,6 +259,51 @@ int evis_read_voxels(evis_ctx *ctx, float *dst, int dst_is_device, int normalize
  * The next step's accumulation waits for the copy too. */
 int evis_read_voxels_begin(evis_ctx *ctx, float *host_dst, int normalize, int restart);
 int evis_read_voxels_end(evis_ctx *ctx);
+
+/* The voxel grid of a FINISHED event stream, for callers that must not allocate device memory.
+ *
+ * Who that is: evis_set_voxels calls cudaMalloc for its accumulator, and cudaMalloc / cudaFree both can fail and make
+ * every stream of the device wait.  A rollout loop in which the simulator, the renderer and the learner have shared out
+ * the GPU's memory among their own pools beforehand can afford neither while it runs; nor can a consumer that was handed
+ * events (a recording, another process's stream) and owns no evis_ctx at all.  This call gives them the same grid from
+ * memory the library already holds: it calls no cudaMalloc, cudaFree or other allocating routine, creates no stream or
+ * event and needs no context.  The caller brings the input and the output; the 32.32 fixed-point accumulator between
+ * them is ONE array of EVIS_VOXELIZE_STATIC_MAX_CELLS 64-bit words (16 MiB) that is part of the library's device image:
+ * every GPU on which this library's kernels are loaded holds it until the process exits, whether or not this function
+ * is ever called.
+ *
+ *   events  [n_events] DEVICE, 16-byte aligned, read-only: evis_event records as evis_read_events / evis_events_device
+ *           deliver them (any order).  NULL is allowed when n_events = 0.
+ *   grid    [num_envs, 2, bins, height, width] float32 DEVICE, written: the grid evis_read_voxels returns for a window
+ *           of `window_steps` intervals of length keyframe_dt that starts with interval first_kf -- an event counts with
+ *           t = (kf - first_kf) * keyframe_dt + t_off (binary32, as evis_step forms it); channel 0 = ON, 1 = OFF;
+ *           height x width is the frame the events' x, y refer to (the cropped frame when a margin was set).  Events
+ *           whose kf lies outside the window, whose x, y lie outside the frame or whose env >= num_envs add nothing.
+ *   normalize != 0: every (env, channel, bin) plane is divided by its own maximum when that is > 0.
+ *   cuda_stream: a cudaStream_t of the CURRENT device (NULL = default stream).  The call only enqueues (a clear of the
+ *           cells it uses, the accumulation, the conversion to float32) and does not wait: `grid` is complete when the
+ *           stream has run that work; `events` must stay valid until then.
+ *   cuda_error (nullable): receives the cudaError_t behind an EVIS_ERR_CUDA return, else 0.
+ *
+ * The device that is current when the call is made is the one whose copy of the array is used: events, grid and the
+ * stream must belong to it.  The FIRST call on each device also looks up the array's device address
+ * (cudaGetSymbolAddress) and may make the CUDA runtime load the library's kernels; make that first call before any
+ * stream capture is begun.  Later calls only enqueue the three operations.
+ *
+ * Sharing: all calls on a device use the same array, and it keeps whatever the last call left in it; each call clears
+ * the cells it is about to use first, on its stream.  Calls whose work is ordered on the GPU (same stream, or streams
+ * ordered by events) are safe back to back.  Calls whose work may OVERLAP on the GPU -- different unordered streams,
+ * from one host thread or several -- race on the array and give wrong grids; so they must be serialised by the caller.
+ *
+ * Limit: 2 * num_envs * bins * height * width <= EVIS_VOXELIZE_STATIC_MAX_CELLS (2^21, e.g. 346 x 260, 5 bins, 2
+ * environments); a larger grid is refused with EVIS_ERR_TOO_LARGE before anything is enqueued and `grid` is left
+ * untouched -- call it per group of environments on that group's events, or use evis_set_voxels where allocating is allowed.
+ * Errors: INVALID_ARG (NULL grid, NULL events with n_events > 0, a size or bins or window_steps < 1, keyframe_dt not
+ * finite and > 0), TOO_LARGE, CUDA.  Argument errors are detected before any CUDA call. */
+#define EVIS_VOXELIZE_STATIC_MAX_CELLS (1u << 21)
+int evis_voxelize_static(const evis_event *events, uint64_t n_events, int32_t num_envs, int32_t height, int32_t width,
+                         int32_t bins, int32_t window_steps, float keyframe_dt, uint32_t first_kf, int normalize,
+                         float *grid, void *cuda_stream, int *cuda_error);
 
 /* Time-sorted per-environment stream (the stream E = {(u_k, t_k, p_k)} of PAPER.md:90 in time order): with on != 0 the
  * stored stream of every later step is ordered by (env, t_off); events of one environment with equal timestamps keep

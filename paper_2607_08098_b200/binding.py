@@ -19,6 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libevis.so")
 EVIS_OK = 0
 EVIS_ERR_INVALID_ARG, EVIS_ERR_CUDA, EVIS_ERR_OOM = -1, -2, -3
 EVIS_ERR_OVERFLOW, EVIS_ERR_MOTION_BOUND, EVIS_ERR_BAD_STATE = -4, -5, -6
+EVIS_ERR_TOO_LARGE = -7
+VOXELIZE_STATIC_MAX_CELLS = 1 << 21      # EVIS_VOXELIZE_STATIC_MAX_CELLS of include/evis.h
 PATH_AUTO, PATH_GLOBAL = 0, 1
 COMPOSITE_B_PRIMARY, COMPOSITE_BLEND, COMPOSITE_WEIGHTED = 0, 1, 2
 
@@ -55,7 +57,8 @@ class evis_profile(C.Structure):
 SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "evis_events_device",
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
            "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end",
-           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus", "evis_set_time_sorted", "evis_set_compact_events", "evis_read_events8", "evis_read_events8_begin"]
+           "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus", "evis_set_time_sorted", "evis_set_compact_events", "evis_read_events8", "evis_read_events8_begin",
+           "evis_voxelize_static"]
 
 _lib = None
 
@@ -103,6 +106,8 @@ def load() -> C.CDLL:
     L.evis_set_compact_events.argtypes = [vp, C.c_int]
     L.evis_read_events8.argtypes = [vp, vp, C.c_int, C.c_uint64, u64p]
     L.evis_read_events8_begin.argtypes = [vp, vp, C.c_uint64, u64p]
+    L.evis_voxelize_static.argtypes = [vp, C.c_uint64, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_float,
+                                       C.c_uint32, C.c_int, vp, vp, C.POINTER(C.c_int)]
     L.evis_last_cuda_error.argtypes = [vp]
     L.evis_version.restype = C.c_char_p
     for name in SYMBOLS:
@@ -395,6 +400,34 @@ class Evis:
             self.destroy()
         except Exception:
             pass
+
+
+def voxelize_static(events: torch.Tensor, grid: torch.Tensor, window_steps: int, keyframe_dt: float, first_kf: int = 0,
+                    normalize: bool = False, stream: Optional[torch.cuda.Stream] = None) -> None:
+    """evis_voxelize_static: the voxel grid of finished events WITHOUT any device allocation -- for code that runs where
+    cudaMalloc is off limits (a rollout loop whose memory was shared out among the simulator's, the renderer's and the
+    learner's pools beforehand, and where an allocation would also stall every stream of the GPU) and so cannot use
+    ``Evis.set_voxels``.  The caller owns both tensors, and this wrapper creates none: ``events`` is a contiguous CUDA
+    tensor of 16-byte evis_event records (uint8 [n, 16] or int32 [n, 4]; n may be 0), ``grid`` a contiguous float32 CUDA
+    tensor [E, 2, bins, H, W] on the same device, overwritten.  The accumulator in between is a fixed 16 MiB array inside
+    the library, shared by all calls on a GPU: E * 2 * bins * H * W may not exceed ``VOXELIZE_STATIC_MAX_CELLS``
+    (EvisError with EVIS_ERR_TOO_LARGE otherwise), and calls whose GPU work can overlap (unordered streams) must be
+    serialised by the caller.  Only enqueues on ``stream`` (default: torch's current stream of that device).  The first
+    call on a device also does the library's one-time address look-up: make it before any stream capture."""
+    if not (events.is_cuda and events.is_contiguous() and events.dim() == 2 and
+            events.shape[1] * events.element_size() == 16 and events.data_ptr() % 16 == 0):
+        raise ValueError("events: need a contiguous, 16-byte aligned CUDA tensor of 16-byte records, shape [n, 16 / itemsize]")
+    if not (grid.is_cuda and grid.dtype == torch.float32 and grid.is_contiguous() and grid.dim() == 5 and grid.shape[1] == 2
+            and grid.device == events.device):
+        raise ValueError("grid: need a contiguous float32 CUDA tensor [E, 2, bins, H, W] on the events' device")
+    E, _, bins, H, W = (int(v) for v in grid.shape)
+    err = C.c_int(0)
+    with torch.cuda.device(grid.device):            # the library uses the current device's copy of its array
+        st = (stream or torch.cuda.current_stream(grid.device)).cuda_stream
+        rc = load().evis_voxelize_static(events.data_ptr() if events.shape[0] else None, int(events.shape[0]), E, H, W, bins,
+                                         int(window_steps), float(keyframe_dt), int(first_kf), int(bool(normalize)),
+                                         grid.data_ptr(), C.c_void_p(st), C.byref(err))
+    _check(rc, f"evis_voxelize_static (cudaError {err.value})" if err.value else "evis_voxelize_static")
 
 
 def decode_events8(ev8: np.ndarray, keyframe_dt: float, substeps: int, kf: int = 0) -> np.ndarray:

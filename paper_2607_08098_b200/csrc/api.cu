@@ -460,6 +460,7 @@ const char *evis_strerror(int s)
         case EVIS_ERR_OVERFLOW: return "event capacity exceeded";
         case EVIS_ERR_MOTION_BOUND: return "motion vector exceeds max_motion_px";
         case EVIS_ERR_BAD_STATE: return "call order violated";
+        case EVIS_ERR_TOO_LARGE: return "grid larger than the fixed accumulator of evis_voxelize_static";
         default: return "unknown status";
     }
 }

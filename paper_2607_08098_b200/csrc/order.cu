@@ -6,6 +6,8 @@
 // are laid out in directory order: exclusive scan of the counts (three small kernels) and a
 // chunk-by-chunk 128-bit copy.  Inside a chunk the order is the block scan order of the producer
 // (pixel rank in the tile, then crossing index k), which is deterministic as well.
+#include <mutex>
+
 #include "kernels.h"
 
 namespace evis {
@@ -345,4 +347,97 @@ cudaError_t launch_voxel_finish(const unsigned long long *v, float *out, uint32_
     return cudaGetLastError();
 }
 
+// ---- evis_voxelize_static: the voxel grid of a finished event stream, with no device allocation (include/evis.h) ------
+//
+// For callers that must not allocate on the device while they run: a rollout loop whose simulator, renderer and learner
+// have divided the GPU's memory among their own pools up front (a cudaMalloc there can fail, and cudaMalloc / cudaFree
+// make every stream of the device wait), or a consumer that holds events but no evis_ctx.  evis_set_voxels allocates its
+// accumulator; this entry point keeps ONE accumulator of fixed size in the library's image instead.
+//
+// g_voxel_static is that accumulator (scratch: 32.32 fixed-point sums, like evis_ctx::vox_v): every GPU that loads the
+// library holds its EVIS_VOXELIZE_STATIC_MAX_CELLS * 8 bytes = 16 MiB from the moment the module is loaded until the
+// process exits.  In HOST code the name g_voxel_static is only a handle for the runtime, not a device address (a kernel
+// handed it would fault or touch the wrong memory): voxel_static_address() asks the runtime for the address on the
+// current device, once per device, and the kernels get that pointer.
+__device__ __align__(256) static unsigned long long g_voxel_static[EVIS_VOXELIZE_STATIC_MAX_CELLS];
+
+constexpr int VOXEL_STATIC_MAX_DEVICES = 64;
+static unsigned long long *g_voxel_static_ptr[VOXEL_STATIC_MAX_DEVICES];      // per device ordinal; null = not asked yet
+static std::mutex g_voxel_static_mu;
+
+// device address of g_voxel_static on the CURRENT device (set-up on the first call per device)
+static cudaError_t voxel_static_address(unsigned long long **out)
+{
+    int dev = -1;
+    cudaError_t rc = cudaGetDevice(&dev);
+    if (rc != cudaSuccess) return rc;
+    if (dev < 0 || dev >= VOXEL_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_voxel_static_mu);
+    if (!g_voxel_static_ptr[dev]) {
+        unsigned long long *p = nullptr;
+        rc = cudaGetSymbolAddress(reinterpret_cast<void **>(&p), g_voxel_static);
+        if (rc != cudaSuccess) return rc;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_voxel_static_ptr[dev] = p;
+    }
+    *out = g_voxel_static_ptr[dev];
+    return cudaSuccess;
+}
+
+// The accumulation of k_expand / k_dir_copy (voxel_add) as a kernel of its own over finished 16-byte events: the
+// event's interval index places it in the window, t = (kf - first_kf) T + t_off.  Events outside the window, the
+// frame or the env range add nothing.
+__global__ void __launch_bounds__(256)
+k_voxel_events(const uint4 *__restrict__ events, unsigned long long n, uint32_t E, uint32_t first_kf, uint32_t window_steps,
+               float T, const VoxelSink vox)
+{
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint4 ev = __ldcs(events + i);              // x | y << 16, env | p << 16 | substep << 24, t_off, kf
+        const uint32_t j = ev.w - first_kf;
+        if (j >= window_steps || (ev.x & 0xFFFFu) >= vox.wc || (ev.x >> 16) >= vox.hc || (ev.y & 0xFFFFu) >= E) continue;
+        VoxelSink v = vox;
+        v.t_base = __fmul_rn((float)j, T);
+        voxel_add(v, ev.x, ev.y, __uint_as_float(ev.z));
+    }
+}
+
 }  // namespace evis
+
+extern "C" int evis_voxelize_static(const evis_event *events, uint64_t n_events, int32_t num_envs, int32_t height, int32_t width,
+                                    int32_t bins, int32_t window_steps, float keyframe_dt, uint32_t first_kf, int normalize,
+                                    float *grid, void *cuda_stream, int *cuda_error)
+{
+    using namespace evis;
+    if (cuda_error) *cuda_error = 0;
+    if (!grid || (!events && n_events) || num_envs <= 0 || num_envs > 65535 || height <= 0 || height > 32767 || width <= 0 ||
+        width > 32767 || bins < 1 || window_steps < 1 || !(keyframe_dt > 0.0f) || !(keyframe_dt <= 3.0e38f))
+        return EVIS_ERR_INVALID_ARG;
+    const unsigned long long plane = (unsigned long long)height * (unsigned long long)width;
+    const unsigned long long planes = 2ull * (unsigned long long)num_envs * (unsigned long long)bins;     // < 2^48
+    if (planes > EVIS_VOXELIZE_STATIC_MAX_CELLS || plane * planes > EVIS_VOXELIZE_STATIC_MAX_CELLS) return EVIS_ERR_TOO_LARGE;
+    const unsigned long long cells = plane * planes;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned long long *acc = nullptr;
+    cudaError_t rc = voxel_static_address(&acc);
+    // the array keeps what the last call left in it: the part this call uses starts at zero
+    if (rc == cudaSuccess) rc = cudaMemsetAsync(acc, 0, cells * sizeof(unsigned long long), st);
+    if (rc == cudaSuccess && n_events) {
+        VoxelSink vs{};
+        vs.v = acc;
+        vs.bins = (uint32_t)bins; vs.hc = (uint32_t)height; vs.wc = (uint32_t)width;
+        volatile float sc = (float)(bins - 1) / ((float)window_steps * keyframe_dt);      // as evis_step forms it
+        vs.scale = sc;
+        const unsigned long long want = (n_events + 255ull) / 256ull;
+        const unsigned blocks = (unsigned)(want < 148ull * 16ull ? want : 148ull * 16ull);
+        k_voxel_events<<<blocks, 256, 0, st>>>(reinterpret_cast<const uint4 *>(events), n_events, (uint32_t)num_envs, first_kf,
+                                               (uint32_t)window_steps, keyframe_dt, vs);
+        rc = cudaGetLastError();
+    }
+    if (rc == cudaSuccess) rc = launch_voxel_finish(acc, grid, (uint32_t)planes, (uint32_t)plane, normalize, st);
+    if (rc != cudaSuccess) {
+        if (cuda_error) *cuda_error = (int)rc;
+        return EVIS_ERR_CUDA;
+    }
+    return EVIS_OK;
+}
