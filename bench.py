@@ -338,12 +338,19 @@ def run_ours(args, spec) -> None:
     for k in range(Wm + 1):
         step(k)
     torch.cuda.synchronize(dev)
+    j0 = ev.info()
     ev.profile_enable(True)
     for k in range(Wm + 1, Wm + 1 + K):
         step(k)
     prof = ev.profile_read()
     ev.profile_enable(False)
+    j1 = ev.info()
     ev.destroy()
+    # the same keyframes must give the same events: the timed pass runs fully asynchronously (regions' streams not joined,
+    # the host far ahead), this pass with every region joined to the caller's stream
+    if j1.total_events - j0.total_events != events:
+        raise SystemExit(f"bench.py: the timed pass produced {events} events, the stage-timed pass over the same keyframes "
+                         f"{j1.total_events - j0.total_events}: the asynchronous schedule is not deterministic")
 
     (ms,), (events, launches) = sharding.reduce_max_sum([ms], [float(events), float(launches)], dev)
     launches = int(launches)

@@ -523,6 +523,13 @@ static int step_enqueue(evis_ctx *ctx, const float *rad, const float *mv_bwd, co
     B.has_fwd = mv_fwd != nullptr;
     const bool first = ctx->steps == 0;
     if (ctx->prof_on) { ctx->prof_acc.steps += 1; if (ctx->prof_spans.size() > 8192) prof_drain(ctx); }
+    // slot of this step's arrival buffer, directory and per-step counters; the order stage that used it last
+    // (two steps ago with overlap, the last step without) must be done before it is cleared.  The same wait guards the
+    // keyframe buffers, so it comes BEFORE the prep: kf[cur] was keyframe A of the step two steps ago, whose chunk kernels
+    // run on the regions' streams and are not joined to `st`; that step's order stage started after them, so once it is
+    // done nothing reads kf[cur] (or lin[cur]) any more.  The prep of step k + 1 still runs under step k's chunk kernels.
+    const int sl = ctx->overlap ? (int)(ctx->steps & 1) : 0;
+    if (ctx->ord_pending[sl]) CU(cudaStreamWaitEvent(st, ctx->ev_order[sl], 0));
     {
         Span sp(ctx, st, EVIS_STAGE_PREP, 1);
         CU(launch_prep(rad, mv_bwd, mv_fwd, depth, (long long)P, ctx->cfg.log_eps, ctx->channel_set ? ctx->channel : -1, B.L, B.mv, B.fwd, B.Z,
@@ -545,11 +552,7 @@ static int step_enqueue(evis_ctx *ctx, const float *rad, const float *mv_bwd, co
     }
 
     ctx->ep.kf = ctx->kf_next;
-    // slot of this step's arrival buffer, directory and per-step counters; the order stage that used it last
-    // (two steps ago with overlap, the last step without) must be done before it is cleared
-    const int sl = ctx->overlap ? (int)(ctx->steps & 1) : 0;
     unsigned long long *cnt = ctx->counters_s[sl];
-    if (ctx->ord_pending[sl]) CU(cudaStreamWaitEvent(st, ctx->ev_order[sl], 0));
     EventSink sink{ctx->arrival_s[sl], ctx->arrival_cap, cnt + C_ALLOC, cnt + C_EVENTS, ctx->directory_s[sl]};
     const Thresholds th{ctx->th_active ? ctx->th_on : nullptr, ctx->th_active ? ctx->th_off : nullptr};
     // direct mode (the resolve kernel writes events) serves the refractory period and the noise events
@@ -576,7 +579,7 @@ static int step_enqueue(evis_ctx *ctx, const float *rad, const float *mv_bwd, co
     // The regions' streams do NOT join `st` again (unless the stage timers are on or EVIS_NO_OVERLAP=1): the order stream
     // waits for them instead, and every call that returns results waits for the order stream.  `st` is then free to run
     // the NEXT step's prep (HBM-bound, into the third keyframe buffer) under this step's chunk kernels; it cannot run
-    // further ahead than that, because a step's clears wait for the order stage of two steps before (ev_order).
+    // further ahead than that, because a step's prep waits for the order stage of two steps before (ev_order, above).
     const bool join_st = !ctx->overlap || ctx->prof_on || capturing;
     {
         // nreg > 1: the env chunks are dealt round-robin to the regions' streams, which fork from `st` here; the

@@ -503,6 +503,47 @@ def test_back_to_back_steps_overlap_the_order_stage(path, monkeypatch):
         assert np.array_equal(a[3][0], other[3][0]) and np.array_equal(a[3][1], other[3][1])
 
 
+@pytest.mark.parametrize("variant", ["plain", "defocus", "weighted"])
+def test_steps_enqueued_far_ahead_keep_their_keyframes(variant, monkeypatch):
+    """Several z-buffer regions (24 envs at cfg 4's 346 x 260: one env per chunk, four regions on four streams that do
+    not join the caller's stream) and a host that runs far ahead of the GPU: the stream is held up by a spin kernel while
+    six steps are enqueued without any synchronisation.  Step k + 2's prep overwrites the keyframe buffer that was A of
+    step k; it must wait for step k's chunk kernels on the regions' streams.  The last step's events, the event total,
+    the holes and the carried state must equal those of the same steps synchronised one by one and of a context with the
+    overlap switched off (EVIS_NO_OVERLAP=1).  Also with defocus (the linear keyframes rotate the same way) and the
+    weighted splat."""
+    spec = scenes.small(scenes.config(4), num_envs=24, num_keyframes=7)
+    assert (spec.height, spec.width) == (260, 346)
+    sc = scenes.make_scene(spec)
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(7)]
+    torch.cuda.synchronize()
+
+    def run(sync_each):
+        ev = binding.Evis(spec.num_envs, spec.height, spec.width, spec.substeps, spec.c_pos, spec.c_neg, spec.log_eps,
+                          spec.keyframe_dt, max_motion_px=spec.max_motion_px(), event_capacity=1 << 24,
+                          composite_mode=binding.COMPOSITE_WEIGHTED if variant == "weighted" else 0)
+        if variant == "defocus":
+            ev.set_defocus(0.5)
+        if not sync_each:
+            torch.cuda._sleep(400_000_000)             # ~0.2 s: every step below is enqueued before the first one runs
+        for kf in kfs:
+            ev.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=sync_each)
+        last = ev.read_events().copy()
+        info = ev.info()
+        state = ev.get_state()
+        ev.destroy()
+        return last, info.total_events, info.last_holes, state
+
+    a = run(False)
+    b = run(True)
+    monkeypatch.setenv("EVIS_NO_OVERLAP", "1")
+    c = run(False)
+    for other in (b, c):
+        assert a[1] == other[1] and a[2] == other[2], (a[1], other[1])
+        assert len(a[0]) > 0 and np.array_equal(a[0], other[0])
+        assert np.array_equal(a[3][0], other[3][0]) and np.array_equal(a[3][1], other[3][1])
+
+
 @pytest.mark.parametrize("use_fwd", [True, False])
 def test_degenerate_inputs(use_fwd):
     """Inputs the readings R3, R17 and R18 cover: negative, NaN and infinite radiance (luminance clamps to 0, NaN -> 0);
