@@ -190,6 +190,13 @@ int evis_set_noise(evis_ctx *ctx, const evis_noise *noise, const uint8_t *hot_ma
  * events carry the original indices and a noise run draws the same noise events.  Errors: INVALID_ARG. */
 int evis_set_interval_index(evis_ctx *ctx, uint32_t next_kf);
 
+/* Env sharding: this context holds the environments [first_env, first_env + num_envs) of a larger
+ * batch (0 = the default: it holds the batch's first environments).  The noise generator is keyed by the environment's
+ * index in the WHOLE batch (R29), so with the offset set a shard draws exactly the noise events the single context of the
+ * whole batch draws for those environments.  Events keep the context's LOCAL env index (add first_env to get the batch's).
+ * Applies from the next evis_step on.  Errors: INVALID_ARG (first_env + num_envs > 2^32). */
+int evis_set_env_offset(evis_ctx *ctx, uint32_t first_env);
+
 /* Colour events ("Replacing I with individual R, G, B channels and applying the event model to each
  * independently produces color events"; R28): channel = 0, 1 or 2 makes this context take
  * L = log(channel + eps) of the radiance's R, G or B instead of the Rec.709 luminance; -1 = luminance (default).

@@ -58,7 +58,7 @@ SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "ev
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
            "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end",
            "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus", "evis_set_time_sorted", "evis_set_compact_events", "evis_read_events8", "evis_read_events8_begin",
-           "evis_voxelize_static"]
+           "evis_voxelize_static", "evis_set_env_offset"]
 
 _lib = None
 
@@ -92,6 +92,7 @@ def load() -> C.CDLL:
     L.evis_set_margin.argtypes = [vp, C.c_int]
     L.evis_set_channel.argtypes = [vp, C.c_int]
     L.evis_set_interval_index.argtypes = [vp, C.c_uint32]
+    L.evis_set_env_offset.argtypes = [vp, C.c_uint32]
     L.evis_wait_events.argtypes = [vp, vp]
     L.evis_read_events_begin.argtypes = [vp, vp, C.c_uint64, u64p]
     L.evis_read_events_end.argtypes = [vp]
@@ -281,6 +282,10 @@ class Evis:
     def set_interval_index(self, next_kf: int) -> None:
         """evis_set_interval_index: the index the next closed interval gets (checkpoint / resume)."""
         _check(self._lib.evis_set_interval_index(self._ctx, int(next_kf)), "evis_set_interval_index")
+
+    def set_env_offset(self, first_env: int) -> None:
+        """evis_set_env_offset: this context holds envs [first_env, first_env + E) of a larger batch (keys the noise events)."""
+        _check(self._lib.evis_set_env_offset(self._ctx, int(first_env)), "evis_set_env_offset")
 
     def set_margin(self, margin: int) -> None:
         """evis_set_margin: the frames carry `margin` over-rendered pixels per side, cropped after the warp."""

@@ -118,6 +118,7 @@ struct evis_ctx {
 
     uint64_t steps, launches, device_bytes;
     uint32_t kf_next;                 // index the next closed interval gets (evis_set_interval_index)
+    uint32_t env_offset;              // index of this context's env 0 in the whole batch (evis_set_env_offset): noise keys
     uint64_t last_events, last_holes;
     int last_overflow, last_motion;
     bool have_events;
@@ -564,7 +565,9 @@ static int step_enqueue(evis_ctx *ctx, const float *rad, const float *mv_bwd, co
         // P = r dt, binary32 products of the rates and T / S (R29); the per-step part of the generator keys
         volatile float pl = ctx->noise.r_leak * ctx->ep.dt, ps = ctx->noise.r_shot * ctx->ep.dt, ph = ctx->noise.r_hot * ctx->ep.dt;
         rf.noise_on = 1;
-        rf.noise_key = host_mix64(ctx->noise.seed ^ (0x9E3779B97F4A7C15ull * ((unsigned long long)ctx->ep.kf + 1ull)));
+        // the kernel keys env e of this context with mix64(noise_key + e): a shard's first env sits at env_offset of the batch
+        rf.noise_key = host_mix64(ctx->noise.seed ^ (0x9E3779B97F4A7C15ull * ((unsigned long long)ctx->ep.kf + 1ull))) +
+                       (unsigned long long)ctx->env_offset;
         rf.p_leak = pl; rf.p_shot = ps; rf.p_hot = ph;
         rf.i_white = ctx->noise.i_white;
         rf.eps = ctx->cfg.log_eps;
@@ -1012,6 +1015,13 @@ int evis_set_interval_index(evis_ctx *ctx, uint32_t next_kf)
 {
     if (!ctx) return EVIS_ERR_INVALID_ARG;
     ctx->kf_next = next_kf;
+    return EVIS_OK;
+}
+
+int evis_set_env_offset(evis_ctx *ctx, uint32_t first_env)
+{
+    if (!ctx || (unsigned long long)first_env + (unsigned long long)ctx->g.E > 0x100000000ull) return EVIS_ERR_INVALID_ARG;
+    ctx->env_offset = first_env;
     return EVIS_OK;
 }
 

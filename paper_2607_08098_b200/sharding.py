@@ -57,7 +57,8 @@ class ShardedEvis:
     own event stream; there is no exchange step (the envs are batched for efficiency only).
 
     ``step`` takes the rank's SLICE of the keyframe (``[e0:e1]`` of the batch tensors); events carry LOCAL env indices,
-    ``global_env`` maps them back.  ``rank`` / ``world`` default to the process group's (1 rank without one), so the same
+    ``global_env`` maps them back.  Noise events (``ctx.set_noise``) are keyed by the env's index in the whole batch
+    (``evis_set_env_offset``), so the shards draw what the single context would; a hot-pixel mask is the rank's slice.  ``rank`` / ``world`` default to the process group's (1 rank without one), so the same
     code runs under ``torchrun`` and in a single process; passing them explicitly builds one shard by hand.
     """
 
@@ -77,6 +78,7 @@ class ShardedEvis:
         self.device = torch.device("cuda", device)
         self.ctx = binding.Evis(self.e1 - self.e0, height, width, substeps, c_pos, c_neg, log_eps, keyframe_dt,
                                 device=device, **kw)
+        self.ctx.set_env_offset(self.e0)          # noise events are keyed by the env's index in the whole batch
 
     def local(self, batch_tensor: torch.Tensor) -> torch.Tensor:
         """This rank's slice of a tensor that holds the whole batch (env-major)."""

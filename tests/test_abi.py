@@ -53,6 +53,7 @@ def test_argument_validation_needs_no_gpu(lib):
     assert lib.evis_step(None, None, None, None, None, None, None) == binding.EVIS_ERR_INVALID_ARG
     assert lib.evis_read_events(None, None, 0, 0, None) == binding.EVIS_ERR_INVALID_ARG
     assert lib.evis_get_info(None, None) == binding.EVIS_ERR_INVALID_ARG
+    assert lib.evis_set_env_offset(None, 0) == binding.EVIS_ERR_INVALID_ARG
     assert lib.evis_destroy(None) == binding.EVIS_OK
     assert lib.evis_strerror(binding.EVIS_ERR_OVERFLOW) == b"event capacity exceeded"
     assert b"sm_100a" in lib.evis_version()

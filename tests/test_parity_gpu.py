@@ -1043,10 +1043,11 @@ def test_defocus_api_contract():
 # env-sharded multi-GPU entry; one GPU here, so the two shards run one after the other
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.gpu
-@pytest.mark.parametrize("world", [2, 3])
-def test_env_shards_reproduce_the_single_context_stream(world):
+@pytest.mark.parametrize("world,noise", [(2, False), (3, False), (2, True), (3, True)])
+def test_env_shards_reproduce_the_single_context_stream(world, noise):
     """sharding.ShardedEvis: the union of the ranks' event streams (local env + e0) is the single-context stream of the
-    whole batch, event for event and bit for bit, and the carried state is the slice of the single context's."""
+    whole batch, event for event and bit for bit, and the carried state is the slice of the single context's.  With the
+    noise events on as well: their generator is keyed by the env's index in the whole batch (evis_set_env_offset)."""
     from paper_2607_08098_b200 import sharding
     spec = scenes.small(scenes.config(4), num_envs=5, height=70, width=93, num_keyframes=4)
     sc = scenes.make_scene(spec)
@@ -1055,7 +1056,11 @@ def test_env_shards_reproduce_the_single_context_stream(world):
     kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(spec.num_keyframes)]
     key = lambda e: np.sort(e, order=["kf", "env", "substep", "y", "x", "t_off"])
 
+    hot = (torch.rand((E, H, W), generator=torch.Generator().manual_seed(5)) < 0.01).to(torch.uint8).cuda()
+    nz = dict(seed=1234, r_leak=40.0, r_shot=60.0, r_hot=500.0, i_white=50.0)
     one = binding.Evis(E, *args, event_capacity=1 << 22)
+    if noise:
+        one.set_noise(hot=hot, **nz)
     ref = []
     for kf in kfs:
         one.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
@@ -1068,6 +1073,8 @@ def test_env_shards_reproduce_the_single_context_stream(world):
     for rank in range(world):
         sh = sharding.ShardedEvis(E, *args, rank=rank, world=world, event_capacity=1 << 22)
         covered += list(range(sh.e0, sh.e1))
+        if noise:
+            sh.ctx.set_noise(hot=sh.local(hot), **nz)
         for k, kf in enumerate(kfs):
             if k % 2:          # either the rank slices the batch tensors, or it renders its own envs
                 loc = {a: sh.local(b) for a, b in kf.items()}
