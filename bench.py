@@ -400,10 +400,11 @@ def run_ours(args, spec) -> None:
            "x_realtime": spec.keyframe_dt / (ms / K * 1e-3),
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
 
-    # ---- e2e: HOST buffers through evis_step_host; every step uploads its keyframe from pinned memory and downloads
-    #      its result.  Two arms: the result is (a) the per-polarity accumulation image of the step (evis_set_voxels,
-    #      bins = 1, no 16-byte event leaves the GPU) -- `e2e` --, (b) the full ordered event stream -- `e2e_events`.
-    #      The upload of step k + 1 overlaps the kernels of step k (two staging sets) and the download of step k.
+    # ---- e2e: HOST buffers through evis_step_host; every step uploads its keyframe from pinned memory and downloads its
+    #      result into pinned memory.  `e2e` = the hot path's product, the ordered event stream (8-byte compact events, inside
+    #      north_star's stamp tolerance); `e2e_events16` = the same stream as 16-byte events; `e2e_voxels` = the per-polarity
+    #      accumulation image (no event leaves the GPU).  Upload of keyframe k + 1, kernels of step k and download of step
+    #      k - 1 run concurrently (two staging sets, doubled ordered stream, deferred read).
     if not args.no_e2e and not args.profile_range:
         Ke = max(1, min(args.e2e_steps, K))
         hk = []
@@ -415,64 +416,75 @@ def run_ours(args, spec) -> None:
 
         def e2e_arm(voxels: bool, compact: bool = False):
             ev = mk()
-            if compact:
-                ev.set_compact_events(True)
-                hcap = int(min(cap, 2 * ev_per_step + (1 << 20)))
-                hbufs = [torch.empty(hcap, dtype=torch.int64).pin_memory() for _ in range(2)]
-                harrs = [hb.numpy().view(np.uint64) for hb in hbufs]
-            elif voxels:
+            esize = 8 if compact else 16
+            if voxels:
                 ev.set_voxels(1, window_steps=1, keep_events=False)
                 nel = int(np.prod(ev.voxel_shape()))
                 hbufs = [torch.empty(nel, dtype=torch.float32).pin_memory() for _ in range(2)]
                 harrs = [hb.numpy() for hb in hbufs]
             else:
+                if compact:
+                    ev.set_compact_events(True)
                 hcap = int(min(cap, 2 * ev_per_step + (1 << 20)))
-                hbufs = [torch.empty((hcap, 16), dtype=torch.uint8).pin_memory() for _ in range(2)]
-                harrs = [hb.numpy().view(binding.EVENT_DTYPE).reshape(-1) for hb in hbufs]
+                hbufs = [torch.empty(hcap * esize, dtype=torch.uint8).pin_memory() for _ in range(2)]
+                harrs = [hb.numpy().view(np.uint64 if compact else binding.EVENT_DTYPE) for hb in hbufs]
             for k in range(Wm + 1):
                 f = hk[k]
                 ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
             barrier()
             tt0 = time.perf_counter()
-            got = 0
-            for k in range(Wm + 1, Wm + 1 + Ke):
+            got, pending, n_last = 0, False, 0
+            first = Wm + 1
+            for k in range(first, first + Ke):
                 f = hk[k]
+                # enqueue only: this keyframe's upload starts while the previous step still computes
+                ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"], sync=False)
                 if voxels:
-                    ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"], sync=False)
                     ev.read_voxels_begin(harrs[k & 1])             # ends the previous copy first
                     got += harrs[0].nbytes
-                else:
-                    n_step = ev.step_host(f["rad"], f["mv_bwd"], f["depth"], f["mv_fwd"])
-                    n_copy = (ev.read_events8_begin if compact else ev.read_events_begin)(harrs[k & 1])   # ends the previous copy first
-                    if n_copy != n_step:
-                        raise SystemExit("bench.py: e2e host buffer too small for a step's events")
-                    got += (8 if compact else 16) * n_copy
+                elif k > first:
+                    if pending:                                    # the stream of step k - 2 has arrived
+                        got += esize * ev.read_events_finish()
+                    # step k is enqueued: wait for step k - 1 alone and start copying its stream
+                    ev.read_events_enqueue(harrs[(k - 1) & 1], previous_step=True)
+                    pending = True
             if voxels:
                 ev.read_voxels_end()
             else:
-                ev.read_events_end()
+                if pending:
+                    got += esize * ev.read_events_finish()
+                ev.read_events_enqueue(harrs[(first + Ke - 1) & 1])   # the last step of the timed region
+                n_last = ev.read_events_finish()
+                got += esize * n_last
             barrier()
             dt = time.perf_counter() - tt0
-            if voxels:                                                # (outside the timed region) the last image really arrived:
+            # (outside the timed region) the last result really arrived
+            if voxels:
                 total = float(harrs[(Wm + Ke) & 1].sum(dtype=np.float64))             # one unit per event
                 if abs(total - ev.info().last_events) > 0.5:
                     raise SystemExit("bench.py: the downloaded accumulation image does not hold the step's events")
+            else:
+                last = harrs[(Wm + Ke) & 1][:n_last]
+                envs = ((last >> np.uint64(24)) & np.uint64(0xFFFF)) if compact else last["env"]
+                if n_last != ev.info().last_events or n_last >= hcap or int(envs.max()) != E - 1 or np.any(np.diff(envs.astype(np.int64)) < 0):
+                    raise SystemExit("bench.py: the downloaded event stream is not the step's ordered stream")
             ev.destroy()
             (dt,), _ = sharding.reduce_max_sum([dt], [], dev)
             return {"value": global_envs * H * W * S * Ke / dt, "unit": METRIC, "steps": Ke,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(got / Ke), "ms_per_step": dt / Ke * 1e3,
                     "x_realtime": spec.keyframe_dt / (dt / Ke)}
 
-        out["e2e"] = dict(e2e_arm(True), result="per-polarity accumulation image of the step [E,2,1,H,W] float32 "
-                          "(evis_set_voxels bins=1, keep_events=0)",
-                          api="evis_step_host (pinned host keyframes, upload overlapping the previous step) + "
-                              "evis_read_voxels_begin / _end (pinned host image, overlapping the next upload)")
-        out["e2e_events8"] = dict(e2e_arm(False, compact=True), result="the full ordered event stream as 8-byte compact events "
-                                  "(evis_set_compact_events; stamps within T/S * 2^-16)",
-                                  api="evis_step_host + evis_read_events8_begin / evis_read_events_end")
-        out["e2e_events"] = dict(e2e_arm(False), result="the full ordered event stream, 16 B per event",
-                                 api="evis_step_host (pinned host keyframes) + evis_read_events_begin / _end (pinned host "
-                                     "stream, overlapping the next upload)")
+        ev_api = ("evis_step_host with n_events = NULL (pinned host keyframes; the upload of keyframe k + 1 overlaps step k) + "
+                  "evis_read_events_enqueue(previous_step) / _finish (pinned host stream: the stream of step k - 1 is copied out "
+                  "after step k has been enqueued, waiting for step k - 1 only)")
+        out["e2e"] = dict(e2e_arm(False, compact=True), result="the full ordered event stream (env, x, y, substep, polarity exact; the "
+                          "stamp within T/S * 2^-16 = 1.6e-8 s, inside north_star's 1e-7 s) as 8-byte compact events "
+                          "(evis_set_compact_events)", api=ev_api)
+        out["e2e_events16"] = dict(e2e_arm(False), result="the full ordered event stream, 16 B per event (binary32 stamps)", api=ev_api)
+        out["e2e_voxels"] = dict(e2e_arm(True), result="per-polarity accumulation image of the step [E,2,1,H,W] float32 "
+                                 "(evis_set_voxels bins=1, keep_events=0)",
+                                 api="evis_step_host with n_events = NULL + evis_read_voxels_begin / _end (pinned host image, "
+                                     "overlapping the next upload)")
 
     if rank == 0 and not args.no_cpu and not args.profile_range:
         out["cpu_baseline"] = cpu_baseline(scenes.small(spec, seed=spec.seed - 1000 * rank), args.cpu_seconds)

@@ -348,6 +348,24 @@ int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t
 int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, uint64_t *n_out);
 int evis_read_events_end(evis_ctx *ctx);
 
+/* The same copy for a PIPELINED loop: with previous_step != 0 the call copies the stream of the step BEFORE the last
+ * evis_step / evis_step_host call -- still intact, because the ordered stream is double-buffered inside the context -- and
+ * waits only for THAT step, not for the one enqueued after it.  So in
+ *     evis_step_host(k + 1, n_events = NULL);  evis_read_events_finish(&n) [step k - 1];  evis_read_events_enqueue(buf[k & 1], max, 1) [step k]
+ * the upload of keyframe k + 1, the kernels of step k and the download of step k - 1 are in flight together, while the
+ * read calls above must wait for the last step before the next one can be enqueued.  _enqueue waits for the chosen step's
+ * ordering stage, starts the copy of min(stored, max) events on a stream of the library's own and returns; _finish waits
+ * for the copy and returns that number.  previous_step = 0: the last step, like evis_read_events_begin.  `pinned_dst`:
+ * page-locked HOST memory (cudaHostAlloc / cudaHostRegister; e.g. a pinned torch tensor) with room for `max` events of
+ * the stored format (16-byte evis_event, or 8-byte evis_event8 after evis_set_compact_events), untouched until _finish.
+ * One deferred copy at a time: _enqueue first waits for an unfinished earlier copy.  The ordering stage of step k + 2
+ * waits for the copy of step k (they share a buffer).
+ * Errors: INVALID_ARG (NULL or pageable memory), BAD_STATE (no stored stream; previous_step before two intervals have
+ * been closed, or with EVIS_NO_OVERLAP=1 / EVIS_GRAPH=1; _finish without _enqueue), CUDA; _finish returns OVERFLOW when
+ * that step overflowed (the valid prefix, if any, has been copied). */
+int evis_read_events_enqueue(evis_ctx *ctx, void *pinned_dst, uint64_t max, int previous_step);
+int evis_read_events_finish(evis_ctx *ctx, uint64_t *n_out);
+
 /* Device pointer to the ordered stream of the last step and its stored length (no copy);
  * valid until the next evis_step on the same context. */
 int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_stored);

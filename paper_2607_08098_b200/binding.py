@@ -58,7 +58,8 @@ SYMBOLS = ["evis_create", "evis_step", "evis_step_host", "evis_read_events", "ev
            "evis_get_info", "evis_profile_enable", "evis_profile_read", "evis_get_state", "evis_set_state", "evis_debug_read", "evis_destroy",
            "evis_strerror", "evis_last_cuda_error", "evis_version", "evis_set_thresholds", "evis_set_refractory", "evis_set_margin", "evis_set_channel", "evis_set_noise", "evis_wait_events", "evis_refractory_state", "evis_read_events_begin", "evis_read_events_end",
            "evis_set_interval_index", "evis_set_voxels", "evis_read_voxels", "evis_read_voxels_begin", "evis_read_voxels_end", "evis_set_defocus", "evis_set_time_sorted", "evis_set_compact_events", "evis_read_events8", "evis_read_events8_begin",
-           "evis_voxelize_static", "evis_set_env_offset"]
+           "evis_voxelize_static", "evis_set_env_offset",
+           "evis_read_events_enqueue", "evis_read_events_finish"]
 
 _lib = None
 
@@ -96,6 +97,8 @@ def load() -> C.CDLL:
     L.evis_wait_events.argtypes = [vp, vp]
     L.evis_read_events_begin.argtypes = [vp, vp, C.c_uint64, u64p]
     L.evis_read_events_end.argtypes = [vp]
+    L.evis_read_events_enqueue.argtypes = [vp, vp, C.c_uint64, C.c_int]
+    L.evis_read_events_finish.argtypes = [vp, u64p]
     L.evis_refractory_state.argtypes = [vp, vp, vp]
     L.evis_set_noise.argtypes = [vp, C.POINTER(evis_noise), vp, C.c_int]
     L.evis_set_voxels.argtypes = [vp, C.POINTER(evis_voxel_config)]
@@ -339,6 +342,19 @@ class Evis:
         got = C.c_uint64(0)
         _check(self._lib.evis_read_events_begin(self._ctx, host_buf.ctypes.data, host_buf.shape[0], C.byref(got)),
                "evis_read_events_begin")
+        return int(got.value)
+
+    def read_events_enqueue(self, pinned_buf: np.ndarray, previous_step: bool = False) -> None:
+        """evis_read_events_enqueue: start copying the stored stream of the last step -- or, with ``previous_step``, of the step
+        before it, waiting only for that one (the pipelined loop) -- into a PINNED host array (EVENT_DTYPE, or uint64 with
+        compact events); ``read_events_finish`` waits for the copy and returns how many events arrived."""
+        assert pinned_buf.flags.c_contiguous and pinned_buf.dtype.itemsize in (8, 16)
+        _check(self._lib.evis_read_events_enqueue(self._ctx, pinned_buf.ctypes.data, pinned_buf.shape[0], int(bool(previous_step))),
+               "evis_read_events_enqueue")
+
+    def read_events_finish(self, allow=()) -> int:
+        got = C.c_uint64(0)
+        _check(self._lib.evis_read_events_finish(self._ctx, C.byref(got)), "evis_read_events_finish", allow)
         return int(got.value)
 
     def read_events_end(self) -> None:

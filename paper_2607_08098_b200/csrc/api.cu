@@ -65,6 +65,16 @@ struct evis_ctx {
     cudaStream_t copy_stream;         // evis_read_events_begin: device -> host copy of the ordered stream
     cudaEvent_t ev_copy;
     bool copy_pending;
+    // `ordered` is doubled like the arrival buffers (slot = step & 1; one buffer without the overlap), so that the order
+    // stage of step k + 1 does not wait for step k's stream to be copied out.  copy_slot: the slot the pending copy
+    // reads (-1: the voxel image).  h_copy (pinned): [0], [1] = events copied and overflow code of the deferred read;
+    // from H_SLOT + slot * H_SLOT_WORDS on, a mirror of each slot's per-step counters C_EVENTS .. C_ALLOC (the deferred read
+    // of the step before the last needs that step's counts while h_counters already belongs to the last step).
+    uint4 *ordered_s[2];
+    int copy_slot;
+    bool deferred;
+    unsigned long long *h_copy;
+    static constexpr int H_SLOT = 8, H_SLOT_WORDS = 40;
     cudaEvent_t ev_chunks[2], ev_order[2];
     bool ord_pending[2];
     bool overlap;
@@ -252,6 +262,8 @@ void free_all(evis_ctx *ctx)
     if (ctx->arrival_s[1] != ctx->arrival_s[0]) {
         cudaFree(ctx->arrival_s[1]); cudaFree(ctx->directory_s[1]); cudaFree(ctx->counters_s[1]);
     }
+    if (ctx->ordered_s[1] != ctx->ordered_s[0]) cudaFree(ctx->ordered_s[1]);
+    if (ctx->h_copy) cudaFreeHost(ctx->h_copy);
     if (ctx->ord_stream) cudaStreamDestroy(ctx->ord_stream);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->ev_copy) cudaEventDestroy(ctx->ev_copy);
@@ -389,6 +401,11 @@ int create_impl(evis_ctx *ctx)
         ctx->overlap = !(no && no[0] == '1');
         ctx->arrival_s[0] = ctx->arrival; ctx->directory_s[0] = ctx->directory; ctx->counters_s[0] = ctx->counters;
         ctx->arrival_s[1] = ctx->arrival; ctx->directory_s[1] = ctx->directory; ctx->counters_s[1] = ctx->counters;
+        ctx->ordered_s[0] = ctx->ordered_s[1] = ctx->ordered;
+        if (ctx->overlap) CU(dalloc(ctx, &ctx->ordered_s[1], (size_t)c.event_capacity));
+        ctx->copy_slot = -1;
+        CU(cudaHostAlloc((void **)&ctx->h_copy, (evis_ctx::H_SLOT + 2 * evis_ctx::H_SLOT_WORDS) * sizeof(unsigned long long), cudaHostAllocDefault));
+        memset(ctx->h_copy, 0, (evis_ctx::H_SLOT + 2 * evis_ctx::H_SLOT_WORDS) * sizeof(unsigned long long));
         if (ctx->overlap) {
             CU(dalloc(ctx, &ctx->arrival_s[1], (size_t)ctx->arrival_cap));
             CU(dalloc(ctx, &ctx->directory_s[1], (size_t)ent));
@@ -662,7 +679,9 @@ static int step_enqueue(evis_ctx *ctx, const float *rad, const float *mv_bwd, co
     CU(cudaStreamWaitEvent(os, ctx->ev_chunks[sl], 0));
     if (ctx->nreg > 1 && !join_st)
         for (int r = 0; r < ctx->nreg; ++r) CU(cudaStreamWaitEvent(os, ctx->ev_join[r], 0));
-    if (ctx->copy_pending) CU(cudaStreamWaitEvent(os, ctx->ev_copy, 0));   // `ordered` is still being copied out
+    // this slot's `ordered` (or the voxel image) is still being copied out
+    if (ctx->copy_pending && (ctx->copy_slot < 0 || ctx->copy_slot == sl || ctx->ordered_s[0] == ctx->ordered_s[1]))
+        CU(cudaStreamWaitEvent(os, ctx->ev_copy, 0));
     VoxelSink vs{};
     vs.store_events = ctx->compact ? 2 : 1;
     vs.dt = ctx->ep.dt;
@@ -686,21 +705,23 @@ static int step_enqueue(evis_ctx *ctx, const float *rad, const float *mv_bwd, co
         unsigned long long *sticky = ctx->counters_s[0];             // C_MOTION, C_TOTAL live in slot 0's array
         if (!rf.t_last) {
             const uint32_t tx = (g.W + G_TILE_W - 1) / G_TILE_W, ty = (g.H + G_TILE_H - 1) / G_TILE_H;
-            CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
+            CU(launch_expand(sink, ctx->dir_entries, ctx->bsum, ctx->ordered_s[sl], ctx->cfg.event_capacity,
                              cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, ctx->ep, th, (uint32_t)g.W,
                              (uint32_t)g.HW, (uint32_t)g.margin, tx, tx * ty, (uint32_t)g.S, vs, os));
         } else {
-            CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered, ctx->cfg.event_capacity,
+            CU(launch_order(sink, ctx->dir_entries, ctx->bsum, ctx->ordered_s[sl], ctx->cfg.event_capacity,
                             cnt + C_EVENTS, sticky + C_TOTAL, sticky + C_OVERFLOW, vs, os));
         }
         if (ctx->time_sorted && vs.store_events == 1) {
             // the arrival buffer of this slot is free once the stream has been laid out: it is the sort's scratch
             CU(launch_time_sort(sink.directory, ctx->dir_entries, rf.t_last ? 0 : DIR_EV_SHIFT, (uint32_t)g.E,
                                 ctx->cfg.event_capacity < ctx->arrival_cap ? ctx->cfg.event_capacity : ctx->arrival_cap,
-                                ctx->ordered, ctx->arrival_s[sl], ctx->sort_ws, os));
+                                ctx->ordered_s[sl], ctx->arrival_s[sl], ctx->sort_ws, os));
             ctx->launches += 14;
         }
         CU(cudaMemcpyAsync(ctx->h_counters, cnt, C_STEP_END * sizeof(unsigned long long), cudaMemcpyDeviceToHost, os));
+        CU(cudaMemcpyAsync(ctx->h_copy + evis_ctx::H_SLOT + sl * evis_ctx::H_SLOT_WORDS, cnt, (C_ALLOC + 1) * sizeof(unsigned long long),
+                           cudaMemcpyDeviceToHost, os));
         CU(cudaMemcpyAsync(ctx->h_counters + C_MOTION, sticky + C_MOTION, (NCOUNTERS - C_MOTION) * sizeof(unsigned long long),
                            cudaMemcpyDeviceToHost, os));
     }
@@ -913,6 +934,7 @@ int evis_read_voxels_begin(evis_ctx *ctx, float *host_dst, int normalize, int re
     CU(cudaMemcpyAsync(host_dst, ctx->vox_out, ctx->vox_cells * sizeof(float), cudaMemcpyDeviceToHost, ctx->copy_stream));
     CU(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
     ctx->copy_pending = true;
+    ctx->copy_slot = -1;
     if (restart) ctx->vox_restart = true;
     return EVIS_OK;
 }
@@ -946,11 +968,12 @@ static int read_events8(evis_ctx *ctx, uint64_t *dst, int dst_is_device, uint64_
     uint64_t n = stored_events(ctx);
     if (n > max) n = max;
     if (n && !async)
-        CU(cudaMemcpy(dst, ctx->ordered, n * sizeof(uint64_t), dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+        CU(cudaMemcpy(dst, ctx->ordered_s[ctx->last_slot], n * sizeof(uint64_t), dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
     if (n && async) {
-        CU(cudaMemcpyAsync(dst, ctx->ordered, n * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->copy_stream));
+        CU(cudaMemcpyAsync(dst, ctx->ordered_s[ctx->last_slot], n * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->copy_stream));
         CU(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
         ctx->copy_pending = true;
+        ctx->copy_slot = ctx->last_slot;
     }
     if (n_out) *n_out = n;
     return ctx->last_overflow ? EVIS_ERR_OVERFLOW : EVIS_OK;
@@ -1114,7 +1137,7 @@ int evis_read_events(evis_ctx *ctx, evis_event *dst, int dst_is_device, uint64_t
     if (rc != EVIS_OK) return rc;
     uint64_t n = stored_events(ctx);
     if (n > max) n = max;
-    if (n) CU(cudaMemcpy(dst, ctx->ordered, n * sizeof(evis_event),
+    if (n) CU(cudaMemcpy(dst, ctx->ordered_s[ctx->last_slot], n * sizeof(evis_event),
                          dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
     if (n_out) *n_out = n;
     return ctx->last_overflow ? EVIS_ERR_OVERFLOW : EVIS_OK;
@@ -1132,9 +1155,10 @@ int evis_read_events_begin(evis_ctx *ctx, evis_event *host_dst, uint64_t max, ui
     uint64_t n = stored_events(ctx);
     if (n > max) n = max;
     if (n) {
-        CU(cudaMemcpyAsync(host_dst, ctx->ordered, n * sizeof(evis_event), cudaMemcpyDeviceToHost, ctx->copy_stream));
+        CU(cudaMemcpyAsync(host_dst, ctx->ordered_s[ctx->last_slot], n * sizeof(evis_event), cudaMemcpyDeviceToHost, ctx->copy_stream));
         CU(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
         ctx->copy_pending = true;
+        ctx->copy_slot = ctx->last_slot;
     }
     if (n_out) *n_out = n;
     return ctx->last_overflow ? EVIS_ERR_OVERFLOW : EVIS_OK;
@@ -1150,6 +1174,53 @@ int evis_read_events_end(evis_ctx *ctx)
     return EVIS_OK;
 }
 
+int evis_read_events_enqueue(evis_ctx *ctx, void *pinned_dst, uint64_t max, int previous_step)
+{
+    if (!ctx || !pinned_dst) return EVIS_ERR_INVALID_ARG;
+    if (!ctx->have_events || (ctx->vox_on && !ctx->vox.keep_events)) return EVIS_ERR_BAD_STATE;
+    // the step before the last: its stream lives in the other half of the doubled buffer (needs the overlap: EVIS_NO_OVERLAP
+    // keeps one buffer), and there must be such a step
+    if (previous_step && (ctx->ordered_s[0] == ctx->ordered_s[1] || ctx->steps < 3 || ctx->graph_mode)) return EVIS_ERR_BAD_STATE;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    cudaPointerAttributes at;                      // page-locked memory only: a pageable destination would make the copy synchronous
+    if (cudaPointerGetAttributes(&at, pinned_dst) != cudaSuccess || at.type != cudaMemoryTypeHost) {
+        cudaGetLastError();
+        return EVIS_ERR_INVALID_ARG;
+    }
+    if (ctx->copy_pending) { CU(cudaStreamSynchronize(ctx->copy_stream)); ctx->copy_pending = false; }
+    const int sl = previous_step ? ctx->last_slot ^ 1 : ctx->last_slot;
+    // wait for THAT step's ordering stage only (not for the steps enqueued after it), then its counts are on the host
+    if (ctx->ord_pending[sl]) CU(cudaEventSynchronize(ctx->ev_order[sl]));
+    const unsigned long long *hc = ctx->h_copy + evis_ctx::H_SLOT + sl * evis_ctx::H_SLOT_WORDS;
+    const unsigned long long made = ctx->steps < 2 ? 0ull : hc[C_EVENTS];
+    const bool lost = ctx->steps >= 2 && hc[C_ALLOC] > ctx->arrival_cap;
+    uint64_t n = lost ? 0ull : (made < ctx->cfg.event_capacity ? made : ctx->cfg.event_capacity);
+    if (n > max) n = max;
+    if (n) CU(cudaMemcpyAsync(pinned_dst, ctx->ordered_s[sl], n * (ctx->compact ? sizeof(uint64_t) : sizeof(evis_event)),
+                              cudaMemcpyDeviceToHost, ctx->copy_stream));
+    CU(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
+    ctx->copy_pending = true;
+    ctx->copy_slot = sl;
+    ctx->deferred = true;
+    ctx->h_copy[0] = n;
+    ctx->h_copy[1] = lost ? 2ull : (made > ctx->cfg.event_capacity ? 1ull : 0ull);
+    return EVIS_OK;
+}
+
+int evis_read_events_finish(evis_ctx *ctx, uint64_t *n_out)
+{
+    if (!ctx) return EVIS_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    if (!guard.ok) return EVIS_ERR_CUDA;
+    if (!ctx->deferred) return EVIS_ERR_BAD_STATE;      // no _enqueue to finish
+    if (ctx->copy_pending) CU(cudaStreamSynchronize(ctx->copy_stream));
+    ctx->copy_pending = false;
+    ctx->deferred = false;
+    if (n_out) *n_out = ctx->h_copy[0];
+    return ctx->h_copy[1] ? EVIS_ERR_OVERFLOW : EVIS_OK;
+}
+
 int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_stored)
 {
     if (!ctx || !dev_ptr || !n_stored) return EVIS_ERR_INVALID_ARG;
@@ -1157,7 +1228,7 @@ int evis_events_device(evis_ctx *ctx, const evis_event **dev_ptr, uint64_t *n_st
     DeviceGuard guard(ctx->cfg.device);
     const int rc = fetch_counters(ctx);
     if (rc != EVIS_OK) return rc;
-    *dev_ptr = reinterpret_cast<const evis_event *>(ctx->ordered);
+    *dev_ptr = reinterpret_cast<const evis_event *>(ctx->ordered_s[ctx->last_slot]);
     *n_stored = stored_events(ctx);
     return ctx->last_overflow ? EVIS_ERR_OVERFLOW : EVIS_OK;
 }

@@ -1250,6 +1250,73 @@ def test_async_step_host_equals_the_device_path():
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("compact,envs", [(True, 6), (False, 6), (True, 24)])
+def test_deferred_event_read_is_the_stream_of_every_step(compact, envs):
+    """evis_read_events_enqueue(previous_step) / _finish: the stream of step k - 1 is read after step k has been enqueued,
+    waiting only for step k - 1 (upload, kernels and download of three consecutive steps in flight together; the ordered
+    stream is double-buffered).  Every step's stream must be byte for byte the one the synchronous read call of a twin
+    context returns (16-byte and 8-byte events; 24 envs at 346 x 260 = four z-buffer regions), the host buffers scribbled as
+    the asynchronous step_host contract allows; the error contract on the side."""
+    spec = scenes.small(scenes.config(4), num_envs=envs, num_keyframes=7, **({} if envs == 24 else dict(height=120, width=160)))
+    sc = scenes.make_scene(spec)
+    E, H, W, S = spec.num_envs, spec.height, spec.width, spec.substeps
+    mk = lambda: binding.Evis(E, H, W, S, spec.c_pos, spec.c_neg, spec.log_eps, spec.keyframe_dt,
+                              max_motion_px=spec.max_motion_px(), event_capacity=1 << 24)
+    a, b = mk(), mk()
+    if compact:
+        a.set_compact_events(True); b.set_compact_events(True)
+    read_a = a.read_events8 if compact else a.read_events
+    kfs = [scenes.render_keyframe(sc, k, device="cuda") for k in range(spec.num_keyframes)]
+    want = []
+    for kf in kfs:
+        a.step(kf["rad"], kf["mv_bwd"], kf["depth"], mv_fwd=kf["mv_fwd"], sync=True)
+        want.append(read_a().copy())
+    want = want[1:]
+    assert sum(len(x) for x in want) > 5000
+    host = [{k: v.cpu().pin_memory() for k, v in kf.items()} for kf in kfs]
+    cap = max(len(x) for x in want) + 7
+    dt = np.uint64 if compact else binding.EVENT_DTYPE
+    bufs = [torch.empty(cap * dt().itemsize if compact else cap * 16, dtype=torch.uint8).pin_memory() for _ in range(2)]
+    arrs = [bb.numpy().view(dt) for bb in bufs]
+    with pytest.raises(binding.EvisError) as ei:               # nothing to read yet
+        b.read_events_enqueue(arrs[0])
+    assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+    got = []
+    for k, h in enumerate(host):
+        b.step_host(h["rad"], h["mv_bwd"], h["depth"], h["mv_fwd"], sync=False)
+        if k >= 1:
+            for key in host[k - 1]:                           # the previous call's buffers are free now
+                host[k - 1][key].fill_(float("nan"))
+        if k == 1:
+            with pytest.raises(binding.EvisError) as ei:      # one interval closed: there is no step before the last yet
+                b.read_events_enqueue(arrs[0], previous_step=True)
+            assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+            with pytest.raises(binding.EvisError) as ei:      # nothing enqueued yet
+                b.read_events_finish()
+            assert ei.value.status == binding.EVIS_ERR_BAD_STATE
+            with pytest.raises(binding.EvisError) as ei:      # pageable memory is refused
+                b.read_events_enqueue(np.empty(cap, dt))
+            assert ei.value.status == binding.EVIS_ERR_INVALID_ARG
+        if k >= 3:                                            # collect step k - 2, whose copy was started a step ago
+            got.append(arrs[k & 1][:b.read_events_finish()].copy())
+            arrs[k & 1][:] = np.zeros(1, dt)[0]
+        if k >= 2:                                            # step k is enqueued and running: start the copy of step k - 1
+            b.read_events_enqueue(arrs[(k - 1) & 1], previous_step=True)
+    got.append(arrs[(len(host) - 2) & 1][:b.read_events_finish()].copy())
+    b.read_events_enqueue(arrs[(len(host) - 1) & 1])          # the last step itself
+    got.append(arrs[(len(host) - 1) & 1][:b.read_events_finish()].copy())
+    assert len(got) == len(want)
+    for x, y in zip(want, got):
+        assert len(x) == len(y) and x.tobytes() == y.tobytes()
+    # a buffer smaller than the step: the first `max` events; the counters are those of the synchronous calls
+    small = arrs[0][:1001]
+    b.read_events_enqueue(small)
+    assert b.read_events_finish() == 1001 and small.tobytes() == want[-1][:1001].tobytes()
+    assert b.info().total_events == a.info().total_events
+    a.destroy(); b.destroy()
+
+
+@pytest.mark.gpu
 @pytest.mark.parametrize("kw", [{"defocus": 0.5}, {"mode": 2}, {"mode": 2, "tau_r": 5e-4}])
 def test_new_features_on_concurrent_regions(kw):
     """Defocus and the weighted splat with 9 envs at cfg 4's full 346x260 resolution: one env per chunk, four concurrent
