@@ -34,22 +34,47 @@ ALGO_BYTES_PER_EVENT = 16
 FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 ISSUE_PEAK = 148 * 4 * 32 * 1.965e9   # thread-instructions/s: SMs x schedulers x lanes x clocks.max.sm
 SURVEY_INSTR_BOUNDS = (60.0, 150.0)   # algorithmic estimate of issued instructions per pixel-substep
-# whole-step counters of a committed ncu capture (profiles/round2_a_range_cfg4.md says how it was made): the range is
-# RANGE_STEPS steps of RANGE_WORKLOAD.  Instruction counts do not depend on the schedule; the DRAM bytes of that capture
-# do (ncu serialises the streams), so they are reported as what they are.
-RANGE_CAPTURE = os.path.join("profiles", "round2_a_range_cfg4.csv")
+# Committed ncu captures the line quotes (profiles/*.md say how each was made).  They are constants of a build, not
+# measurements of this run: each names the git head and the hash of paper_2607_08098_b200/csrc it was taken on and the
+# events per step of ITS steps; `stale` is set when the tree's kernels differ from the capture's, and the ratio
+# traffic / algorithmic is formed with the capture's own algorithmic bytes.
+RANGE_CAPTURE = os.path.join("profiles", "round2_a_range_cfg4.csv")      # instruction counts (schedule-independent)
 RANGE_WORKLOAD, RANGE_STEPS = "cfg4_256env_346x260_S16_rl", 5
+RANGE_CSRC_SHA = "6931bcd6ccdd"
+GRAPH_CAPTURES = {      # workload -> whole steps as CUDA graphs (`ncu --graph-profiling graph`, bench.py --graph-probe)
+    "cfg4_256env_346x260_S16_rl": {"file": os.path.join("profiles", "round3_b_graph_cfg4.csv"), "doc": "profiles/round3_b_graph_cfg4.md",
+                                   "git_head": "0f0284c", "csrc_sha": "0afb0723d1b1", "events_per_step": None},
+    "cfg2_16env_640x480_S16": {"file": os.path.join("profiles", "round2_h_graph_cfg2.csv"), "doc": "profiles/round2_h_graph_cfg2_cfg3.md",
+                               "git_head": "120e9a6", "csrc_sha": "6931bcd6ccdd", "events_per_step": 10.3e6},
+    "cfg3_64env_1280x720_S33_disk": {"file": os.path.join("profiles", "round2_h_graph_cfg3.csv"), "doc": "profiles/round2_h_graph_cfg2_cfg3.md",
+                                "git_head": "120e9a6", "csrc_sha": "6931bcd6ccdd", "events_per_step": 88.0e6},
+}
+
+
+def csrc_sha() -> str:
+    """Hash of the kernel sources in the tree (names and contents of csrc/*.cu, *.cuh, *.h), to tell whether a committed
+    capture still describes this build."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2607_08098_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".h")):
+            h.update(f.encode())
+            with open(os.path.join(d, f), "rb") as fh:
+                h.update(fh.read())
+    return h.hexdigest()[:12]
 
 
 def step_traffic(workload: str):
-    """DRAM bytes (read + write) of ONE WHOLE STEP in the schedule the bench runs: mean over the graph launches of the
-    committed `ncu --graph-profiling graph` capture (profiles/round2_f_graph_cfg4.md), or None for another workload."""
-    if workload != RANGE_WORKLOAD:
-        return None
+    """(DRAM bytes read + written of ONE WHOLE STEP in the schedule the bench runs, capture record) from the committed
+    `ncu --graph-profiling graph` capture of `workload`: the mean over its graph launches; (None, None) without one."""
+    meta = GRAPH_CAPTURES.get(workload)
+    if not meta:
+        return None, None
     try:
         import csv
         rd, wr = [], []
-        with open(os.path.join(ROOT, "profiles", "round2_f_graph_cfg4.csv")) as f:
+        with open(os.path.join(ROOT, meta["file"])) as f:
             for row in csv.reader(f):
                 if len(row) >= 15 and row[4] == "graph":
                     if row[12] == "dram__bytes_read.sum":
@@ -57,10 +82,11 @@ def step_traffic(workload: str):
                     elif row[12] == "dram__bytes_write.sum":
                         wr.append(float(row[14].replace(",", "")))
         if not rd or len(rd) != len(wr):
-            return None
-        return (sum(rd) + sum(wr)) / len(rd)
+            return None, None
+        rec = dict(meta, steps=len(rd), stale=meta["csrc_sha"] != csrc_sha())
+        return (sum(rd) + sum(wr)) / len(rd), rec
     except (OSError, ValueError):
-        return None
+        return None, None
 
 
 def range_capture(workload: str):
@@ -367,18 +393,28 @@ def run_ours(args, spec) -> None:
     achieved = algo_bytes_step / step_s / 1e9
     pxss_step = E * H * W * S
     cap_ = range_capture(spec.name)
+    traffic, trec = step_traffic(spec.name)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": step_traffic(spec.name),
-                "traffic_note": "DRAM bytes of one WHOLE step in its real multi-stream schedule: the step captured as one CUDA graph "
-                "and measured by `ncu --graph-profiling graph` (profiles/round2_f_graph_cfg4.md; steps with ~130 M events, "
-                "3.3 GB algorithmic)",
+                "traffic": traffic,
                 "algorithmic_bytes_per_step": algo_bytes_step, "basis": "whole step: algorithmic bytes / ms_per_step",
                 "dominant_stage_ms": stage_ms[dom], "dominant_stage_launches_per_step": max(1.0, prof["launches"][dom] / K),
                 "stage_ms_per_step": stage_ms, "stage_launches_per_step": {k: v / K for k, v in prof["launches"].items()}}
+    if trec:
+        # the capture's own steps decide its algorithmic bytes (the same steps as this run's when events_per_step is None:
+        # the capture was then taken with this command's --steps / --warmup on the same seeded keyframes)
+        cap_events = trec["events_per_step"] if trec["events_per_step"] is not None else ev_per_step
+        cap_algo = ALGO_BYTES_PER_PIXEL * E * H * W + ALGO_BYTES_PER_EVENT * cap_events
+        roofline["traffic_capture"] = {
+            "what": "DRAM bytes of one WHOLE step in its real multi-stream schedule: every step captured as one CUDA graph and "
+                    "measured by `ncu --graph-profiling graph` (a committed capture, not this run)",
+            "file": trec["file"], "doc": trec["doc"], "git_head": trec["git_head"], "csrc_sha": trec["csrc_sha"],
+            "stale": trec["stale"], "steps": trec["steps"], "events_per_step": cap_events,
+            "algorithmic_bytes_per_step": cap_algo, "traffic_over_algorithmic": traffic / cap_algo}
     if cap_ and "smsp__inst_executed.sum" in cap_:
         ipp = cap_["smsp__inst_executed.sum"] * 32.0 / pxss_step           # issue slots (thread-instructions) per pixel-substep
         roofline["capture"] = {"file": RANGE_CAPTURE, "steps": RANGE_STEPS, "schedule": "serialised by ncu",
+                               "csrc_sha": RANGE_CSRC_SHA, "stale": RANGE_CSRC_SHA != csrc_sha(),
                                "warp_instructions_per_step": cap_["smsp__inst_executed.sum"],
                                "dram_bytes_per_step": cap_.get("dram__bytes_read.sum", 0.0) + cap_.get("dram__bytes_write.sum", 0.0),
                                "l2_red_sectors_per_step": cap_.get("lts__t_sectors_op_red.sum")}

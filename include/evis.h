@@ -14,6 +14,24 @@
  * Motion vectors are in pixels: mv_bwd[p] is the displacement from pixel p of this keyframe to
  * the same surface point in the PREVIOUS keyframe.
  *
+ * Environment variables read by evis_create (test and measurement hooks; none is needed in production, every default
+ * is the measured best):
+ *   EVIS_ZBUF_MB=<n>     budget of one z-buffer region in MiB (default 24 when an env's S substeps fit, else 512 / regions)
+ *   EVIS_STREAMS=<n>     concurrent z-buffer regions / streams (default 4, or 2 for very large frames; at most 8)
+ *   EVIS_CHUNK_NI=<n>, EVIS_CHUNK_NE=<n>   explicit chunk shape in substeps / envs (experiments)
+ *   EVIS_NO_ZTAG=1       untagged 64-bit keys, z-buffers cleared before every chunk (the path frames > 2^24 pixels take)
+ *   EVIS_NO_TMA=1        the resolve kernel loads keys directly instead of staging them by TMA
+ *   EVIS_NO_OVERLAP=1    the ordering stage of a step is not overlapped with the next step (single buffers)
+ *   EVIS_GRAPH=1         every evis_step is captured and launched as one CUDA graph (for `ncu --graph-profiling graph`;
+ *                        the steps are serialised: no throughput claim)
+ * (EVIS_NVCC_EXTRA is read by the build script, not by the library: extra nvcc flags for experiments.)
+ *
+ * Checkpoint / resume: evis_get_state / evis_set_state carry L_ref and L_prev, evis_refractory_state the refractory stamps,
+ * evis_set_interval_index the interval counter.  Two pieces of state are NOT exposed: the carried unblurred frame of the
+ * defocus path (a resumed context rebuilds it from keyframe A, so pixels that were holding an older value through a hole
+ * or invalid depth can differ until they are reached again) and the position inside a voxel window (resume at a window
+ * boundary, or read the grid first).
+ *
  * Threading: a context may be used by one host thread at a time.  No function throws or aborts;
  * every function returns an evis_status (0 = OK, negative = error).
  */

@@ -37,8 +37,15 @@ def test_bench_reads_the_committed_captures():
     cap = bench.range_capture(bench.RANGE_WORKLOAD)
     assert cap and 2.0e9 < cap["smsp__inst_executed.sum"] < 4.0e9          # warp-instructions per cfg 4 step
     assert cap["dram__bytes_read.sum"] > 1e9
-    tr = bench.step_traffic(bench.RANGE_WORKLOAD)
+    tr, rec = bench.step_traffic(bench.RANGE_WORKLOAD)
     assert tr and 5.0e9 < tr < 3.0e10                                       # one whole step: ~11 GB
-    assert bench.range_capture("cfg2_16env_640x480_S16") is None and bench.step_traffic("other") is None
+    # the capture names the build it was taken on; `stale` compares that with the kernels in the tree
+    assert rec["steps"] >= 2 and len(rec["csrc_sha"]) == 12 and rec["stale"] == (rec["csrc_sha"] != bench.csrc_sha())
+    for w in ("cfg2_16env_640x480_S16", "cfg3_64env_1280x720_S33_disk"):
+        t2, r2 = bench.step_traffic(w)
+        assert t2 > 1e9 and r2["events_per_step"] > 1e6
+    assert bench.range_capture("cfg2_16env_640x480_S16") is None and bench.step_traffic("other") == (None, None)
+    from paper_2607_08098_b200 import scenes
+    assert {scenes.config(c).name for c in (2, 3, 4)} == set(bench.GRAPH_CAPTURES)
     peak, src = bench.hbm_peak()
     assert 3000.0 < peak < 9000.0 and src
