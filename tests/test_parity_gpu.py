@@ -207,6 +207,31 @@ def test_config5_sweep_shapes_reduced(point):
     assert rep.events_oracle > 0
 
 
+@pytest.mark.parametrize("point,n_kf", [(3, 2), (14, 3), (17, 3)])
+def test_config5_full_size_sampled_envs(point, n_kf):
+    """BASELINE.json config 5 at its REAL shapes (north_star: "oracle-matching events for all five configs"): three sweep
+    points -- 1 env at 1920x1080 with S = 166, 256 envs at 160x120 with S = 33, 1024 envs at 128x128 with S = 16 -- in the
+    launch configuration the sweep runs (PATH_AUTO, default regions and streams).  The GPU runs the whole batch, the oracle
+    the first, the middle and the last env (envs are independent); events, stamps and carried state of those envs must
+    match as in the reduced cases."""
+    spec = scenes.small(scenes.sweep_points()[point], num_keyframes=n_kf)
+    assert (spec.num_envs, spec.height, spec.width, spec.substeps) in ((1, 1080, 1920, 166), (256, 120, 160, 33), (1024, 128, 128, 16))
+    envs = sorted({0, spec.num_envs // 2, spec.num_envs - 1})
+    cap = int(min(0x7FFFFFFF, 10 * spec.num_envs * spec.height * spec.width))
+    rep = parity.run_parity(spec, n_kf, envs=envs, path=binding.PATH_AUTO, debug=False, capacity=cap)
+    _assert_tolerances(rep)
+
+
+def test_winners_at_full_resolution_on_concurrent_regions():
+    """Splat winners (source index and direction per pixel-substep) compared with the oracle at cfg 4's full 346 x 260
+    resolution with 9 envs: one env per chunk, four concurrent z-buffer regions on four streams -- the launch configuration
+    the bench times, where the full-size tests above compare events and state only (debug capture off)."""
+    spec = scenes.small(scenes.config(4), num_envs=9, num_keyframes=3)
+    rep = parity.run_parity(spec, 3, envs=[0, 4, 8], path=binding.PATH_AUTO, debug=True, capacity=1 << 24)
+    _assert_tolerances(rep)
+    assert rep.events_oracle > 10000
+
+
 def test_threshold_maps_eq8():
     """Threshold mismatch (Eq. 8): per-pixel theta_ON / theta_OFF maps drawn as
     max(N(C, sigma^2), theta_min) by the seeded generator; events, counts, L_ref and timestamps must match the
