@@ -73,7 +73,7 @@ def step_traffic(workload: str):
         return None, None
     try:
         import csv
-        rd, wr = [], []
+        rd, wr, inst = [], [], []
         with open(os.path.join(ROOT, meta["file"])) as f:
             for row in csv.reader(f):
                 if len(row) >= 15 and row[4] == "graph":
@@ -81,9 +81,12 @@ def step_traffic(workload: str):
                         rd.append(float(row[14].replace(",", "")))
                     elif row[12] == "dram__bytes_write.sum":
                         wr.append(float(row[14].replace(",", "")))
+                    elif row[12] == "smsp__inst_executed.sum":
+                        inst.append(float(row[14].replace(",", "")))
         if not rd or len(rd) != len(wr):
             return None, None
-        rec = dict(meta, steps=len(rd), stale=meta["csrc_sha"] != csrc_sha())
+        rec = dict(meta, steps=len(rd), stale=meta["csrc_sha"] != csrc_sha(),
+                   warp_instructions_per_step=sum(inst) / len(inst) if len(inst) == len(rd) else None)
         return (sum(rd) + sum(wr)) / len(rd), rec
     except (OSError, ValueError):
         return None, None
@@ -412,13 +415,17 @@ def run_ours(args, spec) -> None:
             "stale": trec["stale"], "steps": trec["steps"], "events_per_step": cap_events,
             "algorithmic_bytes_per_step": cap_algo, "traffic_over_algorithmic": traffic / cap_algo}
     if cap_ and "smsp__inst_executed.sum" in cap_:
-        ipp = cap_["smsp__inst_executed.sum"] * 32.0 / pxss_step           # issue slots (thread-instructions) per pixel-substep
+        # instructions of the step: from the graph capture of these very steps when it has them, else the older range capture
+        winst, isrc = cap_["smsp__inst_executed.sum"], RANGE_CAPTURE
+        if trec and trec.get("warp_instructions_per_step"):
+            winst, isrc = trec["warp_instructions_per_step"], trec["file"]
+        ipp = winst * 32.0 / pxss_step                                       # issue slots (thread-instructions) per pixel-substep
         roofline["capture"] = {"file": RANGE_CAPTURE, "steps": RANGE_STEPS, "schedule": "serialised by ncu",
                                "csrc_sha": RANGE_CSRC_SHA, "stale": RANGE_CSRC_SHA != csrc_sha(),
                                "warp_instructions_per_step": cap_["smsp__inst_executed.sum"],
                                "dram_bytes_per_step": cap_.get("dram__bytes_read.sum", 0.0) + cap_.get("dram__bytes_write.sum", 0.0),
                                "l2_red_sectors_per_step": cap_.get("lts__t_sectors_op_red.sum")}
-        roofline["issue_roof"] = {"bound": "alu", "unit": "thread-instr/s", "peak": ISSUE_PEAK, "derived_from": RANGE_CAPTURE,
+        roofline["issue_roof"] = {"bound": "alu", "unit": "thread-instr/s", "peak": ISSUE_PEAK, "derived_from": isrc,
                                   "instr_per_pixel_substep": ipp, "achieved": ipp * pxss_step / step_s,
                                   "frac": ipp * pxss_step / step_s / ISSUE_PEAK,
                                   "note": "utilisation of issue slots by the kernels' own instruction stream; against "

@@ -41,6 +41,7 @@ def test_bench_reads_the_committed_captures():
     assert tr and 5.0e9 < tr < 3.0e10                                       # one whole step: ~11 GB
     # the capture names the build it was taken on; `stale` compares that with the kernels in the tree
     assert rec["steps"] >= 2 and len(rec["csrc_sha"]) == 12 and rec["stale"] == (rec["csrc_sha"] != bench.csrc_sha())
+    assert 2.0e9 < rec["warp_instructions_per_step"] < 4.0e9               # the same steps' instruction count (issue roof)
     for w in ("cfg2_16env_640x480_S16", "cfg3_64env_1280x720_S33_disk"):
         t2, r2 = bench.step_traffic(w)
         assert t2 > 1e9 and r2["events_per_step"] > 1e6
